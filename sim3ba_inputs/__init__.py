@@ -1,0 +1,8 @@
+"""Seeded synthetic Sim(3) pose-graph inputs (shared by the oracle tests and the CUDA tests).
+
+This package only *draws inputs*: scenes, keyframe poses, pointmaps, confidences, edge lists and
+pixel-match maps shaped like the five workloads of BASELINE.json.  It
+contains none of the method's arithmetic (no residual, Jacobian, normal equations, Sim(3) Exp/Log,
+solve) and imports neither ``oracle/`` nor the CUDA package.
+"""
+from .graphs import CONFIGS, Graph, GraphSpec, make_graph, make_config, PRESETS  # noqa: F401
