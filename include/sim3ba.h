@@ -1,0 +1,166 @@
+/*
+ * sim3ba.h - C ABI of libsim3ba: the Gauss-Newton step of the unified multi-agent Sim(3) pose graph
+ * over dense pointmap correspondences (CoMo3R-SLAM, arxiv 2605.30488, section III-D,
+ * PAPER.md:106-122), hand-written CUDA for sm_100a (B200).
+ *
+ * Conventions
+ *   - Pose of keyframe i: T_WCi : X -> s_i R_i X + t_i, stored as 8 doubles
+ *     (tx, ty, tz, qx, qy, qz, qw, s), q a unit quaternion.
+ *   - Tangent vector tau_i = (v, omega, zeta) in R^7; update T <- Exp(tau) T.
+ *   - N keyframes, HW = height*width pixels per keyframe, E directed edges, n = 7N.
+ *   - "d_" arguments are DEVICE pointers, "h_" arguments are HOST pointers.
+ *   - Every function returns SIM3BA_OK (0) or a negative sim3ba_status; nothing throws or aborts
+ *     across this boundary.  sim3ba_last_error() gives a human-readable message for the last
+ *     failure on that context (or for a failed create when ctx == NULL).
+ *   - All work is enqueued on the stream given at create; functions taking host pointers
+ *     synchronise that stream before returning, the others do not unless stated.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point fails with
+ *     SIM3BA_ERR_CUDA.
+ */
+#ifndef SIM3BA_H_
+#define SIM3BA_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sim3ba_ctx sim3ba_ctx; /* opaque, owned by the library */
+
+typedef enum {
+  SIM3BA_OK = 0,
+  SIM3BA_ERR_INVALID_ARG = -1,
+  SIM3BA_ERR_CUDA = -2,
+  SIM3BA_ERR_ALLOC = -3,
+  SIM3BA_ERR_BAD_STATE = -4
+} sim3ba_status;
+
+/* Robust-kernel and solver constants.  PAPER.md:76,177: Sigma = diag(sigma_r^2 I3, sigma_d^2),
+ * sigma_r = 0.003, sigma_d = 10, Huber breakpoint kappa = 1.345 on the whitened residual
+ * r_c = sqrt(q) e_c / sigma_c, IRLS weight w = min(1, kappa/|r_c|).  PAPER.md:120-122: Eq. (7)
+ * (H + lambda diag(H) + eps_r I) tau = -g, eps_r = eps0 * 100^r, r = 0..max_attempts-1
+ * (paper: eps0 = 1e-6, six attempts), zero update when all attempts fail. */
+typedef struct {
+  float sigma_ray;   /* sigma_r  > 0 */
+  float sigma_dist;  /* sigma_d  > 0 */
+  float huber_k;     /* kappa    > 0 */
+  float conf_min;    /* a match (m,n) is valid iff 0 <= n < HW, c_i[m] > conf_min, c_j[n] > conf_min */
+  double lm_lambda;  /* lambda >= 0; global backend: 0 (Gauss-Newton) */
+  double eps0;       /* eps_0 >= 0 */
+  int32_t max_attempts; /* 1..16 */
+  int32_t reserved;
+} sim3ba_params;
+
+/* Fills *p with the paper's constants (0.003, 10, 1.345, conf_min 0, lambda 0, 1e-6, 6). */
+int sim3ba_default_params(sim3ba_params* p);
+
+/* Creates a context for one graph (vertices = keyframe poses in one flat index
+ * space, edges with dense matches, validity masks and endpoint confidences).
+ *   d_points  [N][HW][3] float32, canonical pointmap of each keyframe in its own camera frame
+ *   d_conf    [N][HW]    float32, per-pixel confidence (q_mn = sqrt(c_i[m] c_j[n]))
+ *   d_edges   [E][2]     int32 (i, j): the match map is dense over the pixels m of i, X_j[n] is
+ *                        mapped into camera i by T_ij = T_WCi^-1 T_WCj (Eq. (1))
+ *   d_match   [E][HW]    int32, pixel m of i -> pixel n of j; n < 0 or n >= HW means "no match"
+ *   h_fixed_kf[n_fixed]  int32 gauge keyframes whose pose is held fixed (paper: {0})
+ * Ownership: the library copies points+conf into an internal packed float4 array and copies the
+ * edge list; d_match is BORROWED and must stay valid and unchanged until sim3ba_destroy.
+ * Poses start as identity; call sim3ba_set_poses.  Errors: i == j or endpoint outside [0,N),
+ * fixed keyframe outside [0,N), non-positive sizes or sigmas -> SIM3BA_ERR_INVALID_ARG.
+ * Synchronises the stream. */
+int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width, int32_t n_edges,
+                  const float* d_points, const float* d_conf, const int32_t* d_edges,
+                  const int32_t* d_match, const int32_t* h_fixed_kf, int32_t n_fixed,
+                  const sim3ba_params* params, void* cuda_stream);
+
+int sim3ba_destroy(sim3ba_ctx* ctx);
+
+/* Replace the robust-kernel / solver constants (takes effect at the next build/solve). */
+int sim3ba_set_params(sim3ba_ctx* ctx, const sim3ba_params* params);
+
+/* Poses [N][8] double, device pointers; asynchronous device-to-device copies. */
+int sim3ba_set_poses(sim3ba_ctx* ctx, const double* d_poses);
+int sim3ba_get_poses(sim3ba_ctx* ctx, double* d_poses);
+
+/* a1-a6 at the current poses: per-match residuals (Eq. (1)), weights, Jacobians
+ * (Eq. (6)), per-edge reduction into 7x7 blocks, scatter into the dense 7N
+ * system with the gauge keyframes' rows/columns replaced by identity and their gradient by 0.
+ * Fills the per-edge statistics and blocks and the undamped dense (H, g). */
+int sim3ba_build_system(sim3ba_ctx* ctx);
+
+/* a7 on the last built system: Eq. (7) with the epsilon escalation of PAPER.md:122 by blocked
+ * FP64 Cholesky and two triangular solves.  Requires a previous build (else BAD_STATE).
+ * "All attempts failed" is not an error: tau = 0, attempts = max_attempts.  Synchronises the
+ * stream once per attempt to read the factorisation flag. */
+int sim3ba_solve(sim3ba_ctx* ctx);
+
+/* One Gauss-Newton iteration: a1-a5, assembly of the damped system, a7, and the retraction
+ * T_i <- Exp(tau_i) T_i of every non-fixed keyframe.  (The undamped dense H of
+ * sim3ba_get_system is not refreshed by this call; the per-edge blocks and g are.) */
+int sim3ba_step(sim3ba_ctx* ctx);
+
+/* Same iteration with HOST pose buffers: copies h_poses_in [N][8] to the device (if non-NULL),
+ * runs sim3ba_step, copies the new poses to h_poses_out [N][8] and the robust cost at the input
+ * poses to *h_cost (each if non-NULL).  Pinned host memory recommended.  Synchronises. */
+int sim3ba_step_host(sim3ba_ctx* ctx, const double* h_poses_in, double* h_poses_out, double* h_cost);
+
+/* a8 only: T_i <- Exp(tau_i) T_i with the tau of the last solve. */
+int sim3ba_retract(sim3ba_ctx* ctx);
+
+/* ---- read-back for parity.  Returned DEVICE pointers are owned by the context and stay valid
+ * until the next build/solve/step/destroy on it; the caller synchronises the stream. ---- */
+
+/* n_valid [E] int32 valid matches per edge; checksum [E] uint64 = sum over the valid matches of
+ * (m*HW + n) mod 2^64; cost [E] double = sum of Huber rho over the edge's matches. */
+int sim3ba_get_edge_stats(sim3ba_ctx* ctx, const int32_t** d_n_valid, const uint64_t** d_checksum,
+                          const double** d_cost);
+
+/* blocks35 [E][35] double: the 28 upper-triangular entries (row-major, r <= c) of
+ * A_e = sum J_j^T Omega J_j followed by the 7 entries of b_e = sum J_j^T Omega e, with
+ * J_j = J_xi Ad_{T_WCi^-1}.  H_ii += A_e, H_jj += A_e, H_ij -= A_e, H_ji -= A_e,
+ * g_j += b_e, g_i -= b_e. */
+int sim3ba_get_edge_blocks(sim3ba_ctx* ctx, const double** d_blocks35);
+
+/* Undamped dense system of the last sim3ba_build_system: H column-major == row-major (symmetric),
+ * leading dimension *ld >= 7N, lower triangle (row >= col) valid, strict upper triangle zero;
+ * g [7N].  Gauge keyframes: identity diagonal block, zero off-diagonal blocks, zero gradient. */
+int sim3ba_get_system(sim3ba_ctx* ctx, const double** d_H, int32_t* ld, const double** d_g);
+
+/* tau [7N] double (device); scalars are written to host memory (synchronises the stream):
+ * attempts used (1 = first factorisation succeeded), eps of the successful attempt (NaN if none),
+ * total robust cost at the poses of the last build. */
+int sim3ba_get_update(sim3ba_ctx* ctx, const double** d_tau, int32_t* h_attempts, double* h_eps_used,
+                      double* h_cost);
+
+/* a0 bookkeeping, HOST pointers owned by the context: keyframe -> incident-edge CSR
+ * (kf_ptr [N+1], kf_edge [2E], edges ascending) and the sorted unique unordered keyframe pairs
+ * (pair_kf [P][2] = (hi, lo), pair_ptr [P+1], pair_edge [E], edges ascending). */
+int sim3ba_get_bookkeeping(sim3ba_ctx* ctx, const int32_t** h_kf_ptr, const int32_t** h_kf_edge,
+                           int32_t* n_pairs, const int32_t** h_pair_kf, const int32_t** h_pair_ptr,
+                           const int32_t** h_pair_edge);
+
+/* Overrides the system of the next sim3ba_solve with a caller-supplied dense one (decomposition
+ * tests: oracle (H, g) -> GPU solver).  d_H [7N][7N] row-major symmetric double, d_g [7N]. */
+int sim3ba_load_system(sim3ba_ctx* ctx, const double* d_H, const double* d_g);
+
+/* Number of kernels this library launched on the context since create (for bench accounting). */
+int sim3ba_get_launch_count(sim3ba_ctx* ctx, int64_t* h_count);
+
+/* Device time in milliseconds of the phases of the last sim3ba_step / build / solve, measured
+ * with CUDA events on the context's stream: [0] accumulate+reduce (a1-a5), [1] assembly (a6),
+ * [2] factor+solve (a7), [3] retraction (a8).  Synchronises.  Phase timing is only recorded
+ * after sim3ba_set_profiling(ctx, 1). */
+int sim3ba_set_profiling(sim3ba_ctx* ctx, int32_t enable);
+int sim3ba_get_phase_ms(sim3ba_ctx* ctx, float h_ms[4]);
+
+/* Binding convenience: asynchronous device-to-device copy of `bytes` bytes on the context's stream
+ * (used to move the read-back buffers above into caller-owned device memory). */
+int sim3ba_copy_d2d(sim3ba_ctx* ctx, void* d_dst, const void* d_src, uint64_t bytes);
+
+const char* sim3ba_last_error(const sim3ba_ctx* ctx);
+const char* sim3ba_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SIM3BA_H_ */

@@ -303,6 +303,7 @@ class System:
     edge_A: np.ndarray       # [E,7,7]  J_j^T Omega J_j summed (= H_jj contribution of the edge)
     edge_b: np.ndarray       # [E,7]    J_j^T Omega e summed (= g_j contribution of the edge)
     edge_cost: np.ndarray    # [E]
+    edge_b_abs: np.ndarray   # [E,7]    sum |J_j^T| Omega |e| (floor for converged iterations)
 
 
 def build_system(poses: np.ndarray, points: np.ndarray, conf: np.ndarray, edges: np.ndarray,
@@ -318,6 +319,7 @@ def build_system(poses: np.ndarray, points: np.ndarray, conf: np.ndarray, edges:
     edge_A = np.zeros((E, 7, 7))
     edge_b = np.zeros((E, 7))
     edge_cost = np.zeros(E)
+    edge_b_abs = np.zeros((E, 7))
     cost = 0.0
     for e in (range(E) if edge_subset is None else edge_subset):
         i, j = int(edges[e, 0]), int(edges[e, 1])
@@ -338,14 +340,15 @@ def build_system(poses: np.ndarray, points: np.ndarray, conf: np.ndarray, edges:
         g[si] += gi
         g[sj] += gj
         g_abs[si] += np.abs(WJi).T @ np.abs(ee)
-        g_abs[sj] += np.abs(WJj).T @ np.abs(ee)
+        edge_b_abs[e] = np.abs(WJj).T @ np.abs(ee)
+        g_abs[sj] += edge_b_abs[e]
         n_valid[e] = tm.m.shape[0]
         with np.errstate(over="ignore"):
             checksum[e] = np.sum(tm.m.astype(np.uint64) * np.uint64(HW) + tm.n.astype(np.uint64),
                                  dtype=np.uint64)
         edge_A[e], edge_b[e], edge_cost[e] = Hjj, gj, tm.cost
         cost += tm.cost
-    return System(H, g, g_abs, cost, n_valid, checksum, edge_A, edge_b, edge_cost)
+    return System(H, g, g_abs, cost, n_valid, checksum, edge_A, edge_b, edge_cost, edge_b_abs)
 
 
 def total_cost(poses, points, conf, edges, match, prm: Params) -> float:

@@ -1,0 +1,450 @@
+// C ABI of libsim3ba (include/sim3ba.h): argument checking, memory, a0 bookkeeping, and the
+// sequencing of kernels 1-5.  Host code only; every step of the hot path runs in the kernels.
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+#include <map>
+#include <new>
+#include <numeric>
+#include <utility>
+
+#include "sim3ba_internal.cuh"
+
+using namespace sim3ba;
+
+struct sim3ba_ctx {
+  Ctx c;
+};
+
+namespace {
+
+thread_local std::string g_create_error;
+
+int fail(Ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg; else g_create_error = msg;
+  return code;
+}
+
+int cuda_fail(Ctx* c, cudaError_t e, const char* what) {
+  return fail(c, SIM3BA_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define CU(call)                                              \
+  do {                                                        \
+    cudaError_t e_ = (call);                                  \
+    if (e_ != cudaSuccess) return cuda_fail(c, e_, #call);    \
+  } while (0)
+
+template <class T>
+cudaError_t dev_alloc(T** p, size_t count) {
+  return cudaMalloc(reinterpret_cast<void**>(p), std::max<size_t>(count, 1) * sizeof(T));
+}
+
+bool params_ok(const sim3ba_params* p) {
+  return p && p->sigma_ray > 0.f && p->sigma_dist > 0.f && p->huber_k > 0.f && p->lm_lambda >= 0.0 &&
+         p->eps0 >= 0.0 && p->max_attempts >= 1 && p->max_attempts <= 16 && isfinite(p->sigma_ray) &&
+         isfinite(p->sigma_dist) && isfinite(p->huber_k) && isfinite(p->conf_min);
+}
+
+// a0: keyframe -> incident-edge CSR, unique unordered pairs -> edge CSR, processing order.
+void build_bookkeeping(Ctx* c) {
+  const int N = c->N, E = c->E;
+  const std::vector<int32_t>& ed = c->h_edges;
+  c->h_kf_ptr.assign(N + 1, 0);
+  for (int e = 0; e < E; ++e) { ++c->h_kf_ptr[ed[2 * e] + 1]; ++c->h_kf_ptr[ed[2 * e + 1] + 1]; }
+  for (int k = 0; k < N; ++k) c->h_kf_ptr[k + 1] += c->h_kf_ptr[k];
+  c->h_kf_edge.assign(2 * (size_t)E, 0);
+  std::vector<int32_t> cur(c->h_kf_ptr.begin(), c->h_kf_ptr.end() - 1);
+  for (int e = 0; e < E; ++e) {  // ascending e inside every keyframe's list
+    c->h_kf_edge[cur[ed[2 * e]]++] = e;
+    c->h_kf_edge[cur[ed[2 * e + 1]]++] = e;
+  }
+  std::map<std::pair<int32_t, int32_t>, std::vector<int32_t>> pairs;  // key (hi, lo), sorted
+  for (int e = 0; e < E; ++e) {
+    const int32_t a = ed[2 * e], b = ed[2 * e + 1];
+    pairs[{std::max(a, b), std::min(a, b)}].push_back(e);
+  }
+  c->n_pairs = (int)pairs.size();
+  c->h_pair_kf.clear(); c->h_pair_ptr.assign(1, 0); c->h_pair_edge.clear();
+  for (const auto& kv : pairs) {
+    c->h_pair_kf.push_back(kv.first.first);
+    c->h_pair_kf.push_back(kv.first.second);
+    for (int32_t e : kv.second) c->h_pair_edge.push_back(e);
+    c->h_pair_ptr.push_back((int32_t)c->h_pair_edge.size());
+  }
+}
+
+template <class T>
+cudaError_t upload(T** dst, const std::vector<T>& src, cudaStream_t s) {
+  cudaError_t e = dev_alloc(dst, src.size());
+  if (e != cudaSuccess || src.empty()) return e;
+  return cudaMemcpyAsync(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice, s);
+}
+
+void free_all(Ctx* c) {
+  cudaFree(c->pm); cudaFree(c->edges); cudaFree(c->sched); cudaFree(c->fixed_mask); cudaFree(c->poses);
+  cudaFree(c->kf_ptr); cudaFree(c->kf_edge); cudaFree(c->pair_kf); cudaFree(c->pair_ptr); cudaFree(c->pair_edge);
+  cudaFree(c->partials); cudaFree(c->blocks35); cudaFree(c->edge_cost); cudaFree(c->n_valid); cudaFree(c->checksum);
+  cudaFree(c->Hd); cudaFree(c->L); cudaFree(c->g); cudaFree(c->rhs); cudaFree(c->ysol); cudaFree(c->Dfac);
+  cudaFree(c->tau); cudaFree(c->total_cost); cudaFree(c->fail_flag);
+  if (c->h_flag) cudaFreeHost(c->h_flag);
+  if (c->h_scalar) cudaFreeHost(c->h_scalar);
+  for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
+}
+
+inline void mark(Ctx* c, int i) { if (c->profiling) cudaEventRecord(c->ev[i], c->stream); }
+
+// a1-a5 (+ gradient and total cost): the block-sparse system at the current poses
+int build_blocks(Ctx* c) {
+  CU(launch_accumulate(c));
+  CU(launch_gradient(c));
+  c->built = true; c->solved = false; c->dense_loaded = false;
+  return SIM3BA_OK;
+}
+
+// a6 (damped, into L) + a7 with the escalation of PAPER.md:122
+int solve_impl(Ctx* c) {
+  c->attempts = 0; c->eps_used = NAN;
+  bool ok = false;
+  float asm_ms = 0.f, fac_ms = 0.f;
+  for (int r = 0; r < c->prm.max_attempts; ++r) {
+    const double eps = c->prm.eps0 * pow(100.0, (double)r);
+    mark(c, 1);
+    CU(launch_assemble(c, c->L, c->prm.lm_lambda, eps, c->dense_loaded));
+    mark(c, 2);
+    CU(launch_factor_solve(c));
+    mark(c, 3);
+    CU(cudaMemcpyAsync(c->h_flag, c->fail_flag, sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (c->profiling) {
+      float a = 0.f, f = 0.f;
+      cudaEventElapsedTime(&a, c->ev[1], c->ev[2]);
+      cudaEventElapsedTime(&f, c->ev[2], c->ev[3]);
+      asm_ms += a; fac_ms += f;
+    }
+    c->attempts = r + 1;
+    if (*c->h_flag == 0) { ok = true; c->eps_used = eps; break; }
+  }
+  if (c->profiling) { c->phase_ms[1] = asm_ms; c->phase_ms[2] = fac_ms; }
+  if (!ok) CU(cudaMemsetAsync(c->tau, 0, (size_t)c->npad * sizeof(double), c->stream));  // zero update
+  c->solved = true;
+  return SIM3BA_OK;
+}
+
+}  // namespace
+
+#pragma GCC visibility push(default)
+extern "C" {
+
+int sim3ba_default_params(sim3ba_params* p) {
+  if (!p) return SIM3BA_ERR_INVALID_ARG;
+  p->sigma_ray = 0.003f; p->sigma_dist = 10.0f; p->huber_k = 1.345f; p->conf_min = 0.0f;
+  p->lm_lambda = 0.0; p->eps0 = 1e-6; p->max_attempts = 6; p->reserved = 0;
+  return SIM3BA_OK;
+}
+
+int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width, int32_t n_edges,
+                  const float* d_points, const float* d_conf, const int32_t* d_edges, const int32_t* d_match,
+                  const int32_t* h_fixed_kf, int32_t n_fixed, const sim3ba_params* params, void* cuda_stream) {
+  Ctx* c = nullptr;
+  if (!out) return fail(c, SIM3BA_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  if (n_kf <= 0 || height <= 0 || width <= 0 || n_edges < 0 || n_fixed < 0 || (int64_t)height * width > (1 << 30) ||
+      (int64_t)n_kf * 7 > (1 << 20))
+    return fail(c, SIM3BA_ERR_INVALID_ARG, "non-positive or oversized dimensions");
+  if (!d_points || !d_conf || (n_edges > 0 && (!d_edges || !d_match)) || (n_fixed > 0 && !h_fixed_kf))
+    return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL input pointer");
+  if (!params_ok(params)) return fail(c, SIM3BA_ERR_INVALID_ARG, "invalid params (sigmas, kappa > 0; lambda, eps0 >= 0; 1 <= attempts <= 16)");
+  int ndev = 0;
+  cudaError_t de = cudaGetDeviceCount(&ndev);
+  if (de != cudaSuccess || ndev == 0) return fail(c, SIM3BA_ERR_CUDA, "no CUDA device (libsim3ba has no CPU fallback)");
+
+  sim3ba_ctx* h = new (std::nothrow) sim3ba_ctx();
+  if (!h) return fail(c, SIM3BA_ERR_ALLOC, "host allocation failed");
+  c = &h->c;
+  c->N = n_kf; c->H = height; c->W = width; c->HW = height * width; c->E = n_edges;
+  c->n = 7 * n_kf; c->npad = (c->n + kNB - 1) / kNB * kNB;
+  c->chunks = (c->HW + kTilePx - 1) / kTilePx;
+  c->stream = (cudaStream_t)cuda_stream;
+  c->prm = *params;
+
+  auto bail = [&](int code, const std::string& msg) {
+    free_all(c);
+    delete h;
+    return fail(nullptr, code, msg);
+  };
+#define CUB(call)                                                                                 \
+  do {                                                                                            \
+    cudaError_t e_ = (call);                                                                      \
+    if (e_ != cudaSuccess)                                                                        \
+      return bail(e_ == cudaErrorMemoryAllocation ? SIM3BA_ERR_ALLOC : SIM3BA_ERR_CUDA,           \
+                  std::string(#call) + ": " + cudaGetErrorString(e_));                            \
+  } while (0)
+
+  // edge list -> host, validation (i != j, endpoints in range)
+  c->h_edges.resize(2 * (size_t)n_edges);
+  if (n_edges > 0) {
+    CUB(cudaMemcpyAsync(c->h_edges.data(), d_edges, c->h_edges.size() * sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+    CUB(cudaStreamSynchronize(c->stream));
+  }
+  for (int e = 0; e < n_edges; ++e) {
+    const int32_t i = c->h_edges[2 * e], j = c->h_edges[2 * e + 1];
+    if (i < 0 || i >= n_kf || j < 0 || j >= n_kf || i == j)
+      return bail(SIM3BA_ERR_INVALID_ARG, "edge " + std::to_string(e) + " has an endpoint out of range or i == j");
+  }
+  c->h_fixed.assign(n_kf, 0);
+  for (int k = 0; k < n_fixed; ++k) {
+    if (h_fixed_kf[k] < 0 || h_fixed_kf[k] >= n_kf) return bail(SIM3BA_ERR_INVALID_ARG, "fixed keyframe out of range");
+    c->h_fixed[h_fixed_kf[k]] = 1;
+  }
+  build_bookkeeping(c);
+  std::vector<int32_t> sched(n_edges);
+  std::iota(sched.begin(), sched.end(), 0);
+  std::stable_sort(sched.begin(), sched.end(), [&](int32_t a, int32_t b) {
+    return std::make_pair(c->h_edges[2 * a], c->h_edges[2 * a + 1]) < std::make_pair(c->h_edges[2 * b], c->h_edges[2 * b + 1]);
+  });
+
+  const size_t NHW = (size_t)c->N * c->HW, np2 = (size_t)c->npad * c->npad;
+  CUB(dev_alloc(&c->pm, NHW));
+  CUB(upload(&c->edges, c->h_edges, c->stream));
+  CUB(upload(&c->sched, sched, c->stream));
+  CUB(upload(&c->fixed_mask, c->h_fixed, c->stream));
+  CUB(upload(&c->kf_ptr, c->h_kf_ptr, c->stream));
+  CUB(upload(&c->kf_edge, c->h_kf_edge, c->stream));
+  CUB(upload(&c->pair_kf, c->h_pair_kf, c->stream));
+  CUB(upload(&c->pair_ptr, c->h_pair_ptr, c->stream));
+  CUB(upload(&c->pair_edge, c->h_pair_edge, c->stream));
+  CUB(dev_alloc(&c->poses, (size_t)8 * c->N));
+  CUB(dev_alloc(&c->partials, (size_t)c->E * c->chunks * kPartialStride));
+  CUB(dev_alloc(&c->blocks35, (size_t)c->E * 35));
+  CUB(dev_alloc(&c->edge_cost, (size_t)c->E));
+  CUB(dev_alloc(&c->n_valid, (size_t)c->E));
+  CUB(dev_alloc(&c->checksum, (size_t)c->E));
+  CUB(dev_alloc(&c->Hd, np2));
+  CUB(dev_alloc(&c->L, np2));
+  CUB(dev_alloc(&c->g, (size_t)c->npad));
+  CUB(dev_alloc(&c->rhs, (size_t)c->npad));
+  CUB(dev_alloc(&c->ysol, (size_t)c->npad));
+  CUB(dev_alloc(&c->Dfac, (size_t)(c->npad / kNB) * kNB * kNB));
+  CUB(dev_alloc(&c->tau, (size_t)c->npad));
+  CUB(dev_alloc(&c->total_cost, 1));
+  CUB(dev_alloc(&c->fail_flag, 1));
+  CUB(cudaMallocHost(reinterpret_cast<void**>(&c->h_flag), sizeof(int32_t)));
+  CUB(cudaMallocHost(reinterpret_cast<void**>(&c->h_scalar), 4 * sizeof(double)));
+  for (auto& ev : c->ev) CUB(cudaEventCreate(&ev));
+  CUB(cudaMemsetAsync(c->g, 0, (size_t)c->npad * sizeof(double), c->stream));
+  CUB(cudaMemsetAsync(c->tau, 0, (size_t)c->npad * sizeof(double), c->stream));
+  CUB(cudaMemsetAsync(c->total_cost, 0, sizeof(double), c->stream));
+  CUB(cudaMemsetAsync(c->fail_flag, 0, sizeof(int32_t), c->stream));
+  {
+    std::vector<double> id(8 * (size_t)c->N, 0.0);
+    for (int k = 0; k < c->N; ++k) { id[8 * k + 6] = 1.0; id[8 * k + 7] = 1.0; }
+    CUB(cudaMemcpyAsync(c->poses, id.data(), id.size() * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CUB(cudaStreamSynchronize(c->stream));
+  }
+  c->match = d_match;
+  CUB(launch_pack(c, d_points, d_conf));
+  CUB(cudaStreamSynchronize(c->stream));
+#undef CUB
+  *out = h;
+  return SIM3BA_OK;
+}
+
+int sim3ba_destroy(sim3ba_ctx* h) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  cudaStreamSynchronize(h->c.stream);
+  free_all(&h->c);
+  delete h;
+  return SIM3BA_OK;
+}
+
+int sim3ba_set_params(sim3ba_ctx* h, const sim3ba_params* p) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (!params_ok(p)) return fail(c, SIM3BA_ERR_INVALID_ARG, "invalid params");
+  c->prm = *p;
+  return SIM3BA_OK;
+}
+
+int sim3ba_set_poses(sim3ba_ctx* h, const double* d_poses) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (!d_poses) return fail(c, SIM3BA_ERR_INVALID_ARG, "d_poses is NULL");
+  CU(cudaMemcpyAsync(c->poses, d_poses, (size_t)8 * c->N * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+  return SIM3BA_OK;
+}
+
+int sim3ba_get_poses(sim3ba_ctx* h, double* d_poses) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (!d_poses) return fail(c, SIM3BA_ERR_INVALID_ARG, "d_poses is NULL");
+  CU(cudaMemcpyAsync(d_poses, c->poses, (size_t)8 * c->N * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+  return SIM3BA_OK;
+}
+
+int sim3ba_build_system(sim3ba_ctx* h) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  mark(c, 0);
+  int rc = build_blocks(c);
+  if (rc) return rc;
+  mark(c, 1);
+  CU(launch_assemble(c, c->Hd, 0.0, 0.0, false));
+  mark(c, 2);
+  c->hd_valid = true;
+  if (c->profiling) {
+    CU(cudaStreamSynchronize(c->stream));
+    cudaEventElapsedTime(&c->phase_ms[0], c->ev[0], c->ev[1]);
+    cudaEventElapsedTime(&c->phase_ms[1], c->ev[1], c->ev[2]);
+    c->phase_ms[2] = c->phase_ms[3] = 0.f;
+  }
+  return SIM3BA_OK;
+}
+
+int sim3ba_solve(sim3ba_ctx* h) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (!c->built && !c->dense_loaded) return fail(c, SIM3BA_ERR_BAD_STATE, "sim3ba_solve before sim3ba_build_system");
+  return solve_impl(c);
+}
+
+int sim3ba_retract(sim3ba_ctx* h) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (!c->solved) return fail(c, SIM3BA_ERR_BAD_STATE, "sim3ba_retract before sim3ba_solve");
+  CU(launch_retract(c));
+  c->built = false; c->solved = false;
+  return SIM3BA_OK;
+}
+
+int sim3ba_step(sim3ba_ctx* h) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  mark(c, 0);
+  int rc = build_blocks(c);
+  if (rc) return rc;
+  c->hd_valid = false;
+  mark(c, 4);
+  rc = solve_impl(c);
+  if (rc) return rc;
+  mark(c, 3);
+  CU(launch_retract(c));
+  if (c->profiling) {
+    mark(c, 2);
+    CU(cudaStreamSynchronize(c->stream));
+    cudaEventElapsedTime(&c->phase_ms[0], c->ev[0], c->ev[4]);
+    cudaEventElapsedTime(&c->phase_ms[3], c->ev[3], c->ev[2]);
+  }
+  c->built = false; c->solved = false;
+  return SIM3BA_OK;
+}
+
+int sim3ba_step_host(sim3ba_ctx* h, const double* h_in, double* h_out, double* h_cost) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  const size_t bytes = (size_t)8 * c->N * sizeof(double);
+  if (h_in) CU(cudaMemcpyAsync(c->poses, h_in, bytes, cudaMemcpyHostToDevice, c->stream));
+  int rc = sim3ba_step(h);
+  if (rc) return rc;
+  if (h_out) CU(cudaMemcpyAsync(h_out, c->poses, bytes, cudaMemcpyDeviceToHost, c->stream));
+  if (h_cost) CU(cudaMemcpyAsync(h_cost, c->total_cost, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  return SIM3BA_OK;
+}
+
+int sim3ba_get_edge_stats(sim3ba_ctx* h, const int32_t** nv, const uint64_t** chk, const double** cost) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (nv) *nv = c->n_valid;
+  if (chk) *chk = reinterpret_cast<const uint64_t*>(c->checksum);
+  if (cost) *cost = c->edge_cost;
+  return SIM3BA_OK;
+}
+
+int sim3ba_get_edge_blocks(sim3ba_ctx* h, const double** b) {
+  if (!h || !b) return SIM3BA_ERR_INVALID_ARG;
+  *b = h->c.blocks35;
+  return SIM3BA_OK;
+}
+
+int sim3ba_get_system(sim3ba_ctx* h, const double** H, int32_t* ld, const double** g) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (!c->hd_valid) return fail(c, SIM3BA_ERR_BAD_STATE, "no dense system: call sim3ba_build_system first");
+  if (H) *H = c->Hd;
+  if (ld) *ld = c->npad;
+  if (g) *g = c->g;
+  return SIM3BA_OK;
+}
+
+int sim3ba_get_update(sim3ba_ctx* h, const double** tau, int32_t* attempts, double* eps_used, double* cost) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (tau) *tau = c->tau;
+  if (attempts) *attempts = c->attempts;
+  if (eps_used) *eps_used = c->eps_used;
+  if (cost) {
+    CU(cudaMemcpyAsync(c->h_scalar, c->total_cost, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    *cost = c->h_scalar[0];
+  }
+  return SIM3BA_OK;
+}
+
+int sim3ba_get_bookkeeping(sim3ba_ctx* h, const int32_t** kf_ptr, const int32_t** kf_edge, int32_t* n_pairs,
+                           const int32_t** pair_kf, const int32_t** pair_ptr, const int32_t** pair_edge) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (kf_ptr) *kf_ptr = c->h_kf_ptr.data();
+  if (kf_edge) *kf_edge = c->h_kf_edge.data();
+  if (n_pairs) *n_pairs = c->n_pairs;
+  if (pair_kf) *pair_kf = c->h_pair_kf.data();
+  if (pair_ptr) *pair_ptr = c->h_pair_ptr.data();
+  if (pair_edge) *pair_edge = c->h_pair_edge.data();
+  return SIM3BA_OK;
+}
+
+int sim3ba_load_system(sim3ba_ctx* h, const double* d_H, const double* d_g) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (!d_H || !d_g) return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL system pointer");
+  CU(cudaMemcpyAsync(c->Hd, d_H, (size_t)c->n * c->n * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+  CU(launch_load_gradient(c, d_g));
+  c->dense_loaded = true; c->hd_valid = false; c->built = false; c->solved = false;
+  return SIM3BA_OK;
+}
+
+int sim3ba_get_launch_count(sim3ba_ctx* h, int64_t* n) {
+  if (!h || !n) return SIM3BA_ERR_INVALID_ARG;
+  *n = h->c.launches;
+  return SIM3BA_OK;
+}
+
+int sim3ba_set_profiling(sim3ba_ctx* h, int32_t enable) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  h->c.profiling = enable != 0;
+  return SIM3BA_OK;
+}
+
+int sim3ba_get_phase_ms(sim3ba_ctx* h, float ms[4]) {
+  if (!h || !ms) return SIM3BA_ERR_INVALID_ARG;
+  for (int k = 0; k < 4; ++k) ms[k] = h->c.phase_ms[k];
+  return SIM3BA_OK;
+}
+
+int sim3ba_copy_d2d(sim3ba_ctx* h, void* dst, const void* src, uint64_t bytes) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (bytes == 0) return SIM3BA_OK;
+  if (!dst || !src) return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL pointer in sim3ba_copy_d2d");
+  CU(cudaMemcpyAsync(dst, src, (size_t)bytes, cudaMemcpyDeviceToDevice, c->stream));
+  return SIM3BA_OK;
+}
+
+const char* sim3ba_last_error(const sim3ba_ctx* h) { return h ? h->c.err.c_str() : g_create_error.c_str(); }
+
+const char* sim3ba_version(void) { return "sim3ba 0.1 (sm_100a)"; }
+
+}  // extern "C"
+#pragma GCC visibility pop

@@ -1,0 +1,78 @@
+// Internal context and kernel launchers of libsim3ba (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/sim3ba.h"
+
+namespace sim3ba {
+
+constexpr int kTilePx = 4096;        // pixels of one edge handled by one accumulate CTA
+constexpr int kAccThreads = 256;
+constexpr int kPartialStride = 40;   // doubles per (edge, chunk) partial: 28 M + 7 c + cost + n_valid + checksum (+2 pad)
+constexpr int kNB = 64;              // Cholesky block size
+
+struct DevParams {       // robust-kernel constants, fp32, passed by value to kernel 1
+  float inv_var_ray;     // 1 / sigma_r^2
+  float inv_var_dist;    // 1 / sigma_d^2
+  float huber_k;
+  float huber_k2;
+  float conf_min;
+};
+
+struct Ctx {
+  int N = 0, H = 0, W = 0, HW = 0, E = 0, n = 0, npad = 0, chunks = 0, n_pairs = 0;
+  cudaStream_t stream = nullptr;
+  sim3ba_params prm{};
+  // inputs
+  float4* pm = nullptr;            // [N][HW] packed (x, y, z, conf)
+  const int32_t* match = nullptr;  // borrowed [E][HW]
+  int32_t* edges = nullptr;        // [E][2]
+  int32_t* sched = nullptr;        // [E] edge processing order (sorted by first endpoint)
+  uint8_t* fixed_mask = nullptr;   // [N]
+  double* poses = nullptr;         // [N][8]
+  // bookkeeping (device + host)
+  int32_t *kf_ptr = nullptr, *kf_edge = nullptr, *pair_kf = nullptr, *pair_ptr = nullptr, *pair_edge = nullptr;
+  std::vector<int32_t> h_edges, h_kf_ptr, h_kf_edge, h_pair_kf, h_pair_ptr, h_pair_edge;
+  std::vector<uint8_t> h_fixed;
+  // per-edge results
+  double* partials = nullptr;      // [E][chunks][kPartialStride]
+  double* blocks35 = nullptr;      // [E][35]
+  double* edge_cost = nullptr;     // [E]
+  int32_t* n_valid = nullptr;      // [E]
+  unsigned long long* checksum = nullptr;  // [E]
+  // dense system
+  double* Hd = nullptr;            // [npad][npad] undamped (API read-back)
+  double* L = nullptr;             // [npad][npad] working copy, factorised in place
+  double* g = nullptr;             // [npad]
+  double* rhs = nullptr;           // [npad] working right-hand side b (starts as -g)
+  double* ysol = nullptr;          // [npad] y = L^-1 b, then consumed by the backward solve
+  double* Dfac = nullptr;          // [npad/kNB][kNB*kNB] factorised diagonal blocks
+  double* tau = nullptr;           // [npad]
+  double* total_cost = nullptr;    // [1]
+  int32_t* fail_flag = nullptr;    // [1] device
+  int32_t* h_flag = nullptr;       // pinned
+  double* h_scalar = nullptr;      // pinned [4]
+  bool built = false, solved = false, dense_loaded = false, hd_valid = false;
+  int attempts = 0;
+  double eps_used = 0.0;
+  int64_t launches = 0;
+  bool profiling = false;
+  cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  float phase_ms[4] = {0, 0, 0, 0};
+  std::string err;
+};
+
+// kernel launchers (each returns the cudaError of the launch)
+cudaError_t launch_pack(Ctx* c, const float* d_points, const float* d_conf);
+cudaError_t launch_accumulate(Ctx* c);                   // kernels 1+2: partials -> blocks35, stats, cost
+cudaError_t launch_assemble(Ctx* c, double* dst, double lambda, double eps, bool from_dense);  // kernel 3
+cudaError_t launch_gradient(Ctx* c);                     // g from the per-edge b_e
+cudaError_t launch_load_gradient(Ctx* c, const double* d_g);
+cudaError_t launch_factor_solve(Ctx* c);                 // kernel 4 on c->L / c->rhs -> c->tau, sets fail_flag
+cudaError_t launch_retract(Ctx* c);                      // kernel 5
+
+}  // namespace sim3ba
