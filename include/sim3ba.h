@@ -147,11 +147,12 @@ int sim3ba_load_system(sim3ba_ctx* ctx, const double* d_H, const double* d_g);
 int sim3ba_get_launch_count(sim3ba_ctx* ctx, int64_t* h_count);
 
 /* Device time in milliseconds of the phases of the last sim3ba_step / build / solve, measured
- * with CUDA events on the context's stream: [0] accumulate+reduce (a1-a5), [1] assembly (a6),
- * [2] factor+solve (a7), [3] retraction (a8).  Synchronises.  Phase timing is only recorded
- * after sim3ba_set_profiling(ctx, 1). */
+ * with CUDA events on the context's stream: [0] kernel 1 (per-match accumulate, a1-a5 partials),
+ * [1] kernel 2 (per-edge reduce + adjoint congruence, gradient, cost), [2] assembly (a6, summed over
+ * attempts), [3] factor + triangular solves (a7, summed over attempts), [4] retraction (a8),
+ * [5..7] reserved (0).  Synchronises.  Only recorded after sim3ba_set_profiling(ctx, 1). */
 int sim3ba_set_profiling(sim3ba_ctx* ctx, int32_t enable);
-int sim3ba_get_phase_ms(sim3ba_ctx* ctx, float h_ms[4]);
+int sim3ba_get_phase_ms(sim3ba_ctx* ctx, float h_ms[8]);
 
 /* Binding convenience: asynchronous device-to-device copy of `bytes` bytes on the context's stream
  * (used to move the read-back buffers above into caller-owned device memory). */

@@ -234,7 +234,7 @@ class Sim3BA:
     def set_profiling(self, on: bool):
         self._check(self.lib.sim3ba_set_profiling(self._h, 1 if on else 0))
 
-    def phase_ms(self) -> Tuple[float, float, float, float]:
-        buf = (C.c_float * 4)()
+    def phase_ms(self) -> Tuple[float, ...]:
+        buf = (C.c_float * 8)()
         self._check(self.lib.sim3ba_get_phase_ms(self._h, buf))
         return tuple(buf)

@@ -24,23 +24,38 @@ constexpr int kNumAcc = 36;                          // 28 M + 7 c + cost
 
 __device__ __forceinline__ float4 ldg_f4(const float4* p) { return __ldg(p); }
 
+#ifdef SIM3BA_EXACT_RSQRT   // debugging aid: IEEE-rounded 1/sqrt instead of the 2-ulp MUFU path
+__device__ __forceinline__ float rsq(float v) { return __frcp_rn(__fsqrt_rn(v)); }
+#else
+__device__ __forceinline__ float rsq(float v) { return rsqrtf(v); }
+#endif
+
 // One valid match: accumulate J_xi^T Omega J_xi (upper triangle, 25 structurally non-zero
 // entries), J_xi^T Omega e (7) and the robust cost into acc[].
 __device__ __forceinline__ void accumulate_match(float (&acc)[kNumAcc], const float4 Xi, const float4 Xj,
-                                                 const float* __restrict__ sR, const float* __restrict__ tt,
-                                                 const DevParams prm) {
-  // x = s_ij R_ij X_j + t_ij
-  const float x0 = fmaf(sR[0], Xj.x, fmaf(sR[1], Xj.y, fmaf(sR[2], Xj.z, tt[0])));
-  const float x1 = fmaf(sR[3], Xj.x, fmaf(sR[4], Xj.y, fmaf(sR[5], Xj.z, tt[1])));
-  const float x2 = fmaf(sR[6], Xj.x, fmaf(sR[7], Xj.y, fmaf(sR[8], Xj.z, tt[2])));
+                                                 const double* __restrict__ Td, const DevParams prm) {
+  // delta = T_ij X_j - X_i in FP64 (Td = s_ij R_ij row-major [9], t_ij [3]).  This difference is the
+  // one cancellation of the residual (|delta| ~ noise << |x|): evaluated in fp32 it would carry an
+  // absolute error of ~ulp(|x|) per match, i.e. 1e-4..1e-3 of the residual itself.  Everything after
+  // it works on small quantities, so fp32 is accurate to ~1e-7 RELATIVE to the residual.
+  const double Xjx = (double)Xj.x, Xjy = (double)Xj.y, Xjz = (double)Xj.z;
+  const float del0 = (float)fma(Td[0], Xjx, fma(Td[1], Xjy, fma(Td[2], Xjz, Td[9] - (double)Xi.x)));
+  const float del1 = (float)fma(Td[3], Xjx, fma(Td[4], Xjy, fma(Td[5], Xjz, Td[10] - (double)Xi.y)));
+  const float del2 = (float)fma(Td[6], Xjx, fma(Td[7], Xjy, fma(Td[8], Xjz, Td[11] - (double)Xi.z)));
+  const float x0 = Xi.x + del0, x1 = Xi.y + del1, x2 = Xi.z + del2;   // x = T_ij X_j (fp32)
   const float d2 = fmaxf(fmaf(x0, x0, fmaf(x1, x1, x2 * x2)), 1e-20f);
-  const float rd = rsqrtf(d2);
+  const float rd = rsq(d2);
   const float d = d2 * rd;
   const float u0 = x0 * rd, u1 = x1 * rd, u2 = x2 * rd;
   const float di2 = fmaxf(fmaf(Xi.x, Xi.x, fmaf(Xi.y, Xi.y, Xi.z * Xi.z)), 1e-20f);
-  const float rdi = rsqrtf(di2);
-  const float e0 = fmaf(-Xi.x, rdi, u0), e1 = fmaf(-Xi.y, rdi, u1), e2 = fmaf(-Xi.z, rdi, u2);
-  const float e3 = fmaf(-di2, rdi, d);
+  const float rdi = rsq(di2);
+  const float di = di2 * rdi;
+  // e3 = |x| - |X_i| = delta . (x + X_i) / (|x| + |X_i|);  e_r = x/|x| - X_i/|X_i| = delta/|x| - psi(X_i) e3/|x|
+  const float e3 = __fdividef(fmaf(del0, x0 + Xi.x, fmaf(del1, x1 + Xi.y, del2 * (x2 + Xi.z))), d + di);
+  const float e3rd = e3 * rd;
+  const float e0 = fmaf(del0, rd, -(Xi.x * rdi) * e3rd);
+  const float e1 = fmaf(del1, rd, -(Xi.y * rdi) * e3rd);
+  const float e2 = fmaf(del2, rd, -(Xi.z * rdi) * e3rd);
   // q = sqrt(c_i c_j); s_c = q / sigma_c^2; r_c^2 = s_c e_c^2
   const float cc = Xi.w * Xj.w;
   const float q = cc * rsqrtf(fmaxf(cc, 1e-30f));
@@ -114,7 +129,7 @@ __global__ void __launch_bounds__(kAccThreads)
 k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, const int32_t* __restrict__ edges,
              const int32_t* __restrict__ sched, const double* __restrict__ poses, double* __restrict__ partials,
              int HW, int chunks, DevParams prm) {
-  __shared__ float s_T[12];
+  __shared__ double s_T[12];  // s_ij R_ij [9], t_ij [3]
   __shared__ double s_red[kAccThreads / 32][kNumAcc];
   __shared__ unsigned long long s_chk[kAccThreads / 32];
   __shared__ int s_cnt[kAccThreads / 32];
@@ -125,16 +140,14 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
   if (threadIdx.x == 0) {
     const Sim3d Tij = relative_pose(load_pose(poses + 8 * i), load_pose(poses + 8 * j));
 #pragma unroll
-    for (int k = 0; k < 9; ++k) s_T[k] = (float)(Tij.s * Tij.R[k]);
+    for (int k = 0; k < 9; ++k) s_T[k] = Tij.s * Tij.R[k];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) s_T[9 + k] = (float)Tij.t[k];
+    for (int k = 0; k < 3; ++k) s_T[9 + k] = Tij.t[k];
   }
   __syncthreads();
-  float sR[9], tt[3];
+  double Td[12];
 #pragma unroll
-  for (int k = 0; k < 9; ++k) sR[k] = s_T[k];
-#pragma unroll
-  for (int k = 0; k < 3; ++k) tt[k] = s_T[9 + k];
+  for (int k = 0; k < 12; ++k) Td[k] = s_T[k];
 
   const float4* __restrict__ Pi = pm + (size_t)i * HW;
   const float4* __restrict__ Pj = pm + (size_t)j * HW;
@@ -170,7 +183,7 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
     for (int b = 0; b < kBatch; ++b) {
       const int m = base + (k0 + b) * kAccThreads;
       if (ok[b] && Xi[b].w > prm.conf_min && Xj[b].w > prm.conf_min) {
-        accumulate_match(acc, Xi[b], Xj[b], sR, tt, prm);
+        accumulate_match(acc, Xi[b], Xj[b], Td, prm);
         ++cnt;
         chk += (unsigned long long)m * (unsigned long long)HW + (unsigned long long)n[b];
       }
@@ -298,6 +311,7 @@ cudaError_t launch_accumulate(Ctx* c) {
                                                                  c->partials, c->HW, c->chunks, p);
   cudaError_t err = cudaGetLastError();
   if (err != cudaSuccess) return err;
+  if (c->profiling) cudaEventRecord(c->ev[1], c->stream);
   k_finalize<<<c->E, 64, 0, c->stream>>>(c->partials, c->edges, c->poses, c->blocks35, c->edge_cost, c->n_valid,
                                          c->checksum, c->chunks);
   c->launches += 2;

@@ -97,8 +97,10 @@ inline void mark(Ctx* c, int i) { if (c->profiling) cudaEventRecord(c->ev[i], c-
 
 // a1-a5 (+ gradient and total cost): the block-sparse system at the current poses
 int build_blocks(Ctx* c) {
-  CU(launch_accumulate(c));
+  mark(c, 0);
+  CU(launch_accumulate(c));   // records ev[1] between kernel 1 and kernel 2 when profiling
   CU(launch_gradient(c));
+  mark(c, 2);
   c->built = true; c->solved = false; c->dense_loaded = false;
   return SIM3BA_OK;
 }
@@ -110,23 +112,23 @@ int solve_impl(Ctx* c) {
   float asm_ms = 0.f, fac_ms = 0.f;
   for (int r = 0; r < c->prm.max_attempts; ++r) {
     const double eps = c->prm.eps0 * pow(100.0, (double)r);
-    mark(c, 1);
-    CU(launch_assemble(c, c->L, c->prm.lm_lambda, eps, c->dense_loaded));
-    mark(c, 2);
-    CU(launch_factor_solve(c));
     mark(c, 3);
+    CU(launch_assemble(c, c->L, c->prm.lm_lambda, eps, c->dense_loaded));
+    mark(c, 4);
+    CU(launch_factor_solve(c));
+    mark(c, 5);
     CU(cudaMemcpyAsync(c->h_flag, c->fail_flag, sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     if (c->profiling) {
       float a = 0.f, f = 0.f;
-      cudaEventElapsedTime(&a, c->ev[1], c->ev[2]);
-      cudaEventElapsedTime(&f, c->ev[2], c->ev[3]);
+      cudaEventElapsedTime(&a, c->ev[3], c->ev[4]);
+      cudaEventElapsedTime(&f, c->ev[4], c->ev[5]);
       asm_ms += a; fac_ms += f;
     }
     c->attempts = r + 1;
     if (*c->h_flag == 0) { ok = true; c->eps_used = eps; break; }
   }
-  if (c->profiling) { c->phase_ms[1] = asm_ms; c->phase_ms[2] = fac_ms; }
+  if (c->profiling) { c->phase_ms[2] = asm_ms; c->phase_ms[3] = fac_ms; }
   if (!ok) CU(cudaMemsetAsync(c->tau, 0, (size_t)c->npad * sizeof(double), c->stream));  // zero update
   c->solved = true;
   return SIM3BA_OK;
@@ -286,18 +288,17 @@ int sim3ba_get_poses(sim3ba_ctx* h, double* d_poses) {
 int sim3ba_build_system(sim3ba_ctx* h) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
-  mark(c, 0);
   int rc = build_blocks(c);
   if (rc) return rc;
-  mark(c, 1);
   CU(launch_assemble(c, c->Hd, 0.0, 0.0, false));
-  mark(c, 2);
+  mark(c, 3);
   c->hd_valid = true;
   if (c->profiling) {
     CU(cudaStreamSynchronize(c->stream));
     cudaEventElapsedTime(&c->phase_ms[0], c->ev[0], c->ev[1]);
     cudaEventElapsedTime(&c->phase_ms[1], c->ev[1], c->ev[2]);
-    c->phase_ms[2] = c->phase_ms[3] = 0.f;
+    cudaEventElapsedTime(&c->phase_ms[2], c->ev[2], c->ev[3]);
+    c->phase_ms[3] = c->phase_ms[4] = 0.f;
   }
   return SIM3BA_OK;
 }
@@ -321,20 +322,19 @@ int sim3ba_retract(sim3ba_ctx* h) {
 int sim3ba_step(sim3ba_ctx* h) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
-  mark(c, 0);
   int rc = build_blocks(c);
   if (rc) return rc;
   c->hd_valid = false;
-  mark(c, 4);
   rc = solve_impl(c);
   if (rc) return rc;
-  mark(c, 3);
+  mark(c, 6);
   CU(launch_retract(c));
   if (c->profiling) {
-    mark(c, 2);
+    mark(c, 7);
     CU(cudaStreamSynchronize(c->stream));
-    cudaEventElapsedTime(&c->phase_ms[0], c->ev[0], c->ev[4]);
-    cudaEventElapsedTime(&c->phase_ms[3], c->ev[3], c->ev[2]);
+    cudaEventElapsedTime(&c->phase_ms[0], c->ev[0], c->ev[1]);
+    cudaEventElapsedTime(&c->phase_ms[1], c->ev[1], c->ev[2]);
+    cudaEventElapsedTime(&c->phase_ms[4], c->ev[6], c->ev[7]);
   }
   c->built = false; c->solved = false;
   return SIM3BA_OK;
@@ -427,9 +427,9 @@ int sim3ba_set_profiling(sim3ba_ctx* h, int32_t enable) {
   return SIM3BA_OK;
 }
 
-int sim3ba_get_phase_ms(sim3ba_ctx* h, float ms[4]) {
+int sim3ba_get_phase_ms(sim3ba_ctx* h, float ms[8]) {
   if (!h || !ms) return SIM3BA_ERR_INVALID_ARG;
-  for (int k = 0; k < 4; ++k) ms[k] = h->c.phase_ms[k];
+  for (int k = 0; k < 8; ++k) ms[k] = h->c.phase_ms[k];
   return SIM3BA_OK;
 }
 

@@ -61,8 +61,8 @@ struct Ctx {
   double eps_used = 0.0;
   int64_t launches = 0;
   bool profiling = false;
-  cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
-  float phase_ms[4] = {0, 0, 0, 0};
+  cudaEvent_t ev[8] = {};
+  float phase_ms[8] = {};
   std::string err;
 };
 
