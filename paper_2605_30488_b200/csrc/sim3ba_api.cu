@@ -86,8 +86,8 @@ void free_all(Ctx* c) {
   cudaFree(c->pm); cudaFree(c->edges); cudaFree(c->sched); cudaFree(c->fixed_mask); cudaFree(c->poses);
   cudaFree(c->kf_ptr); cudaFree(c->kf_edge); cudaFree(c->pair_kf); cudaFree(c->pair_ptr); cudaFree(c->pair_edge);
   cudaFree(c->partials); cudaFree(c->blocks35); cudaFree(c->edge_cost); cudaFree(c->n_valid); cudaFree(c->checksum);
-  cudaFree(c->Hd); cudaFree(c->L); cudaFree(c->g); cudaFree(c->rhs); cudaFree(c->ysol); cudaFree(c->Dfac);
-  cudaFree(c->tau); cudaFree(c->total_cost); cudaFree(c->fail_flag);
+  cudaFree(c->Hd); cudaFree(c->L); cudaFree(c->g); cudaFree(c->rhs); cudaFree(c->ysol); cudaFree(c->Dfac); cudaFree(c->Dinv);
+  cudaFree(c->tau); cudaFree(c->total_cost); cudaFree(c->fail_flag); cudaFree(c->d_eps_used); cudaFree(c->bar);
   if (c->h_flag) cudaFreeHost(c->h_flag);
   if (c->h_scalar) cudaFreeHost(c->h_scalar);
   for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
@@ -105,32 +105,25 @@ int build_blocks(Ctx* c) {
   return SIM3BA_OK;
 }
 
-// a6 (damped, into L) + a7 with the escalation of PAPER.md:122
+// a6 (damped, into L) + a7 with the escalation of PAPER.md:122: one persistent kernel, no host sync
 int solve_impl(Ctx* c) {
-  c->attempts = 0; c->eps_used = NAN;
-  bool ok = false;
-  float asm_ms = 0.f, fac_ms = 0.f;
-  for (int r = 0; r < c->prm.max_attempts; ++r) {
-    const double eps = c->prm.eps0 * pow(100.0, (double)r);
-    mark(c, 3);
-    CU(launch_assemble(c, c->L, c->prm.lm_lambda, eps, c->dense_loaded));
-    mark(c, 4);
-    CU(launch_factor_solve(c));
-    mark(c, 5);
-    CU(cudaMemcpyAsync(c->h_flag, c->fail_flag, sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
-    CU(cudaStreamSynchronize(c->stream));
-    if (c->profiling) {
-      float a = 0.f, f = 0.f;
-      cudaEventElapsedTime(&a, c->ev[3], c->ev[4]);
-      cudaEventElapsedTime(&f, c->ev[4], c->ev[5]);
-      asm_ms += a; fac_ms += f;
-    }
-    c->attempts = r + 1;
-    if (*c->h_flag == 0) { ok = true; c->eps_used = eps; break; }
-  }
-  if (c->profiling) { c->phase_ms[2] = asm_ms; c->phase_ms[3] = fac_ms; }
-  if (!ok) CU(cudaMemsetAsync(c->tau, 0, (size_t)c->npad * sizeof(double), c->stream));  // zero update
+  mark(c, 3);
+  CU(launch_solve(c));
+  mark(c, 5);
   c->solved = true;
+  c->status_stale = true;
+  return SIM3BA_OK;
+}
+
+// attempts / eps of the last solve live on the device until somebody asks for them
+int fetch_status(Ctx* c) {
+  if (!c->status_stale) return SIM3BA_OK;
+  CU(cudaMemcpyAsync(c->h_flag, c->fail_flag, 4 * sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaMemcpyAsync(c->h_scalar + 1, c->d_eps_used, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  c->attempts = c->h_flag[1];
+  c->eps_used = c->h_scalar[1];
+  c->status_stale = false;
   return SIM3BA_OK;
 }
 
@@ -230,15 +223,18 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
   CUB(dev_alloc(&c->ysol, (size_t)c->npad));
   CUB(dev_alloc(&c->Dfac, (size_t)(c->npad / kNB) * kNB * kNB));
   CUB(dev_alloc(&c->tau, (size_t)c->npad));
+  CUB(dev_alloc(&c->Dinv, (size_t)c->npad));
   CUB(dev_alloc(&c->total_cost, 1));
-  CUB(dev_alloc(&c->fail_flag, 1));
-  CUB(cudaMallocHost(reinterpret_cast<void**>(&c->h_flag), sizeof(int32_t)));
+  CUB(dev_alloc(&c->fail_flag, 4));
+  CUB(dev_alloc(&c->d_eps_used, 1));
+  CUB(dev_alloc(&c->bar, 1));
+  CUB(cudaMallocHost(reinterpret_cast<void**>(&c->h_flag), 4 * sizeof(int32_t)));
   CUB(cudaMallocHost(reinterpret_cast<void**>(&c->h_scalar), 4 * sizeof(double)));
   for (auto& ev : c->ev) CUB(cudaEventCreate(&ev));
   CUB(cudaMemsetAsync(c->g, 0, (size_t)c->npad * sizeof(double), c->stream));
   CUB(cudaMemsetAsync(c->tau, 0, (size_t)c->npad * sizeof(double), c->stream));
   CUB(cudaMemsetAsync(c->total_cost, 0, sizeof(double), c->stream));
-  CUB(cudaMemsetAsync(c->fail_flag, 0, sizeof(int32_t), c->stream));
+  CUB(cudaMemsetAsync(c->fail_flag, 0, 4 * sizeof(int32_t), c->stream));
   {
     std::vector<double> id(8 * (size_t)c->N, 0.0);
     for (int k = 0; k < c->N; ++k) { id[8 * k + 6] = 1.0; id[8 * k + 7] = 1.0; }
@@ -334,7 +330,9 @@ int sim3ba_step(sim3ba_ctx* h) {
     CU(cudaStreamSynchronize(c->stream));
     cudaEventElapsedTime(&c->phase_ms[0], c->ev[0], c->ev[1]);
     cudaEventElapsedTime(&c->phase_ms[1], c->ev[1], c->ev[2]);
+    cudaEventElapsedTime(&c->phase_ms[3], c->ev[3], c->ev[5]);
     cudaEventElapsedTime(&c->phase_ms[4], c->ev[6], c->ev[7]);
+    c->phase_ms[2] = 0.f;   // the damped assembly runs inside the persistent solve kernel
   }
   c->built = false; c->solved = false;
   return SIM3BA_OK;
@@ -382,6 +380,10 @@ int sim3ba_get_update(sim3ba_ctx* h, const double** tau, int32_t* attempts, doub
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
   if (tau) *tau = c->tau;
+  if (attempts || eps_used) {
+    int rc = fetch_status(c);
+    if (rc) return rc;
+  }
   if (attempts) *attempts = c->attempts;
   if (eps_used) *eps_used = c->eps_used;
   if (cost) {

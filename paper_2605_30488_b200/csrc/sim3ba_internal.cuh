@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
 #include <string>
 #include <vector>
 
@@ -51,12 +52,15 @@ struct Ctx {
   double* rhs = nullptr;           // [npad] working right-hand side b (starts as -g)
   double* ysol = nullptr;          // [npad] y = L^-1 b, then consumed by the backward solve
   double* Dfac = nullptr;          // [npad/kNB][kNB*kNB] factorised diagonal blocks
+  double* Dinv = nullptr;          // [npad] reciprocals of the diagonal of L
   double* tau = nullptr;           // [npad]
   double* total_cost = nullptr;    // [1]
-  int32_t* fail_flag = nullptr;    // [1] device
+  int32_t* fail_flag = nullptr;    // [4] device: [0] failure flag, [1] attempts used, [2] solved
+  double* d_eps_used = nullptr;    // [1] device
+  unsigned int* bar = nullptr;     // [1] device: grid-barrier counter of k_solve
   int32_t* h_flag = nullptr;       // pinned
   double* h_scalar = nullptr;      // pinned [4]
-  bool built = false, solved = false, dense_loaded = false, hd_valid = false;
+  bool built = false, solved = false, dense_loaded = false, hd_valid = false, status_stale = false;
   int attempts = 0;
   double eps_used = 0.0;
   int64_t launches = 0;
@@ -72,7 +76,7 @@ cudaError_t launch_accumulate(Ctx* c);                   // kernels 1+2: partial
 cudaError_t launch_assemble(Ctx* c, double* dst, double lambda, double eps, bool from_dense);  // kernel 3
 cudaError_t launch_gradient(Ctx* c);                     // g from the per-edge b_e
 cudaError_t launch_load_gradient(Ctx* c, const double* d_g);
-cudaError_t launch_factor_solve(Ctx* c);                 // kernel 4 on c->L / c->rhs -> c->tau, sets fail_flag
+cudaError_t launch_solve(Ctx* c);                        // kernels 3+4 (persistent): damped assembly, Cholesky, solves, eps retry
 cudaError_t launch_retract(Ctx* c);                      // kernel 5
 
 }  // namespace sim3ba
