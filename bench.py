@@ -266,7 +266,7 @@ def run_ours(args):
                      "achieved_stream_accounting": bytes_stream / k1_s / 1e9,
                      "frac_stream_accounting": bytes_stream / k1_s / 1e9 / hbm_peak},
     }
-    if world == 1:
+    if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(g, preset, budget_s=20.0)
     print(json.dumps(out))
 
@@ -339,6 +339,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true",
+                    help="skip the oracle timing leg (profiling runs under ncu; never for a reported line)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
