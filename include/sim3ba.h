@@ -75,7 +75,9 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
 
 int sim3ba_destroy(sim3ba_ctx* ctx);
 
-/* Replace the robust-kernel / solver constants (takes effect at the next build/solve). */
+/* Replace the robust-kernel / solver constants (takes effect at the next build/solve).  conf_min is
+ * fixed at create (the per-pixel validity c > conf_min is decided once, exactly, when the pointmaps
+ * are packed): a different conf_min -> SIM3BA_ERR_INVALID_ARG. */
 int sim3ba_set_params(sim3ba_ctx* ctx, const sim3ba_params* params);
 
 /* Poses [N][8] double, device pointers; asynchronous device-to-device copies. */

@@ -3,14 +3,20 @@
 //
 //   Eq. (1)  PAPER.md:73   e = [psi(x) - psi(X_i); |x| - |X_i|],  x = T_ij X_j
 //   PAPER.md:76            r_c = sqrt(q) e_c / sigma_c, w_c = min(1, kappa/|r_c|), q = sqrt(c_i c_j)
-//   Eq. (6)  PAPER.md:116  J_xi = [Dpsi/Dx; Dd/Dx] [I, -[x]x, x]  (closed form used here:
-//                          J_xi = [[P, -[u]x, 0], [u^T, 0, d]], P = (I - u u^T)/d, u = x/d)
+//   Eq. (6)  PAPER.md:116  J_xi = [Dpsi/Dx; Dd/Dx] [I, -[x]x, x]  (closed form used here, with
+//                          S = -[u]x, u = x/d:  J_xi = [[S S^T / d, S, 0], [u^T, 0, d]])
 //   PAPER.md:118           J_j = J_xi Ad_{T_i^-1}, J_i = -J_j  ->  the adjoint is applied once per
 //                          edge:  A_e = Ad^T (sum J_xi^T Omega J_xi) Ad,  b_e = Ad^T (sum J_xi^T Omega e)
 //
-// Precision plan: per-match arithmetic and per-thread partial sums (<= 16 terms) in
-// fp32; everything from the per-thread partial upwards (warp, CTA, edge, adjoint congruence) in fp64.
-// No floating-point atomics anywhere: the reduction order is fixed, results are run-to-run identical.
+// Work decomposition: one CTA per (keyframe i, tile of 4096 pixels of i).  The
+// tile of X_i is staged in shared memory ONCE by a TMA bulk copy (cp.async.bulk + mbarrier) and reused
+// by every edge (i, j) that leaves i; per edge the match indices are streamed (coalesced) and X_j is
+// gathered (128-bit loads), software-pipelined two batches ahead.
+//
+// Precision plan: delta = T_ij X_j - X_i in FP64 (the one cancellation of the residual); everything
+// after it and the per-thread partial sums (<= 16 terms) in fp32; every sum from the per-thread
+// partial upwards (warp, CTA, edge, adjoint congruence) in FP64.  No floating-point atomics: the
+// reduction order is fixed, results are run-to-run identical.
 #include "sim3ba_internal.cuh"
 #include "sim3_math.cuh"
 
@@ -18,233 +24,331 @@ namespace sim3ba {
 
 namespace {
 
-constexpr int kPxPerThread = kTilePx / kAccThreads;  // 16
-constexpr int kBatch = 4;                            // loads in flight per thread
-constexpr int kNumAcc = 36;                          // 28 M + 7 c + cost
+constexpr int kRows = kTilePx / kAccThreads;   // 16 pixels per thread per (edge, tile)
+constexpr int kWarps = kAccThreads / 32;
+constexpr int kSlots = kPartialStride;         // 40 reduction slots (layout: sim3ba_internal.cuh)
 
-__device__ __forceinline__ float4 ldg_f4(const float4* p) { return __ldg(p); }
+// shared-memory carve-up of k_accumulate (dynamic)
+constexpr size_t kOffXi = 0;                                      // float4 [kTilePx]
+constexpr size_t kOffDer = kOffXi + sizeof(float4) * kTilePx;     // float2 [kTilePx] (1/|X_i|, |X_i|)
+constexpr size_t kOffRed = kOffDer + sizeof(float2) * kTilePx;    // double [kWarps][kSlots]
+constexpr size_t kOffT = kOffRed + sizeof(double) * kWarps * kSlots;   // double [12]
+constexpr size_t kOffCnt = kOffT + sizeof(double) * 12;           // long long [kWarps]
+constexpr size_t kOffChk = kOffCnt + sizeof(long long) * kWarps;  // unsigned long long [kWarps]
+constexpr size_t kOffBar = kOffChk + sizeof(long long) * kWarps;  // mbarrier
+constexpr size_t kAccSmem = kOffBar + 16;
 
-#ifdef SIM3BA_EXACT_RSQRT   // debugging aid: IEEE-rounded 1/sqrt instead of the 2-ulp MUFU path
-__device__ __forceinline__ float rsq(float v) { return __frcp_rn(__fsqrt_rn(v)); }
-#else
-__device__ __forceinline__ float rsq(float v) { return rsqrtf(v); }
-#endif
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
-// One valid match: accumulate J_xi^T Omega J_xi (upper triangle, 25 structurally non-zero
-// entries), J_xi^T Omega e (7) and the robust cost into acc[].
-__device__ __forceinline__ void accumulate_match(float (&acc)[kNumAcc], const float4 Xi, const float4 Xj,
-                                                 const double* __restrict__ Td, const DevParams prm) {
-  // delta = T_ij X_j - X_i in FP64 (Td = s_ij R_ij row-major [9], t_ij [3]).  This difference is the
-  // one cancellation of the residual (|delta| ~ noise << |x|): evaluated in fp32 it would carry an
-  // absolute error of ~ulp(|x|) per match, i.e. 1e-4..1e-3 of the residual itself.  Everything after
-  // it works on small quantities, so fp32 is accurate to ~1e-7 RELATIVE to the residual.
-  const double Xjx = (double)Xj.x, Xjy = (double)Xj.y, Xjz = (double)Xj.z;
-  const float del0 = (float)fma(Td[0], Xjx, fma(Td[1], Xjy, fma(Td[2], Xjz, Td[9] - (double)Xi.x)));
-  const float del1 = (float)fma(Td[3], Xjx, fma(Td[4], Xjy, fma(Td[5], Xjz, Td[10] - (double)Xi.y)));
-  const float del2 = (float)fma(Td[6], Xjx, fma(Td[7], Xjy, fma(Td[8], Xjz, Td[11] - (double)Xi.z)));
-  const float x0 = Xi.x + del0, x1 = Xi.y + del1, x2 = Xi.z + del2;   // x = T_ij X_j (fp32)
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// TMA 1-D bulk copy global -> shared, completion signalled on the mbarrier (bytes % 16 == 0)
+__device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+// One valid match: accumulate J_xi^T Omega J_xi (25 structurally non-zero upper-triangular entries),
+// J_xi^T Omega e (7) and the two robust-cost sums into acc[].
+//   del = T_ij X_j - X_i (fp32 rounding of the FP64 value), Xi = (X_i, sqrt c_i), rdi = 1/|X_i|, di = |X_i|,
+//   wj = sqrt c_j.
+__device__ __forceinline__ void accumulate_match(float (&acc)[kSlots], const float del0, const float del1, const float del2,
+                                                 const float4 Xi, const float rdi, const float di, const float wj,
+                                                 const DevParams& prm) {
+  const float x0 = Xi.x + del0, x1 = Xi.y + del1, x2 = Xi.z + del2;   // x = T_ij X_j
   const float d2 = fmaxf(fmaf(x0, x0, fmaf(x1, x1, x2 * x2)), 1e-20f);
-  const float rd = rsq(d2);
+  const float rd = rsqrtf(d2);
   const float d = d2 * rd;
   const float u0 = x0 * rd, u1 = x1 * rd, u2 = x2 * rd;
-  const float di2 = fmaxf(fmaf(Xi.x, Xi.x, fmaf(Xi.y, Xi.y, Xi.z * Xi.z)), 1e-20f);
-  const float rdi = rsq(di2);
-  const float di = di2 * rdi;
-  // e3 = |x| - |X_i| = delta . (x + X_i) / (|x| + |X_i|);  e_r = x/|x| - X_i/|X_i| = delta/|x| - psi(X_i) e3/|x|
+  // e3 = |x| - |X_i| = delta . (x + X_i) / (|x| + |X_i|);  e_r = x/|x| - X_i/|X_i| = delta/|x| - X_i e3 / (|x| |X_i|)
   const float e3 = __fdividef(fmaf(del0, x0 + Xi.x, fmaf(del1, x1 + Xi.y, del2 * (x2 + Xi.z))), d + di);
-  const float e3rd = e3 * rd;
-  const float e0 = fmaf(del0, rd, -(Xi.x * rdi) * e3rd);
-  const float e1 = fmaf(del1, rd, -(Xi.y * rdi) * e3rd);
-  const float e2 = fmaf(del2, rd, -(Xi.z * rdi) * e3rd);
-  // q = sqrt(c_i c_j); s_c = q / sigma_c^2; r_c^2 = s_c e_c^2
-  const float cc = Xi.w * Xj.w;
-  const float q = cc * rsqrtf(fmaxf(cc, 1e-30f));
+  const float gsc = (e3 * rd) * rdi;
+  const float e0 = fmaf(del0, rd, -(Xi.x * gsc));
+  const float e1 = fmaf(del1, rd, -(Xi.y * gsc));
+  const float e2 = fmaf(del2, rd, -(Xi.z * gsc));
+  // q = sqrt(c_i c_j); s_c = q / sigma_c^2; r_c^2 = s_c e_c^2; omega_c = s_c w_c; rho = w r^2 - min(r^2, k^2)/2
+  const float q = Xi.w * wj;
   const float sr = q * prm.inv_var_ray, sd = q * prm.inv_var_dist;
-  float om[4], cost = 0.f;
+  const float srk = sr * prm.huber_k, sdk = sd * prm.huber_k;
+  float om[4], f[4];
   {
     const float ee[4] = {e0, e1, e2, e3};
     const float ss[4] = {sr, sr, sr, sd};
+    const float sk[4] = {srk, srk, srk, sdk};
 #pragma unroll
     for (int c = 0; c < 4; ++c) {
-      const float r2 = ss[c] * ee[c] * ee[c];
+      const float r2 = (ss[c] * ee[c]) * ee[c];
       const bool out = r2 > prm.huber_k2;
       const float rs = rsqrtf(out ? r2 : 1.f);
-      om[c] = out ? ss[c] * (prm.huber_k * rs) : ss[c];                       // q w / sigma^2
-      cost += out ? fmaf(prm.huber_k, r2 * rs, -0.5f * prm.huber_k2) : 0.5f * r2;
+      om[c] = out ? sk[c] * rs : ss[c];                 // q w / sigma^2
+      f[c] = om[c] * ee[c];
+      acc[35] = fmaf(f[c], ee[c], acc[35]);             // sum w r^2
+      acc[36] += fminf(r2, prm.huber_k2);               // sum min(r^2, k^2)
     }
   }
   const float a = om[0], b = om[1], c = om[2], w3 = om[3];
-  // P = (I - u u^T) / d   (symmetric)
-  const float P00 = (1.f - u0 * u0) * rd, P11 = (1.f - u1 * u1) * rd, P22 = (1.f - u2 * u2) * rd;
-  const float P01 = -(u0 * u1) * rd, P02 = -(u0 * u2) * rd, P12 = -(u1 * u2) * rd;
-  // B = diag(a,b,c) P  (rows scaled)
-  const float B00 = a * P00, B01 = a * P01, B02 = a * P02;
-  const float B10 = b * P01, B11 = b * P11, B12 = b * P12;
-  const float B20 = c * P02, B21 = c * P12, B22 = c * P22;
-  const float wu0 = w3 * u0, wu1 = w3 * u1, wu2 = w3 * u2;
-  // M_vv = P B + w3 u u^T
-  acc[0] += fmaf(P00, B00, fmaf(P01, B10, fmaf(P02, B20, wu0 * u0)));
-  acc[1] += fmaf(P00, B01, fmaf(P01, B11, fmaf(P02, B21, wu0 * u1)));
-  acc[2] += fmaf(P00, B02, fmaf(P01, B12, fmaf(P02, B22, wu0 * u2)));
-  acc[7] += fmaf(P01, B01, fmaf(P11, B11, fmaf(P12, B21, wu1 * u1)));
-  acc[8] += fmaf(P01, B02, fmaf(P11, B12, fmaf(P12, B22, wu1 * u2)));
-  acc[13] += fmaf(P02, B02, fmaf(P12, B12, fmaf(P22, B22, wu2 * u2)));
-  // M_vw(l, m) = sum_k B_kl S_km,  S = -[u]x = [[0,u2,-u1],[-u2,0,u0],[u1,-u0,0]]
-  acc[3] += fmaf(B20, u1, -B10 * u2);
-  acc[4] += fmaf(B00, u2, -B20 * u0);
-  acc[5] += fmaf(B10, u0, -B00 * u1);
-  acc[9] += fmaf(B21, u1, -B11 * u2);
-  acc[10] += fmaf(B01, u2, -B21 * u0);
-  acc[11] += fmaf(B11, u0, -B01 * u1);
-  acc[14] += fmaf(B22, u1, -B12 * u2);
-  acc[15] += fmaf(B02, u2, -B22 * u0);
-  acc[16] += fmaf(B12, u0, -B02 * u1);
+  const float u00 = u0 * u0, u11 = u1 * u1, u22 = u2 * u2, u01 = u0 * u1, u02 = u0 * u2, u12 = u1 * u2;
+  // K = S^T diag(a,b,c) S = M_ww
+  const float K00 = fmaf(b, u22, c * u11), K11 = fmaf(a, u22, c * u00), K22 = fmaf(a, u11, b * u00);
+  const float K01 = -c * u01, K02 = -b * u02, K12 = -a * u12;
+  acc[18] += K00; acc[19] += K01; acc[20] += K02; acc[22] += K11; acc[23] += K12; acc[25] += K22;
+  // G = (S/d) K = M_vw,  S/d = [[0, v2, -v1], [-v2, 0, v0], [v1, -v0, 0]]
+  const float v0 = u0 * rd, v1 = u1 * rd, v2 = u2 * rd;
+  const float G00 = fmaf(v2, K01, -v1 * K02), G01 = fmaf(v2, K11, -v1 * K12), G02 = fmaf(v2, K12, -v1 * K22);
+  const float G10 = fmaf(v0, K02, -v2 * K00), G11 = fmaf(v0, K12, -v2 * K01), G12 = fmaf(v0, K22, -v2 * K02);
+  const float G20 = fmaf(v1, K00, -v0 * K01), G21 = fmaf(v1, K01, -v0 * K11), G22 = fmaf(v1, K02, -v0 * K12);
+  acc[3] += G00; acc[4] += G01; acc[5] += G02;
+  acc[9] += G10; acc[10] += G11; acc[11] += G12;
+  acc[14] += G20; acc[15] += G21; acc[16] += G22;
+  // M_vv = G (S/d)^T + w3 u u^T
+  acc[0] = fmaf(G01, v2, fmaf(-G02, v1, fmaf(w3, u00, acc[0])));
+  acc[1] = fmaf(G02, v0, fmaf(-G00, v2, fmaf(w3, u01, acc[1])));
+  acc[2] = fmaf(G00, v1, fmaf(-G01, v0, fmaf(w3, u02, acc[2])));
+  acc[7] = fmaf(G12, v0, fmaf(-G10, v2, fmaf(w3, u11, acc[7])));
+  acc[8] = fmaf(G10, v1, fmaf(-G11, v0, fmaf(w3, u12, acc[8])));
+  acc[13] = fmaf(G20, v1, fmaf(-G21, v0, fmaf(w3, u22, acc[13])));
   // M_v zeta = w3 d u,  M_zeta zeta = w3 d^2
   const float w3d = w3 * d;
-  acc[6] += w3d * u0;
-  acc[12] += w3d * u1;
-  acc[17] += w3d * u2;
-  acc[27] += w3d * d;
-  // M_ww = S^T diag(a,b,c) S
-  acc[18] += fmaf(b * u2, u2, c * u1 * u1);
-  acc[22] += fmaf(a * u2, u2, c * u0 * u0);
-  acc[25] += fmaf(a * u1, u1, b * u0 * u0);
-  acc[19] -= c * u0 * u1;
-  acc[20] -= b * u0 * u2;
-  acc[23] -= a * u1 * u2;
-  // c_v = B^T e_r + w3 e3 u ; c_w = S^T (Omega e_r) ; c_zeta = w3 d e3
-  const float we3 = w3 * e3;
-  acc[28] += fmaf(B00, e0, fmaf(B10, e1, fmaf(B20, e2, we3 * u0)));
-  acc[29] += fmaf(B01, e0, fmaf(B11, e1, fmaf(B21, e2, we3 * u1)));
-  acc[30] += fmaf(B02, e0, fmaf(B12, e1, fmaf(B22, e2, we3 * u2)));
-  const float f0 = a * e0, f1 = b * e1, f2 = c * e2;
-  acc[31] += fmaf(f2, u1, -f1 * u2);
-  acc[32] += fmaf(f0, u2, -f2 * u0);
-  acc[33] += fmaf(f1, u0, -f0 * u1);
-  acc[34] += we3 * d;
-  acc[35] += cost;
+  acc[6] = fmaf(w3d, u0, acc[6]);
+  acc[12] = fmaf(w3d, u1, acc[12]);
+  acc[17] = fmaf(w3d, u2, acc[17]);
+  acc[27] = fmaf(w3d, d, acc[27]);
+  // c_v = (f - u (u.f)) / d + f3 u ;  c_w = S^T f = u x f ;  c_zeta = f3 d
+  const float uf = fmaf(u0, f[0], fmaf(u1, f[1], u2 * f[2]));
+  acc[28] = fmaf(rd, fmaf(-u0, uf, f[0]), fmaf(f[3], u0, acc[28]));
+  acc[29] = fmaf(rd, fmaf(-u1, uf, f[1]), fmaf(f[3], u1, acc[29]));
+  acc[30] = fmaf(rd, fmaf(-u2, uf, f[2]), fmaf(f[3], u2, acc[30]));
+  acc[31] = fmaf(u1, f[2], fmaf(-u2, f[1], acc[31]));
+  acc[32] = fmaf(u2, f[0], fmaf(-u0, f[2], acc[32]));
+  acc[33] = fmaf(u0, f[1], fmaf(-u1, f[0], acc[33]));
+  acc[34] = fmaf(f[3], d, acc[34]);
 }
 
-__global__ void __launch_bounds__(kAccThreads)
+// Warp reduction of the 40 fp32 thread partials into FP64 warp sums by recursive halving: at every
+// level a lane keeps one half of its slots and hands the other half to its partner, so the whole tree
+// costs 20 + 10 + 5 + 5 + 5 exchanges instead of 40 x 5.  Level 1 exchanges the fp32 partials and
+// converts both operands (the sums are FP64 from here on).  Lanes with (lane & 3) == 0 end up holding
+// the warp totals of slots base .. base + 4, base = 20 b4 + 10 b3 + 5 b2 (bits of the lane index).
+__device__ __forceinline__ void warp_reduce_slots(const float (&acc)[kSlots], double* __restrict__ s_red_warp, const int lane) {
+  double v[20];
+  {
+    const bool up = lane & 16;
+#pragma unroll
+    for (int k = 0; k < 20; ++k) {
+      const float keep = up ? acc[20 + k] : acc[k];
+      const float send = up ? acc[k] : acc[20 + k];
+      v[k] = (double)keep + (double)__shfl_xor_sync(0xffffffffu, send, 16);
+    }
+  }
+  {
+    const bool up = lane & 8;
+#pragma unroll
+    for (int k = 0; k < 10; ++k) {
+      const double keep = up ? v[10 + k] : v[k];
+      const double send = up ? v[k] : v[10 + k];
+      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+  }
+  {
+    const bool up = lane & 4;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+      const double keep = up ? v[5 + k] : v[k];
+      const double send = up ? v[k] : v[5 + k];
+      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    v[k] += __shfl_xor_sync(0xffffffffu, v[k], 2);
+    v[k] += __shfl_xor_sync(0xffffffffu, v[k], 1);
+  }
+  if ((lane & 3) == 0) {
+    const int base = ((lane >> 4) & 1) * 20 + ((lane >> 3) & 1) * 10 + ((lane >> 2) & 1) * 5;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) s_red_warp[base + k] = v[k];
+  }
+}
+
+__global__ void __launch_bounds__(kAccThreads, 2)
 k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, const int32_t* __restrict__ edges,
-             const int32_t* __restrict__ sched, const double* __restrict__ poses, double* __restrict__ partials,
-             int HW, int chunks, DevParams prm) {
-  __shared__ double s_T[12];  // s_ij R_ij [9], t_ij [3]
-  __shared__ double s_red[kAccThreads / 32][kNumAcc];
-  __shared__ unsigned long long s_chk[kAccThreads / 32];
-  __shared__ int s_cnt[kAccThreads / 32];
+             const int32_t* __restrict__ grp_kf, const int32_t* __restrict__ grp_ptr, const int32_t* __restrict__ grp_edge,
+             const double* __restrict__ edgeT, double* __restrict__ partials, int HW, int tiles, DevParams prm) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  float4* s_Xi = reinterpret_cast<float4*>(smem + kOffXi);
+  float2* s_der = reinterpret_cast<float2*>(smem + kOffDer);
+  double* s_red = reinterpret_cast<double*>(smem + kOffRed);
+  double* s_T = reinterpret_cast<double*>(smem + kOffT);
+  long long* s_cnt = reinterpret_cast<long long*>(smem + kOffCnt);
+  unsigned long long* s_chk = reinterpret_cast<unsigned long long*>(smem + kOffChk);
+  uint64_t* s_bar = reinterpret_cast<uint64_t*>(smem + kOffBar);
 
-  const int e = sched[blockIdx.x / chunks];
-  const int chunk = blockIdx.x % chunks;
-  const int i = edges[2 * e], j = edges[2 * e + 1];
-  if (threadIdx.x == 0) {
-    const Sim3d Tij = relative_pose(load_pose(poses + 8 * i), load_pose(poses + 8 * j));
-#pragma unroll
-    for (int k = 0; k < 9; ++k) s_T[k] = Tij.s * Tij.R[k];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) s_T[9 + k] = Tij.t[k];
-  }
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int g = blockIdx.x / tiles, tile = blockIdx.x - g * tiles;
+  const int i = grp_kf[g];
+  const int px0 = tile * kTilePx;
+  const int npx = min(kTilePx, HW - px0);
+  const int nrows = (npx + kAccThreads - 1) / kAccThreads;
+
+  // ---- stage the tile of X_i: one TMA bulk copy per 16 KB, completion on the mbarrier ----
+  if (tid == 0) mbar_init(s_bar, 1);
   __syncthreads();
-  double Td[12];
+  if (tid == 0) {
+    const uint32_t bytes = (uint32_t)npx * (uint32_t)sizeof(float4);
+    mbar_expect_tx(s_bar, bytes);
+    const unsigned char* src = reinterpret_cast<const unsigned char*>(pm + (size_t)i * HW + px0);
+    for (uint32_t off = 0; off < bytes; off += 16384u)
+      tma_bulk_g2s(smem + kOffXi + off, src + off, min(16384u, bytes - off), s_bar);
+  }
+  mbar_wait(s_bar, 0);
+  // per-pixel quantities of X_i shared by all edges leaving i (each thread: its own pixels only)
+#pragma unroll 4
+  for (int r = 0; r < nrows; ++r) {
+    const int p = r * kAccThreads + tid;
+    if (p < npx) {
+      const float4 X = s_Xi[p];
+      const float di2 = fmaxf(fmaf(X.x, X.x, fmaf(X.y, X.y, X.z * X.z)), 1e-20f);
+      const float rdi = rsqrtf(di2);
+      s_der[p] = make_float2(rdi, di2 * rdi);
+    }
+  }
+
+  for (int ei = grp_ptr[g]; ei < grp_ptr[g + 1]; ++ei) {
+    const int e = grp_edge[ei];
+    const int j = edges[2 * e + 1];
+    if (tid < 12) s_T[tid] = edgeT[(size_t)e * 12 + tid];   // s_ij R_ij [9], t_ij [3] (kernel k_edge_prep)
+    __syncthreads();
+    double Td[12];
 #pragma unroll
-  for (int k = 0; k < 12; ++k) Td[k] = s_T[k];
+    for (int k = 0; k < 12; ++k) Td[k] = s_T[k];
 
-  const float4* __restrict__ Pi = pm + (size_t)i * HW;
-  const float4* __restrict__ Pj = pm + (size_t)j * HW;
-  const int32_t* __restrict__ mt = match + (size_t)e * HW;
+    const float4* __restrict__ Pj = pm + (size_t)j * HW;
+    const int32_t* __restrict__ mt = match + (size_t)e * HW + px0;
 
-  float acc[kNumAcc];
+    float acc[kSlots];
 #pragma unroll
-  for (int k = 0; k < kNumAcc; ++k) acc[k] = 0.f;
-  int cnt = 0;
-  unsigned long long chk = 0ull;
+    for (int k = 0; k < kSlots; ++k) acc[k] = 0.f;
+    int cnt = 0;
+    unsigned long long chk = 0ull;
 
-  const int base = chunk * kTilePx + threadIdx.x;
+    auto ld_idx = [&](int r) -> int {
+      const int p = r * kAccThreads + tid;
+      return (p < npx) ? __ldcs(mt + p) : -1;
+    };
+    auto gather = [&](int n) -> float4 {
+      return ((unsigned)n < (unsigned)HW) ? __ldg(Pj + n) : make_float4(0.f, 0.f, 0.f, -1.f);
+    };
+    auto process = [&](int r, int n, const float4 Xj) {
+      if (Xj.w >= 0.f) {
+        const int p = r * kAccThreads + tid;
+        const float4 Xi = s_Xi[p];
+        if (Xi.w >= 0.f) {
+          const float2 der = s_der[p];
+          // delta = T_ij X_j - X_i in FP64: |delta| ~ noise << |x|; in fp32 it would carry ~ulp(|x|) per match
+          const double Xjx = (double)Xj.x, Xjy = (double)Xj.y, Xjz = (double)Xj.z;
+          const float del0 = (float)fma(Td[0], Xjx, fma(Td[1], Xjy, fma(Td[2], Xjz, Td[9] - (double)Xi.x)));
+          const float del1 = (float)fma(Td[3], Xjx, fma(Td[4], Xjy, fma(Td[5], Xjz, Td[10] - (double)Xi.y)));
+          const float del2 = (float)fma(Td[6], Xjx, fma(Td[7], Xjy, fma(Td[8], Xjz, Td[11] - (double)Xi.z)));
+          accumulate_match(acc, del0, del1, del2, Xi, der.x, der.y, Xj.w, prm);
+          ++cnt;
+          chk += (unsigned long long)(px0 + p) * (unsigned long long)HW + (unsigned long long)n;
+        }
+      }
+    };
+
+    // software pipeline: indices two batches ahead, gathers one batch ahead (batch = 2 rows)
+    int nA0 = ld_idx(0), nA1 = ld_idx(1);
+    int nB0 = ld_idx(2), nB1 = ld_idx(3);
+    float4 XA0 = gather(nA0), XA1 = gather(nA1);
 #pragma unroll 1
-  for (int k0 = 0; k0 < kPxPerThread; k0 += kBatch) {
-    int n[kBatch];
-    float4 Xi[kBatch], Xj[kBatch];
-    bool ok[kBatch];
-#pragma unroll
-    for (int b = 0; b < kBatch; ++b) {
-      const int m = base + (k0 + b) * kAccThreads;
-      n[b] = (m < HW) ? __ldg(mt + m) : -1;
+    for (int r = 0; r < nrows; r += 2) {
+      const float4 XB0 = gather(nB0), XB1 = gather(nB1);
+      const int nC0 = ld_idx(r + 4), nC1 = ld_idx(r + 5);
+      process(r, nA0, XA0);
+      process(r + 1, nA1, XA1);
+      nA0 = nB0; nA1 = nB1; XA0 = XB0; XA1 = XB1; nB0 = nC0; nB1 = nC1;
     }
-#pragma unroll
-    for (int b = 0; b < kBatch; ++b) {
-      const int m = base + (k0 + b) * kAccThreads;
-      ok[b] = (n[b] >= 0) && (n[b] < HW);
-      if (ok[b]) {
-        Xi[b] = ldg_f4(Pi + m);
-        Xj[b] = ldg_f4(Pj + n[b]);
-      }
-    }
-#pragma unroll
-    for (int b = 0; b < kBatch; ++b) {
-      const int m = base + (k0 + b) * kAccThreads;
-      if (ok[b] && Xi[b].w > prm.conf_min && Xj[b].w > prm.conf_min) {
-        accumulate_match(acc, Xi[b], Xj[b], Td, prm);
-        ++cnt;
-        chk += (unsigned long long)m * (unsigned long long)HW + (unsigned long long)n[b];
-      }
-    }
-  }
 
-  // thread partial (<= 16 fp32 terms) -> fp64; warp shuffle tree; fixed-order cross-warp sum
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // ---- thread partials (fp32, <= 16 terms) -> FP64 warp sums -> fixed-order cross-warp sum ----
+    warp_reduce_slots(acc, s_red + warp * kSlots, lane);
 #pragma unroll
-  for (int k = 0; k < kNumAcc; ++k) {
-    double v = (double)acc[k];
+    for (int o = 16; o > 0; o >>= 1) {
+      cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+      chk += __shfl_xor_sync(0xffffffffu, chk, o);
+    }
+    if (lane == 0) { s_cnt[warp] = cnt; s_chk[warp] = chk; }
+    __syncthreads();
+    double* out = partials + ((size_t)e * tiles + tile) * kPartialStride;
+    if (tid < kSlotCnt) {
+      double v = 0.0;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    if (lane == 0) s_red[warp][k] = v;
-  }
+      for (int w = 0; w < kWarps; ++w) v += s_red[w * kSlots + tid];
+      out[tid] = v;
+    } else if (tid == kSlotCnt) {
+      long long c = 0;
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
-    chk += __shfl_xor_sync(0xffffffffu, chk, o);
-  }
-  if (lane == 0) { s_cnt[warp] = cnt; s_chk[warp] = chk; }
-  __syncthreads();
-  double* out = partials + ((size_t)e * chunks + chunk) * kPartialStride;
-  if (threadIdx.x < kNumAcc) {
-    double v = 0.0;
+      for (int w = 0; w < kWarps; ++w) c += s_cnt[w];
+      reinterpret_cast<long long*>(out)[kSlotCnt] = c;
+    } else if (tid == kSlotChk) {
+      unsigned long long h = 0ull;
 #pragma unroll
-    for (int w = 0; w < kAccThreads / 32; ++w) v += s_red[w][threadIdx.x];
-    out[threadIdx.x] = v;
-  } else if (threadIdx.x == 64) {
-    long long c = 0;
-    unsigned long long h = 0ull;
-#pragma unroll
-    for (int w = 0; w < kAccThreads / 32; ++w) { c += s_cnt[w]; h += s_chk[w]; }
-    reinterpret_cast<long long*>(out)[36] = c;
-    reinterpret_cast<unsigned long long*>(out)[37] = h;
+      for (int w = 0; w < kWarps; ++w) h += s_chk[w];
+      reinterpret_cast<unsigned long long*>(out)[kSlotChk] = h;
+    }
   }
 }
 
-// Kernel 2: per edge, sum the chunk partials in chunk order (fp64), then the adjoint congruence
+// a1: per-edge pose prep, T_ij = T_i^-1 T_j -> s_ij R_ij [9] row-major, t_ij [3], FP64
+__global__ void __launch_bounds__(128)
+k_edge_prep(const double* __restrict__ poses, const int32_t* __restrict__ edges, double* __restrict__ edgeT, int E) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= E) return;
+  const Sim3d Tij = relative_pose(load_pose(poses + 8 * edges[2 * e]), load_pose(poses + 8 * edges[2 * e + 1]));
+  double* o = edgeT + (size_t)e * 12;
+#pragma unroll
+  for (int k = 0; k < 9; ++k) o[k] = Tij.s * Tij.R[k];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) o[9 + k] = Tij.t[k];
+}
+
+// Kernel 2: per edge, sum the tile partials in tile order (FP64), then the adjoint congruence
 // A_e = Ad^T M Ad, b_e = Ad^T c with Ad = Ad_{T_i^-1}.
 __global__ void __launch_bounds__(64)
 k_finalize(const double* __restrict__ partials, const int32_t* __restrict__ edges, const double* __restrict__ poses,
            double* __restrict__ blocks35, double* __restrict__ edge_cost, int32_t* __restrict__ n_valid,
            unsigned long long* __restrict__ checksum, int chunks) {
-  __shared__ double s_sum[kNumAcc];
+  __shared__ double s_sum[kSlots];
   __shared__ double s_M[49], s_Ad[49], s_T[49];
   const int e = blockIdx.x, t = threadIdx.x;
   const double* p = partials + (size_t)e * chunks * kPartialStride;
-  if (t < kNumAcc) {
+  if (t < kSlotCnt) {
     double v = 0.0;
     for (int c = 0; c < chunks; ++c) v += p[(size_t)c * kPartialStride + t];
     s_sum[t] = v;
-  } else if (t == 36) {
+  } else if (t == kSlotCnt) {
     long long v = 0;
-    for (int c = 0; c < chunks; ++c) v += reinterpret_cast<const long long*>(p + (size_t)c * kPartialStride)[36];
+    for (int c = 0; c < chunks; ++c) v += reinterpret_cast<const long long*>(p + (size_t)c * kPartialStride)[kSlotCnt];
     n_valid[e] = (int32_t)v;
-  } else if (t == 37) {
+  } else if (t == kSlotChk) {
     unsigned long long v = 0ull;
-    for (int c = 0; c < chunks; ++c) v += reinterpret_cast<const unsigned long long*>(p + (size_t)c * kPartialStride)[37];
+    for (int c = 0; c < chunks; ++c) v += reinterpret_cast<const unsigned long long*>(p + (size_t)c * kPartialStride)[kSlotChk];
     checksum[e] = v;
-  } else if (t == 38) {
+  } else if (t == 39) {
     adjoint_of_inverse(load_pose(poses + 8 * edges[2 * e]), s_Ad);
   }
   __syncthreads();
@@ -277,16 +381,20 @@ k_finalize(const double* __restrict__ partials, const int32_t* __restrict__ edge
     for (int k = 0; k < 7; ++k) v += s_Ad[7 * k + r] * s_sum[28 + k];
     blocks35[(size_t)e * 35 + 28 + r] = v;
   } else if (t == 56) {
-    edge_cost[e] = s_sum[35];
+    edge_cost[e] = s_sum[35] - 0.5 * s_sum[36];   // rho = w r^2 - min(r^2, kappa^2) / 2
   }
 }
 
-// packs [N][HW][3] points + [N][HW] confidences into float4 (x, y, z, c)
-__global__ void k_pack(const float* __restrict__ pts, const float* __restrict__ conf, float4* __restrict__ pm, size_t total) {
+// packs [N][HW][3] points + [N][HW] confidences into float4 (x, y, z, w): w = sqrt(c) when the pixel
+// passes the confidence test c > conf_min (decided here, exactly, on the caller's c), else -1.
+__global__ void k_pack(const float* __restrict__ pts, const float* __restrict__ conf, float4* __restrict__ pm, size_t total,
+                       float conf_min) {
   size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   const size_t stride = (size_t)gridDim.x * blockDim.x;
-  for (; idx < total; idx += stride)
-    pm[idx] = make_float4(pts[3 * idx], pts[3 * idx + 1], pts[3 * idx + 2], conf[idx]);
+  for (; idx < total; idx += stride) {
+    const float c = conf[idx];
+    pm[idx] = make_float4(pts[3 * idx], pts[3 * idx + 1], pts[3 * idx + 2], (c > conf_min) ? sqrtf(fmaxf(c, 0.f)) : -1.f);
+  }
 }
 
 }  // namespace
@@ -294,27 +402,35 @@ __global__ void k_pack(const float* __restrict__ pts, const float* __restrict__ 
 cudaError_t launch_pack(Ctx* c, const float* d_points, const float* d_conf) {
   const size_t total = (size_t)c->N * c->HW;
   const int grid = (int)((total + 255) / 256 < 148 * 16 ? (total + 255) / 256 : 148 * 16);
-  k_pack<<<grid, 256, 0, c->stream>>>(d_points, d_conf, c->pm, total);
+  k_pack<<<grid, 256, 0, c->stream>>>(d_points, d_conf, c->pm, total, c->prm.conf_min);
   ++c->launches;
   return cudaGetLastError();
 }
 
 cudaError_t launch_accumulate(Ctx* c) {
   if (c->E == 0) return cudaSuccess;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(k_accumulate, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAccSmem);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
   DevParams p;
   p.inv_var_ray = 1.0f / (c->prm.sigma_ray * c->prm.sigma_ray);
   p.inv_var_dist = 1.0f / (c->prm.sigma_dist * c->prm.sigma_dist);
   p.huber_k = c->prm.huber_k;
   p.huber_k2 = c->prm.huber_k * c->prm.huber_k;
-  p.conf_min = c->prm.conf_min;
-  k_accumulate<<<c->E * c->chunks, kAccThreads, 0, c->stream>>>(c->pm, c->match, c->edges, c->sched, c->poses,
-                                                                 c->partials, c->HW, c->chunks, p);
+  k_edge_prep<<<(c->E + 127) / 128, 128, 0, c->stream>>>(c->poses, c->edges, c->edgeT, c->E);
   cudaError_t err = cudaGetLastError();
+  if (err != cudaSuccess) return err;
+  k_accumulate<<<c->n_groups * c->chunks, kAccThreads, kAccSmem, c->stream>>>(
+      c->pm, c->match, c->edges, c->grp_kf, c->grp_ptr, c->grp_edge, c->edgeT, c->partials, c->HW, c->chunks, p);
+  err = cudaGetLastError();
   if (err != cudaSuccess) return err;
   if (c->profiling) cudaEventRecord(c->ev[1], c->stream);
   k_finalize<<<c->E, 64, 0, c->stream>>>(c->partials, c->edges, c->poses, c->blocks35, c->edge_cost, c->n_valid,
                                          c->checksum, c->chunks);
-  c->launches += 2;
+  c->launches += 3;
   return cudaGetLastError();
 }
 

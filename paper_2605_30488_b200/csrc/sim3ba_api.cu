@@ -83,7 +83,7 @@ cudaError_t upload(T** dst, const std::vector<T>& src, cudaStream_t s) {
 }
 
 void free_all(Ctx* c) {
-  cudaFree(c->pm); cudaFree(c->edges); cudaFree(c->sched); cudaFree(c->fixed_mask); cudaFree(c->poses);
+  cudaFree(c->pm); cudaFree(c->edges); cudaFree(c->grp_kf); cudaFree(c->grp_ptr); cudaFree(c->grp_edge); cudaFree(c->edgeT); cudaFree(c->fixed_mask); cudaFree(c->poses);
   cudaFree(c->kf_ptr); cudaFree(c->kf_edge); cudaFree(c->pair_kf); cudaFree(c->pair_ptr); cudaFree(c->pair_edge);
   cudaFree(c->partials); cudaFree(c->blocks35); cudaFree(c->edge_cost); cudaFree(c->n_valid); cudaFree(c->checksum);
   cudaFree(c->Hd); cudaFree(c->L); cudaFree(c->g); cudaFree(c->rhs); cudaFree(c->ysol); cudaFree(c->Dfac); cudaFree(c->Dinv);
@@ -194,16 +194,27 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
     c->h_fixed[h_fixed_kf[k]] = 1;
   }
   build_bookkeeping(c);
-  std::vector<int32_t> sched(n_edges);
-  std::iota(sched.begin(), sched.end(), 0);
-  std::stable_sort(sched.begin(), sched.end(), [&](int32_t a, int32_t b) {
+  // kernel-1 schedule: edges grouped by their first endpoint i (the tile of X_i is staged once per group)
+  std::vector<int32_t> grp_edge(n_edges), grp_kf, grp_ptr(1, 0);
+  std::iota(grp_edge.begin(), grp_edge.end(), 0);
+  std::stable_sort(grp_edge.begin(), grp_edge.end(), [&](int32_t a, int32_t b) {
     return std::make_pair(c->h_edges[2 * a], c->h_edges[2 * a + 1]) < std::make_pair(c->h_edges[2 * b], c->h_edges[2 * b + 1]);
   });
+  for (int k = 0; k < n_edges; ++k) {
+    const int32_t i = c->h_edges[2 * grp_edge[k]];
+    if (grp_kf.empty() || grp_kf.back() != i) { grp_kf.push_back(i); if (k) grp_ptr.push_back(k); }
+  }
+  grp_ptr.push_back(n_edges);
+  if (n_edges == 0) grp_ptr.assign(1, 0);
+  c->n_groups = (int)grp_kf.size();
 
   const size_t NHW = (size_t)c->N * c->HW, np2 = (size_t)c->npad * c->npad;
   CUB(dev_alloc(&c->pm, NHW));
   CUB(upload(&c->edges, c->h_edges, c->stream));
-  CUB(upload(&c->sched, sched, c->stream));
+  CUB(upload(&c->grp_kf, grp_kf, c->stream));
+  CUB(upload(&c->grp_ptr, grp_ptr, c->stream));
+  CUB(upload(&c->grp_edge, grp_edge, c->stream));
+  CUB(dev_alloc(&c->edgeT, (size_t)c->E * 12));
   CUB(upload(&c->fixed_mask, c->h_fixed, c->stream));
   CUB(upload(&c->kf_ptr, c->h_kf_ptr, c->stream));
   CUB(upload(&c->kf_edge, c->h_kf_edge, c->stream));
@@ -261,6 +272,8 @@ int sim3ba_set_params(sim3ba_ctx* h, const sim3ba_params* p) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
   if (!params_ok(p)) return fail(c, SIM3BA_ERR_INVALID_ARG, "invalid params");
+  if (p->conf_min != c->prm.conf_min)
+    return fail(c, SIM3BA_ERR_INVALID_ARG, "conf_min is fixed at sim3ba_create (the validity mask is baked into the packed pointmap)");
   c->prm = *p;
   return SIM3BA_OK;
 }

@@ -13,7 +13,11 @@ namespace sim3ba {
 
 constexpr int kTilePx = 4096;        // pixels of one edge handled by one accumulate CTA
 constexpr int kAccThreads = 256;
-constexpr int kPartialStride = 40;   // doubles per (edge, chunk) partial: 28 M + 7 c + cost + n_valid + checksum (+2 pad)
+// doubles per (edge, tile) partial record: [0..27] upper triangle of M = sum J_xi^T Omega J_xi (row-major,
+// r <= c; (3,6), (4,6), (5,6) are structurally zero), [28..34] c = sum J_xi^T Omega e, [35] sum w r^2,
+// [36] sum min(r^2, kappa^2) (robust cost = [35] - [36]/2), [37] n_valid (int64 bits), [38] checksum (uint64 bits)
+constexpr int kPartialStride = 40;
+constexpr int kSlotCnt = 37, kSlotChk = 38;
 constexpr int kNB = 64;              // Cholesky block size
 
 struct DevParams {       // robust-kernel constants, fp32, passed by value to kernel 1
@@ -21,7 +25,6 @@ struct DevParams {       // robust-kernel constants, fp32, passed by value to ke
   float inv_var_dist;    // 1 / sigma_d^2
   float huber_k;
   float huber_k2;
-  float conf_min;
 };
 
 struct Ctx {
@@ -32,7 +35,10 @@ struct Ctx {
   float4* pm = nullptr;            // [N][HW] packed (x, y, z, conf)
   const int32_t* match = nullptr;  // borrowed [E][HW]
   int32_t* edges = nullptr;        // [E][2]
-  int32_t* sched = nullptr;        // [E] edge processing order (sorted by first endpoint)
+  // kernel-1 schedule: keyframes with outgoing edges (ascending) and their edges (ascending j, then e)
+  int32_t *grp_kf = nullptr, *grp_ptr = nullptr, *grp_edge = nullptr;
+  int n_groups = 0;
+  double* edgeT = nullptr;         // [E][12] s_ij R_ij, t_ij of the current poses (a1)
   uint8_t* fixed_mask = nullptr;   // [N]
   double* poses = nullptr;         // [N][8]
   // bookkeeping (device + host)
