@@ -145,13 +145,24 @@ int sim3ba_get_bookkeeping(sim3ba_ctx* ctx, const int32_t** h_kf_ptr, const int3
  * tests: oracle (H, g) -> GPU solver).  d_H [7N][7N] row-major symmetric double, d_g [7N]. */
 int sim3ba_load_system(sim3ba_ctx* ctx, const double* d_H, const double* d_g);
 
+/* Solver plan (a7).  mode 0 (default): the Cholesky walks only the non-zero 64x64 tiles of L (symbolic
+ * tile-level factorisation of the keyframe graph, fill included, computed at create); mode 1: every
+ * lower tile (the dense blocked factorisation; also used for systems given by sim3ba_load_system).
+ * Both give the same tau up to rounding. */
+int sim3ba_set_solver_mode(sim3ba_ctx* ctx, int32_t mode);
+/* Host outputs (each may be NULL): non-zero tiles of the active plan, lower tiles of the dense plan,
+ * flop count of the active plan (factor + both triangular solves, at tile granularity), CTAs of
+ * the last persistent solve launch. */
+int sim3ba_get_solver_info(sim3ba_ctx* ctx, int32_t* h_n_tiles, int32_t* h_n_tiles_dense, double* h_flops,
+                           int32_t* h_grid);
+
 /* Number of kernels this library launched on the context since create (for bench accounting). */
 int sim3ba_get_launch_count(sim3ba_ctx* ctx, int64_t* h_count);
 
 /* Device time in milliseconds of the phases of the last sim3ba_step / build / solve, measured
  * with CUDA events on the context's stream: [0] kernel 1 (per-match accumulate, a1-a5 partials),
- * [1] kernel 2 (per-edge reduce + adjoint congruence, gradient, cost), [2] assembly (a6, summed over
- * attempts), [3] factor + triangular solves (a7, summed over attempts), [4] retraction (a8),
+ * [1] kernel 2 (per-edge reduce + adjoint congruence, gradient, cost), [2] damped tile assembly (a6, first
+ * attempt), [3] factor + triangular solves (a7, incl. re-assembly of later attempts), [4] retraction (a8),
  * [5..7] reserved (0).  Synchronises.  Only recorded after sim3ba_set_profiling(ctx, 1). */
 int sim3ba_set_profiling(sim3ba_ctx* ctx, int32_t enable);
 int sim3ba_get_phase_ms(sim3ba_ctx* ctx, float h_ms[8]);

@@ -19,6 +19,7 @@ EXPORTS = (
     "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_host",
     "sim3ba_retract", "sim3ba_get_edge_stats", "sim3ba_get_edge_blocks", "sim3ba_get_system",
     "sim3ba_get_update", "sim3ba_get_bookkeeping", "sim3ba_load_system", "sim3ba_get_launch_count",
+    "sim3ba_set_solver_mode", "sim3ba_get_solver_info",
     "sim3ba_set_profiling", "sim3ba_get_phase_ms", "sim3ba_copy_d2d", "sim3ba_last_error", "sim3ba_version",
 )
 
@@ -68,6 +69,8 @@ def load_library() -> C.CDLL:
         "sim3ba_get_bookkeeping": [vp, P(vp), P(vp), P(i32), P(vp), P(vp), P(vp)],
         "sim3ba_load_system": [vp, vp, vp],
         "sim3ba_get_launch_count": [vp, P(i64)],
+        "sim3ba_set_solver_mode": [vp, i32],
+        "sim3ba_get_solver_info": [vp, P(i32), P(i32), P(C.c_double), P(i32)],
         "sim3ba_set_profiling": [vp, i32],
         "sim3ba_get_phase_ms": [vp, P(C.c_float)],
         "sim3ba_copy_d2d": [vp, vp, vp, C.c_uint64],
@@ -225,6 +228,15 @@ class Sim3BA:
         assert H.is_cuda and H.dtype == t.float64 and H.is_contiguous() and tuple(H.shape) == (self.n, self.n)
         assert g.is_cuda and g.dtype == t.float64 and g.is_contiguous() and tuple(g.shape) == (self.n,)
         self._check(self.lib.sim3ba_load_system(self._h, H.data_ptr(), g.data_ptr()))
+
+    def set_solver_mode(self, mode: int):
+        """0: tile-sparse plan of the graph (default); 1: dense plan (every lower tile)."""
+        self._check(self.lib.sim3ba_set_solver_mode(self._h, int(mode)))
+
+    def solver_info(self) -> Dict[str, float]:
+        nt, ntd, fl, gr = C.c_int32(), C.c_int32(), C.c_double(), C.c_int32()
+        self._check(self.lib.sim3ba_get_solver_info(self._h, C.byref(nt), C.byref(ntd), C.byref(fl), C.byref(gr)))
+        return dict(n_tiles=nt.value, n_tiles_dense=ntd.value, flops=fl.value, grid=gr.value)
 
     def launch_count(self) -> int:
         n = C.c_int64()

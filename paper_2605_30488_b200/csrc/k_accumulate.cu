@@ -24,7 +24,7 @@ namespace sim3ba {
 
 namespace {
 
-constexpr int kRows = kTilePx / kAccThreads;   // 16 pixels per thread per (edge, tile)
+static_assert(kTilePx / kAccThreads == 16, "precision plan: <= 16 fp32 terms per thread partial");
 constexpr int kWarps = kAccThreads / 32;
 constexpr int kSlots = kPartialStride;         // 40 reduction slots (layout: sim3ba_internal.cuh)
 
@@ -63,6 +63,13 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_
                : "memory");
 }
 
+// MUFU.RSQ without the denormal pre/post-scaling of rsqrtf(): every argument here is >= 1e-20 or > kappa^2
+__device__ __forceinline__ float rsq(float v) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
+  return r;
+}
+
 // One valid match: accumulate J_xi^T Omega J_xi (25 structurally non-zero upper-triangular entries),
 // J_xi^T Omega e (7) and the two robust-cost sums into acc[].
 //   del = T_ij X_j - X_i (fp32 rounding of the FP64 value), Xi = (X_i, sqrt c_i), rdi = 1/|X_i|, di = |X_i|,
@@ -72,7 +79,7 @@ __device__ __forceinline__ void accumulate_match(float (&acc)[kSlots], const flo
                                                  const DevParams& prm) {
   const float x0 = Xi.x + del0, x1 = Xi.y + del1, x2 = Xi.z + del2;   // x = T_ij X_j
   const float d2 = fmaxf(fmaf(x0, x0, fmaf(x1, x1, x2 * x2)), 1e-20f);
-  const float rd = rsqrtf(d2);
+  const float rd = rsq(d2);
   const float d = d2 * rd;
   const float u0 = x0 * rd, u1 = x1 * rd, u2 = x2 * rd;
   // e3 = |x| - |X_i| = delta . (x + X_i) / (|x| + |X_i|);  e_r = x/|x| - X_i/|X_i| = delta/|x| - X_i e3 / (|x| |X_i|)
@@ -94,7 +101,7 @@ __device__ __forceinline__ void accumulate_match(float (&acc)[kSlots], const flo
     for (int c = 0; c < 4; ++c) {
       const float r2 = (ss[c] * ee[c]) * ee[c];
       const bool out = r2 > prm.huber_k2;
-      const float rs = rsqrtf(out ? r2 : 1.f);
+      const float rs = rsq(out ? r2 : 1.f);
       om[c] = out ? sk[c] * rs : ss[c];                 // q w / sigma^2
       f[c] = om[c] * ee[c];
       acc[35] = fmaf(f[c], ee[c], acc[35]);             // sum w r^2
@@ -223,7 +230,7 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
     if (p < npx) {
       const float4 X = s_Xi[p];
       const float di2 = fmaxf(fmaf(X.x, X.x, fmaf(X.y, X.y, X.z * X.z)), 1e-20f);
-      const float rdi = rsqrtf(di2);
+      const float rdi = rsq(di2);
       s_der[p] = make_float2(rdi, di2 * rdi);
     }
   }

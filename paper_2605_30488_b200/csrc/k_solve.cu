@@ -1,24 +1,27 @@
-// Kernels 3+4 of the Sim(3) GN step as ONE persistent cooperative kernel: damped assembly of the
-// dense system (a6), blocked FP64 Cholesky, forward and backward triangular solves (a7) and the
-// epsilon escalation of PAPER.md:122 -- all on the device, no host round trip between attempts.
+// Kernels 3+4 of the Sim(3) GN step: damped tile assembly (a6) and ONE persistent cooperative kernel
+// for the blocked FP64 Cholesky, the forward and backward triangular solves (a7) and the epsilon
+// escalation of PAPER.md:122 -- all on the device, no host round trip between attempts.
 //
 //   Eq. (7)  PAPER.md:120   (H + lambda diag(H) + eps_r I) tau = -g
 //   PAPER.md:122            eps_r = eps0 * 100^r on factorisation failure, r < max_attempts, else tau = 0
 //
-// Layout: L is npad x npad row-major (npad multiple of NB = 64, identity padding), lower triangle.
-// One attempt:
-//   phase 0  every CTA zero-fills its share of the lower-triangular 64x64 tiles, then the 7x7 blocks
-//            are gathered from the per-edge blocks through the bookkeeping CSRs (fixed summation
-//            order, no atomics); gauge keyframes get identity blocks; rhs = -g.
-//   panel k  phase A: each participating CTA re-factorises the diagonal block L_kk in registers /
-//            shared memory (redundant work instead of one more grid-wide dependency), forward-
-//            substitutes y_k = L_kk^-1 b_k, solves its row blocks L_ik = A_ik L_kk^-T and updates
-//            b_i -= L_ik y_k.   phase B: trailing update C_ij -= L_ik L_jk^T over the lower tiles.
-//   back     L^T tau = y block by block, last to first.
-// Grid-wide barriers are a monotonically increasing global counter (all CTAs are co-resident:
-// the kernel is launched with cudaLaunchCooperativeKernel).
+// Layout: L is npad x npad row-major (npad multiple of NB = 64, identity padding), lower triangle,
+// addressed in 64x64 tiles.  The kernel walks the tile plan built at create (solve_plan.cu): only the
+// non-zero tiles of L (fill included) are assembled, factorised and used; the dense plan lists all.
+// Right-looking, per block column k:
+//   phase A  every CTA that owns a tile (i, k) re-factorises the diagonal tile L_kk in shared memory
+//            (redundant work instead of one more grid-wide dependency): 8-column micro-panels by one
+//            warp in registers (pivots and column broadcasts by warp shuffles), rank-8 trailing
+//            updates by all warps; then X L_kk^T = A_ik by the same micro-panel scheme, with the
+//            right-hand side riding along as a 65th row (y_k = L_kk^-1 b_k) and b_i -= L_ik y_k.
+//   phase B  trailing update C_ij -= L_ik L_jk^T over the pairs of non-zero tiles of column k, on the
+//            FP64 tensor pipe (mma.sync.m8n8k4.f64 = DMMA.8x8x4).
+//   back     L^T tau = y block by block, last to first, over the row lists.
+// Grid-wide barriers are a monotonically increasing global counter (all CTAs are co-resident: the
+// kernel is launched with cudaLaunchCooperativeKernel, with no more CTAs than the widest phase needs).
 #include <cooperative_groups.h>
 
+#include "assemble_tile.cuh"
 #include "sim3ba_internal.cuh"
 
 namespace sim3ba {
@@ -26,21 +29,29 @@ namespace sim3ba {
 namespace {
 
 constexpr int NB = kNB;          // 64
-constexpr int LDS = NB + 1;      // padded shared-memory row stride (doubles)
-constexpr int KC = 32, LDK = KC + 1;
+constexpr int LDD = NB + 1;      // diagonal tile / TRSM tile in shared memory (odd stride: column walks are conflict-free)
+constexpr int LDT = NB + 4;      // DMMA operand tiles (LDT % 16 == 4: fragment loads are conflict-free)
 constexpr int kSolveThreads = 256;
 
 struct SolveArgs {
+  AsmArgs as;
   double* L; int npad, n, nb;
-  const double* blocks35; const int32_t *kf_ptr, *kf_edge, *pair_kf, *pair_ptr, *pair_edge;
-  const uint8_t* fixed; int N, n_pairs;
-  const double* dense;           // non-NULL: caller-supplied dense H [n][n] instead of the blocks
-  const double* g;
-  double *rhs, *ysol, *Dfac, *Dinv, *tau;
-  double lambda, eps0; int max_attempts;
+  const int32_t *col_ptr, *col_rows, *row_ptr, *row_cols, *tiles; int n_tiles;
+  double *rhs, *ysol, *Dinv, *tau;
+  double eps0; int max_attempts;
   int32_t* status;               // [0] failure flag of the running attempt, [1] attempts used, [2] ok
   double* eps_used;
   unsigned int* bar;
+};
+
+struct Smem {
+  double D[NB * LDD];            // diagonal tile L_kk
+  double A[(NB + 1) * LDT];      // TRSM tile + right-hand-side row (stride LDD) / DMMA operand A (stride LDT)
+  double B[NB * LDT];            // DMMA operand B
+  double y[NB];
+  double dinv[NB];               // 1 / diag(L_kk)
+  double red[256];
+  int flag;
 };
 
 __device__ __forceinline__ unsigned int ld_acquire(const unsigned int* p) {
@@ -49,265 +60,274 @@ __device__ __forceinline__ unsigned int ld_acquire(const unsigned int* p) {
   return v;
 }
 
+__device__ __forceinline__ int ld_flag(const int32_t* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+
 __device__ __forceinline__ void grid_barrier(unsigned int* bar, unsigned int G, unsigned int& gen) {
   __syncthreads();
   gen += 1;
-  if (threadIdx.x == 0) {
+  if (G > 1 && threadIdx.x == 0) {
     __threadfence();
     atomicAdd(bar, 1u);
     const unsigned int target = gen * G;
-    while (ld_acquire(bar) < target) { __nanosleep(32); }
+    while (ld_acquire(bar) < target) { }
     __threadfence();
   }
   __syncthreads();
 }
 
-__device__ __forceinline__ int tri_index(int r, int c) { return r * 7 - r * (r - 1) / 2 + (c - r); }
-
-// ---- phase 0 -----------------------------------------------------------------------------------
-__device__ void assemble_zero(const SolveArgs& a, int G) {
-  const int nb = a.nb;
-  const int ntiles = nb * (nb + 1) / 2;
-  for (int t = blockIdx.x; t < ntiles; t += G) {
-    int ti = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
-    while ((ti + 1) * (ti + 2) / 2 <= t) ++ti;
-    while (ti * (ti + 1) / 2 > t) --ti;
-    const int tj = t - ti * (ti + 1) / 2;
-    double2* base = reinterpret_cast<double2*>(a.L + (size_t)ti * NB * a.npad + (size_t)tj * NB);
-    const size_t ld2 = (size_t)a.npad / 2;
-    for (int idx = threadIdx.x; idx < NB * NB / 2; idx += kSolveThreads) {
-      const int r = idx / (NB / 2), c2 = idx % (NB / 2);
-      base[r * ld2 + c2] = make_double2(0.0, 0.0);
-    }
-  }
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-__device__ void assemble_blocks(const SolveArgs& a, int G, double eps) {
-  const int grp = threadIdx.x >> 6, t = threadIdx.x & 63;   // 4 groups of 64 threads
-  const int r = t / 7, c = t % 7;
-  const size_t ld = (size_t)a.npad;
-  const int items = a.N + a.n_pairs;
-  for (int it = blockIdx.x * 4 + grp; it < items; it += G * 4) {
-    if (t >= 49) continue;
-    if (it < a.N) {
-      if (r < c) continue;
-      double v = 0.0;
-      if (a.fixed[it]) {
-        v = (r == c) ? 1.0 : 0.0;
-      } else {
-        const int idx = tri_index(c, r);
-        for (int p = a.kf_ptr[it]; p < a.kf_ptr[it + 1]; ++p) v += a.blocks35[(size_t)a.kf_edge[p] * 35 + idx];
-      }
-      if (r == c) v = v * (1.0 + a.lambda) + eps;
-      a.L[(size_t)(7 * it + r) * ld + 7 * it + c] = v;
-    } else {
-      const int p = it - a.N;
-      const int hi = a.pair_kf[2 * p], lo = a.pair_kf[2 * p + 1];
-      if (a.fixed[hi] || a.fixed[lo]) continue;
-      const int idx = r <= c ? tri_index(r, c) : tri_index(c, r);
-      double v = 0.0;
-      for (int q = a.pair_ptr[p]; q < a.pair_ptr[p + 1]; ++q) v += a.blocks35[(size_t)a.pair_edge[q] * 35 + idx];
-      a.L[(size_t)(7 * hi + r) * ld + 7 * lo + c] = -v;
-    }
-  }
-  if (blockIdx.x == 0)
-    for (int k = a.n + threadIdx.x; k < a.npad; k += kSolveThreads) a.L[(size_t)k * ld + k] = 1.0;
-}
-
-__device__ void assemble_dense(const SolveArgs& a, int G, double eps) {
-  const size_t ld = (size_t)a.npad;
-  for (int r = blockIdx.x; r < a.npad; r += G) {
-    for (int c = threadIdx.x; c <= r; c += kSolveThreads) {
-      double v;
-      if (r >= a.n || c >= a.n) v = (r == c) ? 1.0 : 0.0;
-      else {
-        if (a.fixed[r / 7] || a.fixed[c / 7]) v = (r == c) ? 1.0 : 0.0;
-        else v = a.dense[(size_t)r * a.n + c];
-        if (r == c) v = v * (1.0 + a.lambda) + eps;
-      }
-      a.L[r * ld + c] = v;
-    }
-  }
-}
-
-// ---- diagonal block --------------------------------------------------------------------------
-// Cholesky of the 64x64 block held as: thread (r = tid/4, g = tid%4) owns columns 4q+g of row r.
-// Result is written to the shared block D (lower triangle).  Returns false on a bad pivot.
-__device__ bool potrf_block(double (&a)[16], double* D, double* col, double* dinv, double* s_p, int tid) {
-  const int r = tid >> 2, g = tid & 3;
-  bool ok = true;
+// ---- rank-8 update shared by POTRF and TRSM -----------------------------------------------------
+// C[r][t0 + j] -= sum_{s<8} C[r][c0 + s] * D[t0 + j][c0 + s]   for the row set of this call, t0 = c0 + 8.
+// Each thread owns a strided 4x4 block: rows r0 + rstep*ii, columns t0 + bj + nblk*jj.
+__device__ __forceinline__ void rank8_block(double* C, int ldc, const double* D, int c0, int r0,
+                                            int rstep, int nr, int bj, int nblk) {
+  const int t0 = c0 + 8;
+  double acc[4][4];
 #pragma unroll
-  for (int c = 0; c < NB; ++c) {
-    const int qc = c >> 2, owner = c & 3;
-    if (r == c && g == owner) *s_p = a[qc];
-    __syncthreads();
-    const double p = *s_p;
-    const bool good = (p > 0.0) && (p < 1.0e300);   // false for NaN, <= 0, inf
-    if (!good) ok = false;
-    const double inv = good ? rsqrt(p) : 1.0;     // 1 / L_cc; one dependent rsqrt per column
-    if (g == owner && r >= c) {
-      const double l = (r == c) ? p * inv : a[qc] * inv;
-      a[qc] = l;
-      col[r] = l;
-      if (r == c) dinv[c] = inv;
-    }
-    __syncthreads();
-    if (r > c) {
-      const double lr = col[r];
+  for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
-      for (int q = 0; q < 16; ++q) {
-        const int cc = 4 * q + g;
-        if (cc > c && cc <= r) a[q] = fma(-lr, col[cc], a[q]);
-      }
-    }
-  }
+    for (int jj = 0; jj < 4; ++jj) acc[ii][jj] = (ii < nr) ? C[(r0 + rstep * ii) * ldc + t0 + bj + nblk * jj] : 0.0;
 #pragma unroll
-  for (int q = 0; q < 16; ++q) D[r * LDS + 4 * q + g] = a[q];
-  __syncthreads();
-  return ok;
-}
-
-struct Smem {
-  double D[NB * LDS];
-  double As[NB * LDK];
-  double Bs[NB * LDK];
-  double y[NB];
-  double col[NB];
-  double dinv[NB];   // 1 / diag(L_kk)
-  double s_p;
-};
-
-// phase A of panel k
-__device__ bool panel_phase(const SolveArgs& a, Smem& sm, int k, int G) {
-  const int tid = threadIdx.x;
-  const size_t ld = (size_t)a.npad;
-  const int nrows = a.nb - k;                 // block rows k .. nb-1 (row 0 = the diagonal block)
-  if ((int)blockIdx.x >= nrows) return true;  // nothing to do for this CTA
-  const int r = tid >> 2, g = tid & 3, lane = tid & 31;
-  const double* Lkk = a.L + (size_t)k * NB * ld + (size_t)k * NB;
-  double d[16];
+  for (int s = 0; s < 8; ++s) {
+    double lr[4], lc[4];
 #pragma unroll
-  for (int q = 0; q < 16; ++q) d[q] = __ldcg(Lkk + r * ld + 4 * q + g);
-  if (tid < NB) sm.y[tid] = __ldcg(a.rhs + k * NB + tid);
-  const bool ok = potrf_block(d, sm.D, sm.col, sm.dinv, &sm.s_p, tid);
-  if (!ok) {
-    if (blockIdx.x == 0 && tid == 0) a.status[0] = 1;
-    return false;
-  }
-  // y_k = D^-1 b_k (warp 0; lane owns rows lane and lane+32)
-  if (tid < 32) {
-    double b0 = sm.y[tid], b1 = sm.y[tid + 32];
-    for (int c = 0; c < NB; ++c) {
-      const double own = (c < 32) ? b0 : b1;
-      const double xc = __shfl_sync(0xffffffffu, own, c & 31) * sm.dinv[c];
-      if (tid == (c & 31)) { if (c < 32) b0 = xc; else b1 = xc; }
-      if (tid > c) b0 -= sm.D[tid * LDS + c] * xc;
-      if (tid + 32 > c) b1 -= sm.D[(tid + 32) * LDS + c] * xc;
-    }
-    sm.y[tid] = b0;
-    sm.y[tid + 32] = b1;
-  }
-  __syncthreads();
-  if (blockIdx.x == 0) {
-    double* Dk = a.Dfac + (size_t)k * NB * NB;
-    for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
-      const int rr = idx / NB, cc = idx % NB;
-      Dk[idx] = (cc <= rr) ? sm.D[rr * LDS + cc] : 0.0;
-    }
-    if (tid < NB) { a.ysol[k * NB + tid] = sm.y[tid]; a.Dinv[k * NB + tid] = sm.dinv[tid]; }
-  }
-  // row blocks: X D^T = A, thread (r, g) keeps columns 4q+g of row r; x_c broadcast by shuffle
-  const int first = (blockIdx.x == 0) ? G : (int)blockIdx.x;   // CTA 0 only helps when G < nrows
-  for (int b = first; b < nrows; b += G) {
-    const int i = k + b;
-    double* Aik = a.L + (size_t)i * NB * ld + (size_t)k * NB;
-    double x[16];
+    for (int ii = 0; ii < 4; ++ii) lr[ii] = (ii < nr) ? C[(r0 + rstep * ii) * ldc + c0 + s] : 0.0;
 #pragma unroll
-    for (int q = 0; q < 16; ++q) x[q] = __ldcg(Aik + r * ld + 4 * q + g);
-    double dot = 0.0;
-#pragma unroll
-    for (int c = 0; c < NB; ++c) {
-      const int q = c >> 2, owner = c & 3;
-      double xc = x[q] * sm.dinv[c];
-      xc = __shfl_sync(0xffffffffu, xc, (lane & ~3) | owner);
-      if (g == owner) { x[q] = xc; dot += xc * sm.y[c]; }
-#pragma unroll
-      for (int qq = 0; qq < 16; ++qq) {
-        const int cc = 4 * qq + g;
-        if (cc > c) x[qq] = fma(-xc, sm.D[cc * LDS + c], x[qq]);
-      }
-    }
-#pragma unroll
-    for (int q = 0; q < 16; ++q) Aik[r * ld + 4 * q + g] = x[q];
-    dot += __shfl_xor_sync(0xffffffffu, dot, 1);
-    dot += __shfl_xor_sync(0xffffffffu, dot, 2);
-    if (g == 0) a.rhs[i * NB + r] -= dot;
-  }
-  return true;
-}
-
-// phase B of panel k: C_ij -= L_ik L_jk^T over the lower tiles of the trailing matrix
-__device__ void update_phase(const SolveArgs& a, Smem& sm, int k, int G) {
-  const int m = a.nb - k - 1;
-  const int ntiles = m * (m + 1) / 2;
-  const int tid = threadIdx.x;
-  const size_t ld = (size_t)a.npad;
-  const int tx = tid & 15, ty = tid >> 4;   // rows ty + 16 ii, cols tx + 16 jj
-  for (int t = blockIdx.x; t < ntiles; t += G) {
-    int ti = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
-    while ((ti + 1) * (ti + 2) / 2 <= t) ++ti;
-    while (ti * (ti + 1) / 2 > t) --ti;
-    const int tj = t - ti * (ti + 1) / 2;
-    const int i = k + 1 + ti, j = k + 1 + tj;
-    const double* Ag = a.L + (size_t)i * NB * ld + (size_t)k * NB;
-    const double* Bg = a.L + (size_t)j * NB * ld + (size_t)k * NB;
-    double acc[4][4];
+    for (int jj = 0; jj < 4; ++jj) lc[jj] = D[(t0 + bj + nblk * jj) * LDD + c0 + s];
 #pragma unroll
     for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
-      for (int jj = 0; jj < 4; ++jj) acc[ii][jj] = 0.0;
-    for (int kc = 0; kc < NB; kc += KC) {
-      __syncthreads();
-      for (int idx = tid; idx < NB * KC; idx += kSolveThreads) {
-        const int rr = idx / KC, cc = idx % KC;
-        sm.As[rr * LDK + cc] = __ldcg(Ag + rr * ld + kc + cc);
-        sm.Bs[rr * LDK + cc] = __ldcg(Bg + rr * ld + kc + cc);
+      for (int jj = 0; jj < 4; ++jj) acc[ii][jj] = fma(-lr[ii], lc[jj], acc[ii][jj]);
+  }
+#pragma unroll
+  for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+    for (int jj = 0; jj < 4; ++jj)
+      if (ii < nr) C[(r0 + rstep * ii) * ldc + t0 + bj + nblk * jj] = acc[ii][jj];
+}
+
+// ---- Cholesky of the 64x64 tile in sm.D (lower triangle; the upper triangle is scratch) ---------
+// Returns false (uniformly) on a pivot that is <= 0 or not finite.
+__device__ bool potrf64(Smem& sm, int tid) {
+  const int lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) sm.flag = 0;
+  for (int pb = 0; pb < 8; ++pb) {
+    const int c0 = 8 * pb;
+    if (warp == 0) {   // micro-panel: rows lane and lane + 32, columns c0 .. c0 + 7, in registers
+      double a0[8], a1[8];
+#pragma unroll
+      for (int t = 0; t < 8; ++t) { a0[t] = sm.D[lane * LDD + c0 + t]; a1[t] = sm.D[(lane + 32) * LDD + c0 + t]; }
+      bool good = true;
+#pragma unroll
+      for (int s = 0; s < 8; ++s) {
+        const int R = c0 + s;
+        const double p = __shfl_sync(0xffffffffu, (R < 32) ? a0[s] : a1[s], R & 31);
+        const bool g = (p > 0.0) && (p < 1.0e300);   // false for NaN, <= 0, inf
+        good = good && g;
+        const double inv = g ? rsqrt(p) : 1.0;
+        a0[s] *= inv;
+        a1[s] *= inv;
+#pragma unroll
+        for (int t = s + 1; t < 8; ++t) {
+          const int Rt = c0 + t;
+          const double lt = __shfl_sync(0xffffffffu, (Rt < 32) ? a0[s] : a1[s], Rt & 31);
+          a0[t] = fma(-a0[s], lt, a0[t]);
+          a1[t] = fma(-a1[s], lt, a1[t]);
+        }
+        if (lane == 0) sm.dinv[R] = inv;
       }
-      __syncthreads();
-#pragma unroll 8
-      for (int kk = 0; kk < KC; ++kk) {
-        double av[4], bv[4];
 #pragma unroll
-        for (int ii = 0; ii < 4; ++ii) av[ii] = sm.As[(ty + 16 * ii) * LDK + kk];
+      for (int t = 0; t < 8; ++t) { sm.D[lane * LDD + c0 + t] = a0[t]; sm.D[(lane + 32) * LDD + c0 + t] = a1[t]; }
+      if (!good && lane == 0) sm.flag = 1;
+    }
+    __syncthreads();
+    const int nblk = (NB - c0 - 8) >> 2;   // 14, 12, ..., 0
+    if (tid < nblk * nblk) {
+      const int bi = tid / nblk, bj = tid - bi * nblk;
+      rank8_block(sm.D, LDD, sm.D, c0, c0 + 8 + bi, nblk, 4, bj, nblk);
+    }
+    __syncthreads();
+  }
+  return sm.flag == 0;
+}
+
+// ---- X L_kk^T = A for the tile in sm.A (stride LDD), rows 0..nrows-1 plus, if with_rhs, row NB -----
+__device__ void trsm64(Smem& sm, int nrows, bool with_rhs, int tid) {
+  const bool row_thread = (tid < nrows) || (with_rhs && tid == NB);
+  for (int pb = 0; pb < 8; ++pb) {
+    const int c0 = 8 * pb;
+    if (row_thread) {
+      double x[8];
 #pragma unroll
-        for (int jj = 0; jj < 4; ++jj) bv[jj] = sm.Bs[(tx + 16 * jj) * LDK + kk];
+      for (int t = 0; t < 8; ++t) x[t] = sm.A[tid * LDD + c0 + t];
 #pragma unroll
-        for (int ii = 0; ii < 4; ++ii)
+      for (int s = 0; s < 8; ++s) {
+        x[s] *= sm.dinv[c0 + s];
 #pragma unroll
-          for (int jj = 0; jj < 4; ++jj) acc[ii][jj] = fma(av[ii], bv[jj], acc[ii][jj]);
+        for (int t = s + 1; t < 8; ++t) x[t] = fma(-x[s], sm.D[(c0 + t) * LDD + c0 + s], x[t]);
       }
+#pragma unroll
+      for (int t = 0; t < 8; ++t) sm.A[tid * LDD + c0 + t] = x[t];
+    }
+    __syncthreads();
+    const int nblk = (NB - c0 - 8) >> 2;
+    if (nblk > 0) {
+      if (nrows > 0 && tid < 16 * nblk) {
+        const int rg = tid / nblk, bj = tid - rg * nblk;
+        rank8_block(sm.A, LDD, sm.D, c0, rg, 16, 4, bj, nblk);
+      } else if (with_rhs && tid >= 224 && tid < 224 + nblk) {
+        rank8_block(sm.A, LDD, sm.D, c0, NB, 0, 1, tid - 224, nblk);
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// ---- phase A of block column k --------------------------------------------------------------------
+__device__ void panel_phase(const SolveArgs& a, Smem& sm, int k, int G) {
+  const int tid = threadIdx.x;
+  const size_t ld = (size_t)a.npad;
+  const int cbeg = a.col_ptr[k], c = a.col_ptr[k + 1] - cbeg;
+  if (blockIdx.x != 0 && (int)blockIdx.x >= c) return;
+  double* Lkk = a.L + (size_t)k * NB * ld + (size_t)k * NB;
+  for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
+    const int r = idx >> 6, cc = idx & 63;
+    sm.D[r * LDD + cc] = __ldcg(Lkk + r * ld + cc);
+  }
+  __syncthreads();
+  if (!potrf64(sm, tid)) {
+    if (blockIdx.x == 0 && tid == 0) a.status[0] = 1;
+    return;
+  }
+  if (blockIdx.x == 0) {   // the factorised diagonal tile goes back in place (strict upper triangle zero)
+    for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
+      const int r = idx >> 6, cc = idx & 63;
+      Lkk[r * ld + cc] = (cc <= r) ? sm.D[r * LDD + cc] : 0.0;
+    }
+    if (tid < NB) a.Dinv[k * NB + tid] = sm.dinv[tid];
+  }
+  bool have_y = false;
+  int t = blockIdx.x;
+  do {
+    const bool has_tile = t < c;
+    double* Aik = nullptr;
+    int i = 0;
+    if (has_tile) {
+      i = a.col_rows[cbeg + t];
+      Aik = a.L + (size_t)i * NB * ld + (size_t)k * NB;
+      for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
+        const int r = idx >> 6, cc = idx & 63;
+        sm.A[r * LDD + cc] = __ldcg(Aik + r * ld + cc);
+      }
+    }
+    if (!have_y && tid < NB) sm.A[NB * LDD + tid] = __ldcg(a.rhs + k * NB + tid);
+    __syncthreads();
+    trsm64(sm, has_tile ? NB : 0, !have_y, tid);
+    if (!have_y) {
+      if (tid < NB) {
+        const double yv = sm.A[NB * LDD + tid];
+        sm.y[tid] = yv;
+        if (blockIdx.x == 0) a.ysol[k * NB + tid] = yv;
+      }
+      have_y = true;
+      __syncthreads();
+    }
+    if (has_tile) {
+      for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
+        const int r = idx >> 6, cc = idx & 63;
+        Aik[r * ld + cc] = sm.A[r * LDD + cc];
+      }
+      // b_i -= L_ik y_k: four threads per row, 16 columns each
+      const int r = tid >> 2, g = tid & 3;
+      double dot = 0.0;
+#pragma unroll
+      for (int cc = 0; cc < 16; ++cc) dot = fma(sm.A[r * LDD + 16 * g + cc], sm.y[16 * g + cc], dot);
+      dot += __shfl_xor_sync(0xffffffffu, dot, 1);
+      dot += __shfl_xor_sync(0xffffffffu, dot, 2);
+      if (g == 0) a.rhs[i * NB + r] = __ldcg(a.rhs + i * NB + r) - dot;
+    }
+    __syncthreads();
+    t += G;
+  } while (t < c);
+}
+
+// ---- phase B of block column k: C_ij -= L_ik L_jk^T on the FP64 tensor pipe --------------------
+__device__ void update_phase(const SolveArgs& a, Smem& sm, int k, int G) {
+  const int cbeg = a.col_ptr[k], c = a.col_ptr[k + 1] - cbeg;
+  const int ntasks = c * (c + 1) / 2;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int gid = lane >> 2, tig = lane & 3;
+  const int wm = warp & 3, wn = warp >> 2;   // rows 16 wm .. +15, columns 32 wn .. +31
+  const size_t ld = (size_t)a.npad;
+  for (int t = blockIdx.x; t < ntasks; t += G) {
+    int ta = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
+    while ((ta + 1) * (ta + 2) / 2 <= t) ++ta;
+    while (ta * (ta + 1) / 2 > t) --ta;
+    const int tb = t - ta * (ta + 1) / 2;
+    const int i = a.col_rows[cbeg + ta], j = a.col_rows[cbeg + tb];
+    const double* Ag = a.L + (size_t)i * NB * ld + (size_t)k * NB;
+    const double* Bg = a.L + (size_t)j * NB * ld + (size_t)k * NB;
+    for (int idx = tid; idx < NB * NB / 2; idx += kSolveThreads) {
+      const int r = idx >> 5, c2 = (idx & 31) * 2;
+      const double2 va = __ldcg(reinterpret_cast<const double2*>(Ag + r * ld + c2));
+      *reinterpret_cast<double2*>(&sm.A[r * LDT + c2]) = va;
+      if (i != j) {
+        const double2 vb = __ldcg(reinterpret_cast<const double2*>(Bg + r * ld + c2));
+        *reinterpret_cast<double2*>(&sm.B[r * LDT + c2]) = vb;
+      }
+    }
+    __syncthreads();
+    const double* Bs = (i != j) ? sm.B : sm.A;
+    double acc[2][4][2];
+#pragma unroll
+    for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+      for (int ni = 0; ni < 4; ++ni) acc[mi][ni][0] = acc[mi][ni][1] = 0.0;
+#pragma unroll 4
+    for (int kk = 0; kk < NB; kk += 4) {
+      double af[2], bf[4];
+#pragma unroll
+      for (int mi = 0; mi < 2; ++mi) af[mi] = sm.A[(16 * wm + 8 * mi + gid) * LDT + kk + tig];
+#pragma unroll
+      for (int ni = 0; ni < 4; ++ni) bf[ni] = Bs[(32 * wn + 8 * ni + gid) * LDT + kk + tig];
+#pragma unroll
+      for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+        for (int ni = 0; ni < 4; ++ni) dmma884(acc[mi][ni][0], acc[mi][ni][1], af[mi], bf[ni]);
     }
     double* Cg = a.L + (size_t)i * NB * ld + (size_t)j * NB;
 #pragma unroll
-    for (int ii = 0; ii < 4; ++ii)
+    for (int mi = 0; mi < 2; ++mi)
 #pragma unroll
-      for (int jj = 0; jj < 4; ++jj) {
-        const int rr = ty + 16 * ii, cc = tx + 16 * jj;
-        if (i != j || cc <= rr) Cg[rr * ld + cc] = __ldcg(Cg + rr * ld + cc) - acc[ii][jj];
+      for (int ni = 0; ni < 4; ++ni) {
+        double2* p = reinterpret_cast<double2*>(Cg + (size_t)(16 * wm + 8 * mi + gid) * ld + 32 * wn + 8 * ni + 2 * tig);
+        double2 v = __ldcg(p);
+        v.x -= acc[mi][ni][0];
+        v.y -= acc[mi][ni][1];
+        *p = v;
       }
+    __syncthreads();
   }
 }
 
 // backward step for block kb: tau_kb = L_kk^-T y_kb (each participating CTA, redundantly), then
-// y_jb -= L[kb, jb]^T tau_kb for the block columns jb < kb this CTA owns; CTA 0 stores tau_kb.
+// y_jb -= L[kb, jb]^T tau_kb for the non-zero tiles of row kb this CTA owns; CTA 0 stores tau_kb.
 __device__ void back_phase(const SolveArgs& a, Smem& sm, int kb, int G) {
   const int tid = threadIdx.x;
-  if ((int)blockIdx.x > kb) return;
+  const int rbeg = a.row_ptr[kb], rc = a.row_ptr[kb + 1] - rbeg;
+  if (blockIdx.x != 0 && (int)blockIdx.x >= rc) return;
   const size_t ld = (size_t)a.npad;
-  const double* Dk = a.Dfac + (size_t)kb * NB * NB;
+  const double* Lkk = a.L + (size_t)kb * NB * ld + (size_t)kb * NB;
   for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
-    const int rr = idx / NB, cc = idx % NB;
-    sm.D[rr * LDS + cc] = __ldcg(Dk + idx);
+    const int r = idx >> 6, cc = idx & 63;
+    sm.D[r * LDD + cc] = __ldcg(Lkk + r * ld + cc);
   }
   if (tid < NB) { sm.y[tid] = __ldcg(a.ysol + kb * NB + tid); sm.dinv[tid] = __ldcg(a.Dinv + kb * NB + tid); }
   __syncthreads();
@@ -318,29 +338,37 @@ __device__ void back_phase(const SolveArgs& a, Smem& sm, int kb, int G) {
       const double own = (c < 32) ? b0 : b1;
       const double xc = __shfl_sync(0xffffffffu, own, c & 31) * sm.dinv[c];
       if (tid == (c & 31)) { if (c < 32) b0 = xc; else b1 = xc; }
-      if (tid < c) b0 -= sm.D[c * LDS + tid] * xc;
-      if (tid + 32 < c) b1 -= sm.D[c * LDS + tid + 32] * xc;
+      if (tid < c) b0 -= sm.D[c * LDD + tid] * xc;
+      if (tid + 32 < c) b1 -= sm.D[c * LDD + tid + 32] * xc;
     }
     sm.y[tid] = b0;
     sm.y[tid + 32] = b1;
   }
   __syncthreads();
   if (blockIdx.x == 0 && tid < NB) a.tau[kb * NB + tid] = sm.y[tid];
-  // 256 threads: column c = tid & 63, quarter of the rows each; reduce the 4 partial sums in smem
+  // 256 threads: column c = tid & 63, a quarter of the rows each; the 4 partial sums meet in shared memory
   const int c = tid & 63, part = tid >> 6;
-  for (int jb = blockIdx.x; jb < kb; jb += G) {
+  for (int t = blockIdx.x; t < rc; t += G) {
+    const int jb = a.row_cols[rbeg + t];
     const double* Lkj = a.L + (size_t)kb * NB * ld + (size_t)jb * NB;
     double acc = 0.0;
 #pragma unroll 4
     for (int rr = part * 16; rr < part * 16 + 16; ++rr) acc = fma(__ldcg(Lkj + rr * ld + c), sm.y[rr], acc);
     __syncthreads();
-    sm.As[part * 64 + c] = acc;
+    sm.red[part * 64 + c] = acc;
     __syncthreads();
-    if (tid < NB) a.ysol[jb * NB + tid] -= (sm.As[tid] + sm.As[64 + tid]) + (sm.As[128 + tid] + sm.As[192 + tid]);
+    if (tid < NB)
+      a.ysol[jb * NB + tid] = __ldcg(a.ysol + jb * NB + tid) - ((sm.red[tid] + sm.red[64 + tid]) + (sm.red[128 + tid] + sm.red[192 + tid]));
   }
 }
 
 __global__ void __launch_bounds__(kSolveThreads)
+k_assemble_tiles(AsmArgs a, const int32_t* __restrict__ tiles, double eps, int32_t* __restrict__ status) {
+  assemble_tile(a, tiles[2 * blockIdx.x], tiles[2 * blockIdx.x + 1], eps, threadIdx.x);
+  if (blockIdx.x == 0 && threadIdx.x == 0) status[0] = 0;
+}
+
+__global__ void __launch_bounds__(kSolveThreads, 2)
 k_solve(SolveArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
@@ -350,28 +378,25 @@ k_solve(SolveArgs a) {
   double eps = a.eps0;
   int r = 0;
   for (; r < a.max_attempts; ++r, eps *= 100.0) {
-    // ---- phase 0: damped assembly, rhs = -g ----
-    if (a.dense) {
-      assemble_dense(a, G, eps);
-    } else {
-      assemble_zero(a, G);
+    if (r > 0) {   // retry: damped re-assembly of the non-zero tiles (the first attempt was assembled by k_assemble_tiles)
+      for (int t = blockIdx.x; t < a.n_tiles; t += G) assemble_tile(a.as, a.tiles[2 * t], a.tiles[2 * t + 1], eps, threadIdx.x);
+      if (blockIdx.x == 0 && threadIdx.x == 0) a.status[0] = 0;
       grid_barrier(a.bar, G, gen);
-      assemble_blocks(a, G, eps);
     }
-    for (int idx = blockIdx.x * kSolveThreads + threadIdx.x; idx < a.npad; idx += G * kSolveThreads)
-      a.rhs[idx] = idx < a.n ? -a.g[idx] : 0.0;
-    if (blockIdx.x == 0 && threadIdx.x == 0) a.status[0] = 0;
-    grid_barrier(a.bar, G, gen);
     // ---- factorisation with the forward solve riding along ----
     bool failed = false;
     for (int k = 0; k < a.nb; ++k) {
       panel_phase(a, sm, k, G);
-      grid_barrier(a.bar, G, gen);
-      if (*reinterpret_cast<volatile int32_t*>(a.status) != 0) { failed = true; break; }
-      if (k + 1 < a.nb) {
+      if (a.col_ptr[k + 1] > a.col_ptr[k]) {
+        grid_barrier(a.bar, G, gen);
+        if (ld_flag(a.status) != 0) { failed = true; break; }
         update_phase(a, sm, k, G);
         grid_barrier(a.bar, G, gen);
       }
+    }
+    if (!failed) {   // block columns without sub-diagonal tiles are factorised by CTA 0 alone
+      grid_barrier(a.bar, G, gen);
+      failed = ld_flag(a.status) != 0;
     }
     if (failed) {
       grid_barrier(a.bar, G, gen);   // everybody has seen the flag before it is cleared again
@@ -380,7 +405,7 @@ k_solve(SolveArgs a) {
     // ---- backward substitution ----
     for (int kb = a.nb - 1; kb >= 0; --kb) {
       back_phase(a, sm, kb, G);
-      if (kb > 0) grid_barrier(a.bar, G, gen);
+      if (a.row_ptr[kb + 1] > a.row_ptr[kb]) grid_barrier(a.bar, G, gen);
     }
     solved = true;
     break;
@@ -411,23 +436,36 @@ cudaError_t launch_solve(Ctx* c) {
     if (e != cudaSuccess) return e;
     if (max_blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
   }
-  const int nb = c->npad / NB;
-  // enough CTAs for the widest phase, never more than can be co-resident
-  long long want = std::max<long long>({(long long)nb * (nb - 1) / 2, (long long)nb, (long long)(c->N + c->n_pairs + 3) / 4, 1LL});
+  const bool dense = c->dense_loaded || c->solver_mode == 1;
+  SolvePlan& plan = dense ? c->plan_dense : c->plan_sparse;
+  if (!plan.ready) {
+    std::string err;
+    if (!build_plan(c, dense, plan, err)) { c->err = err; return cudaErrorUnknown; }
+  }
+  long long want = std::max<long long>({(long long)plan.max_upd, (long long)plan.max_col, (long long)plan.max_row, 1LL});
   const int G = (int)std::min<long long>(want, (long long)num_sms * std::min(max_blocks_per_sm, 2));
   SolveArgs a;
-  a.L = c->L; a.npad = c->npad; a.n = c->n; a.nb = nb;
-  a.blocks35 = c->blocks35; a.kf_ptr = c->kf_ptr; a.kf_edge = c->kf_edge; a.pair_kf = c->pair_kf;
-  a.pair_ptr = c->pair_ptr; a.pair_edge = c->pair_edge; a.fixed = c->fixed_mask; a.N = c->N; a.n_pairs = c->n_pairs;
-  a.dense = c->dense_loaded ? c->Hd : nullptr;
-  a.g = c->g; a.rhs = c->rhs; a.ysol = c->ysol; a.Dfac = c->Dfac; a.Dinv = c->Dinv; a.tau = c->tau;
-  a.lambda = c->prm.lm_lambda; a.eps0 = c->prm.eps0; a.max_attempts = c->prm.max_attempts;
+  AsmArgs& s = a.as;
+  s.L = c->L; s.npad = c->npad; s.n = c->n; s.N = c->N; s.blocks35 = c->blocks35;
+  s.kf_ptr = c->kf_ptr; s.kf_edge = c->kf_edge; s.pair_kf = c->pair_kf; s.pairhi_ptr = c->pairhi_ptr;
+  s.pair_ptr = c->pair_ptr; s.pair_edge = c->pair_edge; s.fixed = c->fixed_mask;
+  s.dense = c->dense_loaded ? c->Hd : nullptr; s.g = c->g; s.rhs = c->rhs; s.lambda = c->prm.lm_lambda;
+  a.L = c->L; a.npad = c->npad; a.n = c->n; a.nb = plan.nb;
+  a.col_ptr = plan.col_ptr; a.col_rows = plan.col_rows; a.row_ptr = plan.row_ptr; a.row_cols = plan.row_cols;
+  a.tiles = plan.tiles; a.n_tiles = plan.n_tiles;
+  a.rhs = c->rhs; a.ysol = c->ysol; a.Dinv = c->Dinv; a.tau = c->tau;
+  a.eps0 = c->prm.eps0; a.max_attempts = c->prm.max_attempts;
   a.status = c->fail_flag; a.eps_used = c->d_eps_used; a.bar = c->bar;
   cudaError_t e = cudaMemsetAsync(c->bar, 0, sizeof(unsigned int), c->stream);
   if (e != cudaSuccess) return e;
+  k_assemble_tiles<<<plan.n_tiles, kSolveThreads, 0, c->stream>>>(s, plan.tiles, c->prm.eps0, c->fail_flag);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  if (c->profiling) cudaEventRecord(c->ev[4], c->stream);
   void* args[] = {&a};
   e = cudaLaunchCooperativeKernel((const void*)k_solve, dim3(G), dim3(kSolveThreads), args, smem, c->stream);
-  ++c->launches;
+  c->launches += 2;
+  c->last_solve_grid = G;
   return e;
 }
 

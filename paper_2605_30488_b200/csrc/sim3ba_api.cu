@@ -67,12 +67,15 @@ void build_bookkeeping(Ctx* c) {
   }
   c->n_pairs = (int)pairs.size();
   c->h_pair_kf.clear(); c->h_pair_ptr.assign(1, 0); c->h_pair_edge.clear();
+  c->h_pairhi_ptr.assign(N + 1, 0);
   for (const auto& kv : pairs) {
     c->h_pair_kf.push_back(kv.first.first);
     c->h_pair_kf.push_back(kv.first.second);
+    ++c->h_pairhi_ptr[kv.first.first + 1];
     for (int32_t e : kv.second) c->h_pair_edge.push_back(e);
     c->h_pair_ptr.push_back((int32_t)c->h_pair_edge.size());
   }
+  for (int k = 0; k < N; ++k) c->h_pairhi_ptr[k + 1] += c->h_pairhi_ptr[k];
 }
 
 template <class T>
@@ -86,7 +89,8 @@ void free_all(Ctx* c) {
   cudaFree(c->pm); cudaFree(c->edges); cudaFree(c->grp_kf); cudaFree(c->grp_ptr); cudaFree(c->grp_edge); cudaFree(c->edgeT); cudaFree(c->fixed_mask); cudaFree(c->poses);
   cudaFree(c->kf_ptr); cudaFree(c->kf_edge); cudaFree(c->pair_kf); cudaFree(c->pair_ptr); cudaFree(c->pair_edge);
   cudaFree(c->partials); cudaFree(c->blocks35); cudaFree(c->edge_cost); cudaFree(c->n_valid); cudaFree(c->checksum);
-  cudaFree(c->Hd); cudaFree(c->L); cudaFree(c->g); cudaFree(c->rhs); cudaFree(c->ysol); cudaFree(c->Dfac); cudaFree(c->Dinv);
+  cudaFree(c->Hd); cudaFree(c->L); cudaFree(c->g); cudaFree(c->rhs); cudaFree(c->ysol); cudaFree(c->Dinv); cudaFree(c->pairhi_ptr);
+  free_plan(c->plan_sparse); free_plan(c->plan_dense);
   cudaFree(c->tau); cudaFree(c->total_cost); cudaFree(c->fail_flag); cudaFree(c->d_eps_used); cudaFree(c->bar);
   if (c->h_flag) cudaFreeHost(c->h_flag);
   if (c->h_scalar) cudaFreeHost(c->h_scalar);
@@ -221,6 +225,7 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
   CUB(upload(&c->pair_kf, c->h_pair_kf, c->stream));
   CUB(upload(&c->pair_ptr, c->h_pair_ptr, c->stream));
   CUB(upload(&c->pair_edge, c->h_pair_edge, c->stream));
+  CUB(upload(&c->pairhi_ptr, c->h_pairhi_ptr, c->stream));
   CUB(dev_alloc(&c->poses, (size_t)8 * c->N));
   CUB(dev_alloc(&c->partials, (size_t)c->E * c->chunks * kPartialStride));
   CUB(dev_alloc(&c->blocks35, (size_t)c->E * 35));
@@ -232,7 +237,6 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
   CUB(dev_alloc(&c->g, (size_t)c->npad));
   CUB(dev_alloc(&c->rhs, (size_t)c->npad));
   CUB(dev_alloc(&c->ysol, (size_t)c->npad));
-  CUB(dev_alloc(&c->Dfac, (size_t)(c->npad / kNB) * kNB * kNB));
   CUB(dev_alloc(&c->tau, (size_t)c->npad));
   CUB(dev_alloc(&c->Dinv, (size_t)c->npad));
   CUB(dev_alloc(&c->total_cost, 1));
@@ -253,6 +257,10 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
     CUB(cudaStreamSynchronize(c->stream));
   }
   c->match = d_match;
+  {
+    std::string perr;
+    if (!build_plan(c, false, c->plan_sparse, perr)) return bail(SIM3BA_ERR_CUDA, perr);
+  }
   CUB(launch_pack(c, d_points, d_conf));
   CUB(cudaStreamSynchronize(c->stream));
 #undef CUB
@@ -343,9 +351,9 @@ int sim3ba_step(sim3ba_ctx* h) {
     CU(cudaStreamSynchronize(c->stream));
     cudaEventElapsedTime(&c->phase_ms[0], c->ev[0], c->ev[1]);
     cudaEventElapsedTime(&c->phase_ms[1], c->ev[1], c->ev[2]);
-    cudaEventElapsedTime(&c->phase_ms[3], c->ev[3], c->ev[5]);
+    cudaEventElapsedTime(&c->phase_ms[2], c->ev[3], c->ev[4]);   // damped tile assembly
+    cudaEventElapsedTime(&c->phase_ms[3], c->ev[4], c->ev[5]);   // persistent factor + solves
     cudaEventElapsedTime(&c->phase_ms[4], c->ev[6], c->ev[7]);
-    c->phase_ms[2] = 0.f;   // the damped assembly runs inside the persistent solve kernel
   }
   c->built = false; c->solved = false;
   return SIM3BA_OK;
@@ -427,6 +435,31 @@ int sim3ba_load_system(sim3ba_ctx* h, const double* d_H, const double* d_g) {
   CU(cudaMemcpyAsync(c->Hd, d_H, (size_t)c->n * c->n * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
   CU(launch_load_gradient(c, d_g));
   c->dense_loaded = true; c->hd_valid = false; c->built = false; c->solved = false;
+  return SIM3BA_OK;
+}
+
+int sim3ba_set_solver_mode(sim3ba_ctx* h, int32_t mode) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (mode != 0 && mode != 1) return fail(c, SIM3BA_ERR_INVALID_ARG, "solver mode must be 0 (tile-sparse) or 1 (dense)");
+  c->solver_mode = mode;
+  return SIM3BA_OK;
+}
+
+int sim3ba_get_solver_info(sim3ba_ctx* h, int32_t* n_tiles, int32_t* n_tiles_dense, double* flops, int32_t* grid) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  const bool dense = c->solver_mode == 1;
+  SolvePlan& plan = dense ? c->plan_dense : c->plan_sparse;
+  if (!plan.ready) {
+    std::string err;
+    if (!build_plan(c, dense, plan, err)) return fail(c, SIM3BA_ERR_CUDA, err);
+  }
+  const int nb = c->npad / kNB;
+  if (n_tiles) *n_tiles = plan.n_tiles;
+  if (n_tiles_dense) *n_tiles_dense = nb * (nb + 1) / 2;
+  if (flops) *flops = plan.flops;
+  if (grid) *grid = c->last_solve_grid;
   return SIM3BA_OK;
 }
 

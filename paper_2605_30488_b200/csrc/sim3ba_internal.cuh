@@ -27,6 +27,18 @@ struct DevParams {       // robust-kernel constants, fp32, passed by value to ke
   float huber_k2;
 };
 
+// Tile-level plan of the Cholesky factorisation (a7), built once per graph on the host (a0): the
+// non-zero 64x64 tiles of L (symbolic factorisation of the keyframe graph, fill included) as
+// column lists (rows i > k with a non-zero tile (i, k)) and row lists (columns j < k), plus the list
+// of all non-zero tiles for the assembly.  The "dense" plan lists every lower tile.
+struct SolvePlan {
+  int nb = 0, n_tiles = 0, n_off = 0, max_col = 0, max_row = 0, max_upd = 0, grid = 1;
+  double flops = 0.0;                                   // tile-level flop count of factor + solves
+  int32_t *col_ptr = nullptr, *col_rows = nullptr, *row_ptr = nullptr, *row_cols = nullptr, *tiles = nullptr;
+  std::vector<int32_t> h_col_ptr, h_col_rows, h_row_ptr, h_row_cols, h_tiles;
+  bool ready = false;
+};
+
 struct Ctx {
   int N = 0, H = 0, W = 0, HW = 0, E = 0, n = 0, npad = 0, chunks = 0, n_pairs = 0;
   cudaStream_t stream = nullptr;
@@ -43,7 +55,10 @@ struct Ctx {
   double* poses = nullptr;         // [N][8]
   // bookkeeping (device + host)
   int32_t *kf_ptr = nullptr, *kf_edge = nullptr, *pair_kf = nullptr, *pair_ptr = nullptr, *pair_edge = nullptr;
-  std::vector<int32_t> h_edges, h_kf_ptr, h_kf_edge, h_pair_kf, h_pair_ptr, h_pair_edge;
+  int32_t* pairhi_ptr = nullptr;   // [N+1] first pair whose larger keyframe is >= k (pairs are sorted by (hi, lo))
+  std::vector<int32_t> h_edges, h_kf_ptr, h_kf_edge, h_pair_kf, h_pair_ptr, h_pair_edge, h_pairhi_ptr;
+  SolvePlan plan_sparse, plan_dense;
+  int solver_mode = 0;             // 0: tile-sparse plan of the graph, 1: dense plan (every lower tile)
   std::vector<uint8_t> h_fixed;
   // per-edge results
   double* partials = nullptr;      // [E][chunks][kPartialStride]
@@ -57,7 +72,6 @@ struct Ctx {
   double* g = nullptr;             // [npad]
   double* rhs = nullptr;           // [npad] working right-hand side b (starts as -g)
   double* ysol = nullptr;          // [npad] y = L^-1 b, then consumed by the backward solve
-  double* Dfac = nullptr;          // [npad/kNB][kNB*kNB] factorised diagonal blocks
   double* Dinv = nullptr;          // [npad] reciprocals of the diagonal of L
   double* tau = nullptr;           // [npad]
   double* total_cost = nullptr;    // [1]
@@ -70,6 +84,7 @@ struct Ctx {
   int attempts = 0;
   double eps_used = 0.0;
   int64_t launches = 0;
+  int last_solve_grid = 0;
   bool profiling = false;
   cudaEvent_t ev[8] = {};
   float phase_ms[8] = {};
@@ -82,7 +97,9 @@ cudaError_t launch_accumulate(Ctx* c);                   // kernels 1+2: partial
 cudaError_t launch_assemble(Ctx* c, double* dst, double lambda, double eps, bool from_dense);  // kernel 3
 cudaError_t launch_gradient(Ctx* c);                     // g from the per-edge b_e
 cudaError_t launch_load_gradient(Ctx* c, const double* d_g);
-cudaError_t launch_solve(Ctx* c);                        // kernels 3+4 (persistent): damped assembly, Cholesky, solves, eps retry
+cudaError_t launch_solve(Ctx* c);                        // kernels 3+4: tile assembly (damped), then the persistent Cholesky / solves / eps retry
+bool build_plan(Ctx* c, bool dense, SolvePlan& plan, std::string& err);   // host symbolic factorisation + upload
+void free_plan(SolvePlan& plan);
 cudaError_t launch_retract(Ctx* c);                      // kernel 5
 
 }  // namespace sim3ba
