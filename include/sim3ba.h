@@ -66,7 +66,7 @@ int sim3ba_default_params(sim3ba_params* p);
  * Ownership: the library copies points+conf into an internal packed float4 array and copies the
  * edge list; d_match is BORROWED and must stay valid and unchanged until sim3ba_destroy.
  * Poses start as identity; call sim3ba_set_poses.  Errors: i == j or endpoint outside [0,N),
- * fixed keyframe outside [0,N), non-positive sizes or sigmas -> SIM3BA_ERR_INVALID_ARG.
+ * fixed keyframe outside [0,N), non-positive sizes or sigmas, height*width > 2^28 -> SIM3BA_ERR_INVALID_ARG.
  * Synchronises the stream. */
 int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width, int32_t n_edges,
                   const float* d_points, const float* d_conf, const int32_t* d_edges,

@@ -149,7 +149,7 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
   Ctx* c = nullptr;
   if (!out) return fail(c, SIM3BA_ERR_INVALID_ARG, "out is NULL");
   *out = nullptr;
-  if (n_kf <= 0 || height <= 0 || width <= 0 || n_edges < 0 || n_fixed < 0 || (int64_t)height * width > (1 << 30) ||
+  if (n_kf <= 0 || height <= 0 || width <= 0 || n_edges < 0 || n_fixed < 0 || (int64_t)height * width > (1 << 28) ||
       (int64_t)n_kf * 7 > (1 << 20))
     return fail(c, SIM3BA_ERR_INVALID_ARG, "non-positive or oversized dimensions");
   if (!d_points || !d_conf || (n_edges > 0 && (!d_edges || !d_match)) || (n_fixed > 0 && !h_fixed_kf))

@@ -11,8 +11,8 @@
 
 namespace sim3ba {
 
-constexpr int kTilePx = 4096;        // pixels of one edge handled by one accumulate CTA
-constexpr int kAccThreads = 256;
+constexpr int kTilePx = 3072;        // pixels of one edge handled by one accumulate CTA
+constexpr int kAccThreads = 192;
 // doubles per (edge, tile) partial record: [0..27] upper triangle of M = sum J_xi^T Omega J_xi (row-major,
 // r <= c; (3,6), (4,6), (5,6) are structurally zero), [28..34] c = sum J_xi^T Omega e, [35] sum w r^2,
 // [36] sum min(r^2, kappa^2) (robust cost = [35] - [36]/2), [37] n_valid (int64 bits), [38] checksum (uint64 bits)
@@ -23,7 +23,8 @@ constexpr int kNB = 64;              // Cholesky block size
 struct DevParams {       // robust-kernel constants, fp32, passed by value to kernel 1
   float inv_var_ray;     // 1 / sigma_r^2
   float inv_var_dist;    // 1 / sigma_d^2
-  float huber_k;
+  float k_over_sigma_ray;   // kappa / sigma_r
+  float k_over_sigma_dist;  // kappa / sigma_d
   float huber_k2;
 };
 
@@ -44,7 +45,7 @@ struct Ctx {
   cudaStream_t stream = nullptr;
   sim3ba_params prm{};
   // inputs
-  float4* pm = nullptr;            // [N][HW] packed (x, y, z, conf)
+  float4* pm = nullptr;            // [N][HW] packed (x, y, z, w): w = c^(1/4) if c > conf_min else -1
   const int32_t* match = nullptr;  // borrowed [E][HW]
   int32_t* edges = nullptr;        // [E][2]
   // kernel-1 schedule: keyframes with outgoing edges (ascending) and their edges (ascending j, then e)
