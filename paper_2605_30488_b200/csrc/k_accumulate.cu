@@ -29,18 +29,20 @@ namespace {
 static_assert(kTilePx == 16 * kAccThreads, "precision plan: <= 16 fp32 terms per thread partial (8 per lane)");
 constexpr int kPairs = kTilePx / (2 * kAccThreads);   // match pairs per thread and edge
 constexpr int kWarps = kAccThreads / 32;
+constexpr int kWarpPx = kTilePx / kWarps;      // contiguous pixels owned by one warp (64 per pair: A = 64 p + lane, B = A + 32)
+constexpr int kStages = 4;                     // ring of gathered X_j pairs per warp: gathers run kStages - 1 pairs ahead
 constexpr int kSlots = kPartialStride;         // 40 reduction slots (layout: sim3ba_internal.cuh)
 constexpr int kAccSlots = 37;                  // slots that carry floating-point sums
 
-// shared-memory carve-up of k_accumulate (dynamic)
-constexpr size_t kOffXi = 0;                                      // float4 [kTilePx], re-laid as lane pairs
-constexpr size_t kOffDer = kOffXi + sizeof(float4) * kTilePx;     // float4 [kTilePx / 2] (1/|X_A|, 1/|X_B|, |X_A|, |X_B|)
-constexpr size_t kOffRed = kOffDer + sizeof(float4) * (kTilePx / 2);   // double [kWarps][kSlots]
-constexpr size_t kOffT = kOffRed + sizeof(double) * kWarps * kSlots;   // double [12]
-constexpr size_t kOffCnt = kOffT + sizeof(double) * 12;           // unsigned [kWarps] (8 B stride)
-constexpr size_t kOffChk = kOffCnt + sizeof(long long) * kWarps;  // unsigned long long [kWarps]
-constexpr size_t kOffBar = kOffChk + sizeof(long long) * kWarps;  // mbarrier
-constexpr size_t kAccSmem = kOffBar + 16;
+// shared-memory carve-up of k_accumulate (dynamic); every array is sliced per warp
+constexpr size_t kOffXi = 0;                                            // float4 [kWarps][kWarpPx], re-laid as lane pairs
+constexpr size_t kOffRdi = kOffXi + sizeof(float4) * kTilePx;           // float2 [kWarps][kWarpPx / 2] (1/|X_A|, 1/|X_B|)
+constexpr size_t kOffIdx = kOffRdi + sizeof(float2) * (kTilePx / 2);    // int32 [kWarps][2][kWarpPx]
+constexpr size_t kOffRing = kOffIdx + sizeof(int32_t) * 2 * kTilePx;    // float4 [kWarps][kStages][64]: gathered X_j in flight
+constexpr size_t kOffBar = kOffRing + sizeof(float4) * kWarps * kStages * 64;          // mbarrier [kWarps][3]
+constexpr size_t kAccSmem = kOffBar + sizeof(uint64_t) * 3 * kWarps;
+constexpr int kAccCtasPerSm = 12 / kWarps;     // 12 warps per SM: bounded by registers (<= 168) and shared memory (18 KB per warp)
+static_assert(kAccCtasPerSm * (kAccSmem + 1024) <= 227 * 1024, "kAccCtasPerSm CTAs per SM");
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -67,6 +69,14 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_
                : "memory");
 }
 
+// per-thread 16-byte asynchronous gather global -> shared (LDGSTS, L2 only): nothing is held in registers while in flight
+__device__ __forceinline__ void cp_async16(void* dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 // MUFU.RSQ / MUFU.RCP without the denormal pre/post-scaling of rsqrtf() / 1/x: arguments are clamped or
 // may legitimately give +inf (handled by the min() that follows)
 __device__ __forceinline__ float rsq(float v) {
@@ -92,11 +102,12 @@ __device__ __forceinline__ f2 bc(float s) { return make_float2(s, s); }
 
 // Two valid-or-masked matches: accumulate J_xi^T Omega J_xi (25 structurally non-zero upper-triangular
 // entries), J_xi^T Omega e (7) and the two robust-cost sums into acc[] (slot layout: sim3ba_internal.cuh).
-//   del = T_ij X_j - X_i (fp32 rounding of the FP64 value), Xi, rdi = 1/|X_i|, di = |X_i|,
+//   del = T_ij X_j - X_i (fp32 rounding of the FP64 value), Xi, rdi = 1/|X_i|,
 //   sq = sqrt(q) = (c_i c_j)^(1/4), 0 for a masked lane (all its weights vanish).
 __device__ __forceinline__ void accumulate_pair(f2 (&acc)[kAccSlots], const f2 del0, const f2 del1, const f2 del2,
-                                                const f2 Xi0, const f2 Xi1, const f2 Xi2, const f2 rdi, const f2 di,
+                                                const f2 Xi0, const f2 Xi1, const f2 Xi2, const f2 rdi,
                                                 const f2 sq, const DevParams& prm) {
+  const f2 di = fma2(Xi0, Xi0, fma2(Xi1, Xi1, Xi2 * Xi2)) * rdi;   // |X_i| (rdi is clamped: 0 for X_i = 0)
   const f2 x0 = Xi0 + del0, x1 = Xi1 + del1, x2 = Xi2 + del2;   // x = T_ij X_j
   f2 d2 = fma2(x0, x0, fma2(x1, x1, x2 * x2));
   d2.x = fmaxf(d2.x, 1e-20f); d2.y = fmaxf(d2.y, 1e-20f);
@@ -173,8 +184,11 @@ __device__ __forceinline__ void accumulate_pair(f2 (&acc)[kAccSlots], const f2 d
 // level a lane keeps one half of its slots and hands the other half to its partner, so the whole tree
 // costs 20 + 10 + 5 + 5 + 5 exchanges instead of 40 x 5.  Level 1 exchanges the fp32 partials and
 // converts both operands (the sums are FP64 from here on).  Lanes with (lane & 3) == 0 end up holding
-// the warp totals of slots base .. base + 4, base = 20 b4 + 10 b3 + 5 b2 (bits of the lane index).
-__device__ __forceinline__ void warp_reduce_slots(const float (&acc)[kSlots], double* __restrict__ s_red_warp, const int lane) {
+// the warp totals of slots base .. base + 4, base = 20 b4 + 10 b3 + 5 b2 (bits of the lane index), and
+// write them to the warp's record; the lane holding slots 35..39 stores the two integers (warp totals,
+// every lane has them) in slots 37 and 38.
+__device__ __forceinline__ void warp_reduce_slots(const float (&acc)[kSlots], double* __restrict__ out, const int lane,
+                                                  unsigned long long cnt, unsigned long long chk) {
   double v[20];
   {
     const bool up = lane & 16;
@@ -210,83 +224,124 @@ __device__ __forceinline__ void warp_reduce_slots(const float (&acc)[kSlots], do
   }
   if ((lane & 3) == 0) {
     const int base = ((lane >> 4) & 1) * 20 + ((lane >> 3) & 1) * 10 + ((lane >> 2) & 1) * 5;
+    if (base == 35) {
+      out[35] = v[0];
+      out[36] = v[1];
+      reinterpret_cast<unsigned long long*>(out)[kSlotCnt] = cnt;
+      reinterpret_cast<unsigned long long*>(out)[kSlotChk] = chk;
+    } else {
 #pragma unroll
-    for (int k = 0; k < 5; ++k) s_red_warp[base + k] = v[k];
+      for (int k = 0; k < 5; ++k) out[base + k] = v[k];
+    }
   }
 }
 
-__global__ void __launch_bounds__(kAccThreads, 2)
+// One warp = one independent worker: it owns kWarpPx contiguous pixels of the tile (its slice of X_i and of every
+// edge's match indices arrive by its own TMA bulk copies on its own mbarriers) and walks the edges leaving i without
+// any CTA-wide barrier, and writes one 40-double record per (edge, slice); k_finalize sums the records in slice order.
+// X_j is gathered by per-lane cp.async into a per-warp shared-memory ring, kStages - 1 pairs ahead of the arithmetic.
+__global__ void __launch_bounds__(kAccThreads, kAccCtasPerSm)
 k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, const int32_t* __restrict__ edges,
              const int32_t* __restrict__ grp_kf, const int32_t* __restrict__ grp_ptr, const int32_t* __restrict__ grp_edge,
-             const double* __restrict__ edgeT, double* __restrict__ partials, int HW, int tiles, DevParams prm) {
+             const double* __restrict__ edgeT, double* __restrict__ partials, int HW, int tiles, int idx_tma, DevParams prm) {
   extern __shared__ __align__(128) unsigned char smem[];
-  float4* s_Xi = reinterpret_cast<float4*>(smem + kOffXi);
-  float4* s_der = reinterpret_cast<float4*>(smem + kOffDer);
-  double* s_red = reinterpret_cast<double*>(smem + kOffRed);
-  double* s_T = reinterpret_cast<double*>(smem + kOffT);
-  unsigned int* s_cnt = reinterpret_cast<unsigned int*>(smem + kOffCnt);
-  unsigned long long* s_chk = reinterpret_cast<unsigned long long*>(smem + kOffChk);
-  uint64_t* s_bar = reinterpret_cast<uint64_t*>(smem + kOffBar);
-
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  float4* s_Xi = reinterpret_cast<float4*>(smem + kOffXi) + warp * kWarpPx;          // this warp's slice, re-laid as lane pairs
+  float2* s_rdi = reinterpret_cast<float2*>(smem + kOffRdi) + warp * (kWarpPx / 2);
+  float4* s_ring = reinterpret_cast<float4*>(smem + kOffRing) + warp * (kStages * 64);   // [kStages][64], slot = pair % kStages
+  int32_t* s_idx = reinterpret_cast<int32_t*>(smem + kOffIdx) + warp * (2 * kWarpPx);  // [2][kWarpPx], double-buffered over edges
+  uint64_t* s_bar = reinterpret_cast<uint64_t*>(smem + kOffBar) + warp * 3;           // [0] X_i slice, [1], [2] index buffers
+
   const int g = blockIdx.x / tiles, tile = blockIdx.x - g * tiles;
   const int i = grp_kf[g];
-  const int px0 = tile * kTilePx;
-  const int npx = min(kTilePx, HW - px0);
+  const int px0 = tile * kTilePx + warp * kWarpPx;                   // first pixel of this warp's slice
+  const int npx = max(0, min(kWarpPx, HW - px0));                    // pixels of the slice inside the keyframe
+  const int e_beg = grp_ptr[g], n_e = grp_ptr[g + 1] - e_beg;
 
-  // ---- stage the tile of X_i: one TMA bulk copy per 16 KB, completion on the mbarrier ----
-  if (tid == 0) mbar_init(s_bar, 1);
-  __syncthreads();
-  if (tid == 0) {
-    const uint32_t bytes = (uint32_t)npx * (uint32_t)sizeof(float4);
-    mbar_expect_tx(s_bar, bytes);
-    const unsigned char* src = reinterpret_cast<const unsigned char*>(pm + (size_t)i * HW + px0);
-    for (uint32_t off = 0; off < bytes; off += 16384u)
-      tma_bulk_g2s(smem + kOffXi + off, src + off, min(16384u, bytes - off), s_bar);
+  if (lane == 0) { mbar_init(s_bar, 1); mbar_init(s_bar + 1, 1); mbar_init(s_bar + 2, 1); }
+  // pixels past the ragged end are never written by the copies: masked once (w = -1, index -1)
+  for (int p = npx + lane; p < kWarpPx; p += 32) {
+    s_Xi[p] = make_float4(0.f, 0.f, 0.f, -1.f);
+    s_idx[p] = -1;
+    s_idx[kWarpPx + p] = -1;
   }
-  mbar_wait(s_bar, 0);
-  // Pair p of this thread = pixels A = 2p T + tid and B = (2p + 1) T + tid (T = kAccThreads).  Re-lay the two
-  // staged float4 in place as lane pairs, (xA, xB, yA, yB) in A's slot and (zA, zB, wA, wB) in B's, and keep
-  // (1/|X_A|, 1/|X_B|, |X_A|, |X_B|): everything the edges leaving i share.  Pixels past the ragged end of the
-  // keyframe were not staged: they become masked lanes (w = -1).
+  __syncwarp();
+  // match indices of edge k (k-th edge leaving i) -> index buffer k & 1.  TMA needs 16-byte granules: HW % 4 == 0
+  // (idx_tma); otherwise the lanes copy (same data, synchronous).
+  auto issue_idx = [&](int k) {
+    if (npx == 0) return;
+    const int32_t* src = match + (size_t)grp_edge[e_beg + k] * HW + px0;
+    int32_t* dst = s_idx + (k & 1) * kWarpPx;
+    if (idx_tma) {
+      if (lane == 0) {
+        mbar_expect_tx(s_bar + 1 + (k & 1), (uint32_t)npx * 4u);
+        tma_bulk_g2s(dst, src, (uint32_t)npx * 4u, s_bar + 1 + (k & 1));
+      }
+    } else {
+      for (int p = lane; p < npx; p += 32) dst[p] = __ldcs(src + p);
+      __syncwarp();
+    }
+  };
+  auto wait_idx = [&](int k) {
+    if (idx_tma && npx > 0) mbar_wait(s_bar + 1 + (k & 1), (uint32_t)(k >> 1) & 1u);
+  };
+  if (npx > 0 && lane == 0) {
+    mbar_expect_tx(s_bar, (uint32_t)npx * 16u);
+    tma_bulk_g2s(s_Xi, pm + (size_t)i * HW + px0, (uint32_t)npx * 16u, s_bar);
+  }
+  if (n_e > 0) issue_idx(0);
+  if (npx > 0) mbar_wait(s_bar, 0);
+  // Pair p of a lane = pixels A = 64 p + lane and B = A + 32 of the slice.  Re-lay the two staged float4 in place as
+  // lane pairs, (xA, xB, yA, yB) in A's slot and (zA, zB, wA, wB) in B's, and keep (1/|X_A|, 1/|X_B|):
+  // everything the edges leaving i share.  Thread-private slots: no synchronisation needed.
 #pragma unroll 2
   for (int p = 0; p < kPairs; ++p) {
-    const int pa = 2 * p * kAccThreads + tid, pb = pa + kAccThreads;
-    float4 A = make_float4(0.f, 0.f, 0.f, -1.f), B = A;
-    if (pa < npx) A = s_Xi[pa];
-    if (pb < npx) B = s_Xi[pb];
+    const int pa = 64 * p + lane, pb = pa + 32;
+    const float4 A = s_Xi[pa], B = s_Xi[pb];
     const float da2 = fmaxf(fmaf(A.x, A.x, fmaf(A.y, A.y, A.z * A.z)), 1e-20f);
     const float db2 = fmaxf(fmaf(B.x, B.x, fmaf(B.y, B.y, B.z * B.z)), 1e-20f);
     const float ra = rsq(da2), rb = rsq(db2);
     s_Xi[pa] = make_float4(A.x, B.x, A.y, B.y);
     s_Xi[pb] = make_float4(A.z, B.z, A.w, B.w);
-    s_der[p * kAccThreads + tid] = make_float4(ra, rb, da2 * ra, db2 * rb);
+    s_rdi[32 * p + lane] = make_float2(ra, rb);
   }
 
-  for (int ei = grp_ptr[g]; ei < grp_ptr[g + 1]; ++ei) {
-    const int e = grp_edge[ei];
-    const int j = edges[2 * e + 1];
-    if (tid < 12) s_T[tid] = edgeT[(size_t)e * 12 + tid];   // s_ij R_ij [9], t_ij [3] (kernel k_edge_prep)
-    __syncthreads();
-    double Td[12];
-#pragma unroll
-    for (int k = 0; k < 12; ++k) Td[k] = s_T[k];
+  // Gathers: per-lane 16-byte cp.async into the warp's ring, kStages - 1 pairs ahead of the arithmetic, flat over the
+  // (edge, pair) sequence so the pipeline never drains between edges.  An out-of-range index is a masked match.
+  auto gather_pair = [&](const float4* __restrict__ Pj, const int32_t* __restrict__ ix, int p, int stage) {
+    const int nA = ix[64 * p + lane], nB = ix[64 * p + 32 + lane];
+    float4* dst = s_ring + stage * 64 + lane;
+    if ((unsigned)nA < (unsigned)HW) cp_async16(dst, Pj + nA); else *dst = make_float4(0.f, 0.f, 0.f, -1.f);
+    if ((unsigned)nB < (unsigned)HW) cp_async16(dst + 32, Pj + nB); else dst[32] = make_float4(0.f, 0.f, 0.f, -1.f);
+  };
+  auto pj_of = [&](int k) -> const float4* { return pm + (size_t)edges[2 * grp_edge[e_beg + k] + 1] * HW; };
 
-    const float4* __restrict__ Pj = pm + (size_t)j * HW;
-    const int32_t* __restrict__ mt = match + (size_t)e * HW + px0;
+  static_assert(kStages - 1 <= kPairs, "the prologue stays inside the first edge");
+  if (n_e > 0) {
+    wait_idx(0);
+    const float4* Pj = pj_of(0);
+#pragma unroll
+    for (int t = 0; t < kStages - 1; ++t) { gather_pair(Pj, s_idx, t, t); cp_async_commit(); }
+  }
+
+  for (int k = 0; k < n_e; ++k) {
+    const int e = grp_edge[e_beg + k];
+    // index buffer (k + 1) & 1 was last read while edge k - 1 was processed: free for edge k + 1
+    const bool has_next = k + 1 < n_e;
+    if (has_next) issue_idx(k + 1);
+    const float4* __restrict__ Pj = pj_of(k);
+    const float4* __restrict__ Pj_next = has_next ? pj_of(k + 1) : Pj;
+    const int32_t* __restrict__ idx = s_idx + (k & 1) * kWarpPx;
+    const int32_t* __restrict__ idx_next = s_idx + ((k + 1) & 1) * kWarpPx;
+    double Td[12];   // s_ij R_ij [9], t_ij [3] (kernel k_edge_prep)
+#pragma unroll
+    for (int q = 0; q < 12; ++q) Td[q] = __ldg(edgeT + (size_t)e * 12 + q);
 
     f2 acc[kAccSlots];
 #pragma unroll
-    for (int k = 0; k < kAccSlots; ++k) acc[k] = make_float2(0.f, 0.f);
+    for (int q = 0; q < kAccSlots; ++q) acc[q] = make_float2(0.f, 0.f);
     unsigned int cnt = 0, sum_m = 0, sum_n = 0;   // <= 16 terms each < 2^28: no overflow (HW <= 2^28 checked at create)
 
-    auto ld_idx = [&](int row) -> int {
-      const int p = row * kAccThreads + tid;
-      return (p < npx) ? __ldcs(mt + p) : -1;
-    };
-    auto gather = [&](int n) -> float4 {
-      return ((unsigned)n < (unsigned)HW) ? __ldg(Pj + n) : make_float4(0.f, 0.f, 0.f, -1.f);
-    };
     // delta = T_ij X_j - X_i in FP64: |delta| ~ noise << |x|; in fp32 it would carry ~ulp(|x|) per match
     auto delta = [&](const float4 Xj, float xi0, float xi1, float xi2, float& d0, float& d1, float& d2_) {
       const double Xjx = (double)Xj.x, Xjy = (double)Xj.y, Xjz = (double)Xj.z;
@@ -294,45 +349,46 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
       d1 = (float)fma(Td[3], Xjx, fma(Td[4], Xjy, fma(Td[5], Xjz, Td[10] - (double)xi1)));
       d2_ = (float)fma(Td[6], Xjx, fma(Td[7], Xjy, fma(Td[8], Xjz, Td[11] - (double)xi2)));
     };
-    auto process = [&](int p, int nA, int nB, const float4 XjA, const float4 XjB) {
-      if (XjA.w < 0.f && XjB.w < 0.f) return;               // neither lane has a match (whole invalid bands: warp-uniform)
-      const int pa = 2 * p * kAccThreads + tid, pb = pa + kAccThreads;
-      const float4 P0 = s_Xi[pa], P1 = s_Xi[pb];           // (xA, xB, yA, yB), (zA, zB, wA, wB)
-      const bool vA = (XjA.w >= 0.f) && (P1.z >= 0.f), vB = (XjB.w >= 0.f) && (P1.w >= 0.f);
-      if (!(vA || vB)) return;
-      const float4 der = s_der[p * kAccThreads + tid];
-      f2 del0, del1, del2;
-      delta(XjA, P0.x, P0.z, P1.x, del0.x, del1.x, del2.x);
-      delta(XjB, P0.y, P0.w, P1.y, del0.y, del1.y, del2.y);
-      f2 sq = make_float2(P1.z, P1.w) * make_float2(XjA.w, XjB.w);
-      sq.x = vA ? sq.x : 0.f;
-      sq.y = vB ? sq.y : 0.f;
-      accumulate_pair(acc, del0, del1, del2, make_float2(P0.x, P0.y), make_float2(P0.z, P0.w), make_float2(P1.x, P1.y),
-                      make_float2(der.x, der.y), make_float2(der.z, der.w), sq, prm);
-      cnt += (vA ? 1u : 0u) + (vB ? 1u : 0u);
-      sum_m += (vA ? (unsigned)pa : 0u) + (vB ? (unsigned)pb : 0u);
-      sum_n += (vA ? (unsigned)nA : 0u) + (vB ? (unsigned)nB : 0u);
-    };
 
-    // software pipeline over the thread's pairs: indices two pairs ahead, gathers one pair ahead
-    int nA0 = ld_idx(0), nA1 = ld_idx(1);
-    int nB0 = ld_idx(2), nB1 = ld_idx(3);
-    float4 XA0 = gather(nA0), XA1 = gather(nA1);
-#pragma unroll 1
+#pragma unroll 4
     for (int p = 0; p < kPairs; ++p) {
-      const float4 XB0 = gather(nB0), XB1 = gather(nB1);
-      const int nC0 = ld_idx(2 * p + 4), nC1 = ld_idx(2 * p + 5);
-      process(p, nA0, nA1, XA0, XA1);
-      nA0 = nB0; nA1 = nB1; XA0 = XB0; XA1 = XB1; nB0 = nC0; nB1 = nC1;
+      // issue the gathers of the pair kStages - 1 ahead (of this edge, or of the next edge) into the slot freed last iteration
+      {
+        const int pn = p + kStages - 1;
+        const int stage = (k * kPairs + pn) % kStages;
+        if (pn < kPairs) {
+          gather_pair(Pj, idx, pn, stage);
+        } else if (has_next) {
+          if (pn == kPairs) wait_idx(k + 1);
+          gather_pair(Pj_next, idx_next, pn - kPairs, stage);
+        }
+        cp_async_commit();                                   // (possibly empty) group: uniform accounting
+        cp_async_wait<kStages - 1>();                        // the group of pair p has landed
+      }
+      const float4* ring = s_ring + ((k * kPairs + p) % kStages) * 64 + lane;
+      const float4 XA0 = ring[0], XA1 = ring[32];
+      const int pa = 64 * p + lane, pb = pa + 32;
+      const float4 P1 = s_Xi[pb];                            // (zA, zB, wA, wB)
+      const bool vA = (XA0.w >= 0.f) && (P1.z >= 0.f), vB = (XA1.w >= 0.f) && (P1.w >= 0.f);
+      if (__any_sync(0xffffffffu, vA || vB)) {               // whole invalid bands are skipped warp-uniformly
+        const float4 P0 = s_Xi[pa];                          // (xA, xB, yA, yB)
+        const float2 rdi = s_rdi[32 * p + lane];
+        f2 del0, del1, del2;
+        delta(XA0, P0.x, P0.z, P1.x, del0.x, del1.x, del2.x);
+        delta(XA1, P0.y, P0.w, P1.y, del0.y, del1.y, del2.y);
+        f2 sq = make_float2(P1.z, P1.w) * make_float2(XA0.w, XA1.w);
+        sq.x = vA ? sq.x : 0.f;
+        sq.y = vB ? sq.y : 0.f;
+        accumulate_pair(acc, del0, del1, del2, make_float2(P0.x, P0.y), make_float2(P0.z, P0.w), make_float2(P1.x, P1.y),
+                        rdi, sq, prm);
+        const unsigned mA = vA ? 0xffffffffu : 0u, mB = vB ? 0xffffffffu : 0u;
+        cnt += (mA & 1u) + (mB & 1u);
+        sum_m += ((unsigned)pa & mA) + ((unsigned)pb & mB);
+        sum_n += ((unsigned)idx[pa] & mA) + ((unsigned)idx[pb] & mB);
+      }
     }
 
-    // ---- lanes A + B -> thread partials (fp32, <= 16 terms) -> FP64 warp sums -> fixed-order cross-warp sum ----
-    {
-      float accs[kSlots];
-#pragma unroll
-      for (int k = 0; k < kSlots; ++k) accs[k] = (k < kAccSlots) ? acc[k].x + acc[k].y : 0.f;
-      warp_reduce_slots(accs, s_red + warp * kSlots, lane);
-    }
+    // ---- lanes A + B -> thread partials (fp32, <= 16 terms) -> FP64 warp sums -> the (edge, slice) record ----
     unsigned long long chk = (unsigned long long)sum_m + (unsigned long long)cnt * (unsigned long long)px0;   // sum of m
     chk = chk * (unsigned long long)HW + (unsigned long long)sum_n;
 #pragma unroll
@@ -340,25 +396,14 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
       cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
       chk += __shfl_xor_sync(0xffffffffu, chk, o);
     }
-    if (lane == 0) { s_cnt[warp] = cnt; s_chk[warp] = chk; }
-    __syncthreads();
-    double* out = partials + ((size_t)e * tiles + tile) * kPartialStride;
-    if (tid < kSlotCnt) {
-      double v = 0.0;
+    {
+      float accs[kSlots];
 #pragma unroll
-      for (int w = 0; w < kWarps; ++w) v += s_red[w * kSlots + tid];
-      out[tid] = v;
-    } else if (tid == kSlotCnt) {
-      long long c = 0;
-#pragma unroll
-      for (int w = 0; w < kWarps; ++w) c += s_cnt[w];
-      reinterpret_cast<long long*>(out)[kSlotCnt] = c;
-    } else if (tid == kSlotChk) {
-      unsigned long long h = 0ull;
-#pragma unroll
-      for (int w = 0; w < kWarps; ++w) h += s_chk[w];
-      reinterpret_cast<unsigned long long*>(out)[kSlotChk] = h;
+      for (int q = 0; q < kSlots; ++q) accs[q] = (q < kAccSlots) ? acc[q].x + acc[q].y : 0.f;
+      warp_reduce_slots(accs, partials + ((size_t)e * (tiles * kWarps) + tile * kWarps + warp) * kPartialStride, lane,
+                        (unsigned long long)cnt, chk);
     }
+    __syncwarp();   // every lane is done with index buffer k & 1 (free for edge k + 2)
   }
 }
 
@@ -375,30 +420,44 @@ k_edge_prep(const double* __restrict__ poses, const int32_t* __restrict__ edges,
   for (int k = 0; k < 3; ++k) o[9 + k] = Tij.t[k];
 }
 
-// Kernel 2: per edge, sum the tile partials in tile order (FP64), then the adjoint congruence
-// A_e = Ad^T M Ad, b_e = Ad^T c with Ad = Ad_{T_i^-1}.
-__global__ void __launch_bounds__(64)
+// Kernel 2: per edge, sum the slice records (FP64, fixed order: kFinGroups interleaved running sums, then group
+// 0..5), then the adjoint congruence A_e = Ad^T M Ad, b_e = Ad^T c with Ad = Ad_{T_i^-1}.
+constexpr int kFinGroups = 6;
+constexpr int kFinThreads = 256;
+__global__ void __launch_bounds__(kFinThreads)
 k_finalize(const double* __restrict__ partials, const int32_t* __restrict__ edges, const double* __restrict__ poses,
            double* __restrict__ blocks35, double* __restrict__ edge_cost, int32_t* __restrict__ n_valid,
-           unsigned long long* __restrict__ checksum, int chunks) {
+           unsigned long long* __restrict__ checksum, int records) {
+  __shared__ double s_part[kFinGroups][kSlots];
   __shared__ double s_sum[kSlots];
   __shared__ double s_M[49], s_Ad[49], s_T[49];
   const int e = blockIdx.x, t = threadIdx.x;
-  const double* p = partials + (size_t)e * chunks * kPartialStride;
+  const double* p = partials + (size_t)e * records * kPartialStride;
+  if (t < kFinGroups * kSlots) {
+    const int grp = t / kSlots, q = t - grp * kSlots;
+    if (q < kSlotCnt) {
+      double v = 0.0;
+      for (int c = grp; c < records; c += kFinGroups) v += p[(size_t)c * kPartialStride + q];
+      s_part[grp][q] = v;
+    } else {   // integer slots (and the unused one): exact in any order
+      unsigned long long v = 0ull;
+      for (int c = grp; c < records; c += kFinGroups) v += reinterpret_cast<const unsigned long long*>(p + (size_t)c * kPartialStride)[q];
+      reinterpret_cast<unsigned long long*>(&s_part[grp][0])[q] = v;
+    }
+  } else if (t == kFinGroups * kSlots) {
+    adjoint_of_inverse(load_pose(poses + 8 * edges[2 * e]), s_Ad);
+  }
+  __syncthreads();
   if (t < kSlotCnt) {
     double v = 0.0;
-    for (int c = 0; c < chunks; ++c) v += p[(size_t)c * kPartialStride + t];
+#pragma unroll
+    for (int grp = 0; grp < kFinGroups; ++grp) v += s_part[grp][t];
     s_sum[t] = v;
-  } else if (t == kSlotCnt) {
-    long long v = 0;
-    for (int c = 0; c < chunks; ++c) v += reinterpret_cast<const long long*>(p + (size_t)c * kPartialStride)[kSlotCnt];
-    n_valid[e] = (int32_t)v;
-  } else if (t == kSlotChk) {
+  } else if (t == kSlotCnt || t == kSlotChk) {
     unsigned long long v = 0ull;
-    for (int c = 0; c < chunks; ++c) v += reinterpret_cast<const unsigned long long*>(p + (size_t)c * kPartialStride)[kSlotChk];
-    checksum[e] = v;
-  } else if (t == 39) {
-    adjoint_of_inverse(load_pose(poses + 8 * edges[2 * e]), s_Ad);
+#pragma unroll
+    for (int grp = 0; grp < kFinGroups; ++grp) v += reinterpret_cast<const unsigned long long*>(&s_part[grp][0])[t];
+    if (t == kSlotCnt) n_valid[e] = (int32_t)v; else checksum[e] = v;
   }
   __syncthreads();
   if (t < 49) {
@@ -473,13 +532,15 @@ cudaError_t launch_accumulate(Ctx* c) {
   k_edge_prep<<<(c->E + 127) / 128, 128, 0, c->stream>>>(c->poses, c->edges, c->edgeT, c->E);
   cudaError_t err = cudaGetLastError();
   if (err != cudaSuccess) return err;
+  // TMA bulk copies of the match indices need 16-byte granules and addresses
+  const int idx_tma = (c->HW % 4 == 0) && (reinterpret_cast<uintptr_t>(c->match) % 16 == 0);
   k_accumulate<<<c->n_groups * c->chunks, kAccThreads, kAccSmem, c->stream>>>(
-      c->pm, c->match, c->edges, c->grp_kf, c->grp_ptr, c->grp_edge, c->edgeT, c->partials, c->HW, c->chunks, p);
+      c->pm, c->match, c->edges, c->grp_kf, c->grp_ptr, c->grp_edge, c->edgeT, c->partials, c->HW, c->chunks, idx_tma, p);
   err = cudaGetLastError();
   if (err != cudaSuccess) return err;
   if (c->profiling) cudaEventRecord(c->ev[1], c->stream);
-  k_finalize<<<c->E, 64, 0, c->stream>>>(c->partials, c->edges, c->poses, c->blocks35, c->edge_cost, c->n_valid,
-                                         c->checksum, c->chunks);
+  k_finalize<<<c->E, kFinThreads, 0, c->stream>>>(c->partials, c->edges, c->poses, c->blocks35, c->edge_cost, c->n_valid,
+                                                  c->checksum, c->chunks * (kAccThreads / 32));
   c->launches += 3;
   return cudaGetLastError();
 }

@@ -227,7 +227,7 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
   CUB(upload(&c->pair_edge, c->h_pair_edge, c->stream));
   CUB(upload(&c->pairhi_ptr, c->h_pairhi_ptr, c->stream));
   CUB(dev_alloc(&c->poses, (size_t)8 * c->N));
-  CUB(dev_alloc(&c->partials, (size_t)c->E * c->chunks * kPartialStride));
+  CUB(dev_alloc(&c->partials, (size_t)c->E * c->chunks * (kAccThreads / 32) * kPartialStride));
   CUB(dev_alloc(&c->blocks35, (size_t)c->E * 35));
   CUB(dev_alloc(&c->edge_cost, (size_t)c->E));
   CUB(dev_alloc(&c->n_valid, (size_t)c->E));

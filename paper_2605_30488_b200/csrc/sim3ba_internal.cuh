@@ -11,9 +11,9 @@
 
 namespace sim3ba {
 
-constexpr int kTilePx = 3072;        // pixels of one edge handled by one accumulate CTA
-constexpr int kAccThreads = 192;
-// doubles per (edge, tile) partial record: [0..27] upper triangle of M = sum J_xi^T Omega J_xi (row-major,
+constexpr int kAccThreads = 64;      // accumulate CTA: two independent warps
+constexpr int kTilePx = 16 * kAccThreads;   // pixels of a keyframe handled by one accumulate CTA (512 contiguous per warp)
+// doubles per (edge, 512-pixel warp slice) partial record: [0..27] upper triangle of M = sum J_xi^T Omega J_xi (row-major,
 // r <= c; (3,6), (4,6), (5,6) are structurally zero), [28..34] c = sum J_xi^T Omega e, [35] sum w r^2,
 // [36] sum min(r^2, kappa^2) (robust cost = [35] - [36]/2), [37] n_valid (int64 bits), [38] checksum (uint64 bits)
 constexpr int kPartialStride = 40;
@@ -62,7 +62,7 @@ struct Ctx {
   int solver_mode = 0;             // 0: tile-sparse plan of the graph, 1: dense plan (every lower tile)
   std::vector<uint8_t> h_fixed;
   // per-edge results
-  double* partials = nullptr;      // [E][chunks][kPartialStride]
+  double* partials = nullptr;      // [E][chunks * warps per CTA][kPartialStride]: one record per (edge, 512-pixel slice)
   double* blocks35 = nullptr;      // [E][35]
   double* edge_cost = nullptr;     // [E]
   int32_t* n_valid = nullptr;      // [E]
