@@ -16,8 +16,8 @@
 // (FFMA2 / FMUL2 / FADD2: one issue slot per two lanes), accumulators included.
 //
 // Precision plan: delta = T_ij X_j - X_i in FP64 (the one cancellation of the residual); everything
-// after it and the per-thread partial sums (<= 8 terms per lane, 16 per thread) in fp32; every sum from
-// the per-thread partial upwards (warp, CTA, edge, adjoint congruence) in FP64.  No floating-point
+// after it, the per-thread partial sums (<= 8 terms per lane, 16 per thread) and the first two levels of
+// the warp tree (<= 64 terms) in fp32; every sum from there upwards (warp, edge, adjoint congruence) in FP64.  No floating-point
 // atomics: the reduction order is fixed, results are run-to-run identical.
 #include "sim3ba_internal.cuh"
 #include "sim3_math.cuh"
@@ -182,30 +182,32 @@ __device__ __forceinline__ void accumulate_pair(f2 (&acc)[kAccSlots], const f2 d
 
 // Warp reduction of the 40 fp32 thread partials into FP64 warp sums by recursive halving: at every
 // level a lane keeps one half of its slots and hands the other half to its partner, so the whole tree
-// costs 20 + 10 + 5 + 5 + 5 exchanges instead of 40 x 5.  Level 1 exchanges the fp32 partials and
-// converts both operands (the sums are FP64 from here on).  Lanes with (lane & 3) == 0 end up holding
-// the warp totals of slots base .. base + 4, base = 20 b4 + 10 b3 + 5 b2 (bits of the lane index), and
-// write them to the warp's record; the lane holding slots 35..39 stores the two integers (warp totals,
-// every lane has them) in slots 37 and 38.
+// costs 20 + 10 + 5 + 5 + 5 exchanges instead of 40 x 5.  The first two levels add fp32 partials (two
+// roundings of 2^-24 on sums of <= 64 terms -- the same order as the rounding every term already
+// carries); from the 64-term partial upwards every sum is FP64.  Lanes with (lane & 3) == 0 end up
+// holding the warp totals of slots base .. base + 4, base = 20 b4 + 10 b3 + 5 b2 (bits of the lane
+// index), and write them to the warp's record; the lane holding slots 35..39 stores the two integers
+// (warp totals, every lane has them) in slots 37 and 38.
 __device__ __forceinline__ void warp_reduce_slots(const float (&acc)[kSlots], double* __restrict__ out, const int lane,
                                                   unsigned long long cnt, unsigned long long chk) {
-  double v[20];
+  float h[20];
   {
     const bool up = lane & 16;
 #pragma unroll
     for (int k = 0; k < 20; ++k) {
       const float keep = up ? acc[20 + k] : acc[k];
       const float send = up ? acc[k] : acc[20 + k];
-      v[k] = (double)keep + (double)__shfl_xor_sync(0xffffffffu, send, 16);
+      h[k] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
     }
   }
+  double v[10];
   {
     const bool up = lane & 8;
 #pragma unroll
     for (int k = 0; k < 10; ++k) {
-      const double keep = up ? v[10 + k] : v[k];
-      const double send = up ? v[k] : v[10 + k];
-      v[k] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+      const float keep = up ? h[10 + k] : h[k];
+      const float send = up ? h[k] : h[10 + k];
+      v[k] = (double)(keep + __shfl_xor_sync(0xffffffffu, send, 8));
     }
   }
   {
