@@ -106,6 +106,19 @@ int sim3ba_step(sim3ba_ctx* ctx);
  * poses to *h_cost (each if non-NULL).  Pinned host memory recommended.  Synchronises. */
 int sim3ba_step_host(sim3ba_ctx* ctx, const double* h_poses_in, double* h_poses_out, double* h_cost);
 
+/* The whole job with HOST buffers (the end-to-end leg of bench.py): allocates device memory, copies the
+ * graph in -- h_points [N][HW][3], h_conf [N][HW], h_edges [E][2], h_match [E][HW], layouts as in
+ * sim3ba_create, pinned host memory recommended -- creates a context, runs n_iters Gauss-Newton
+ * iterations (sim3ba_step, a1-a8 each; fixed count) from h_poses_in [N][8], copies the
+ * final poses to h_poses_out [N][8] and, if h_cost is non-NULL, the robust cost at the start of
+ * iteration it to h_cost[it]; frees everything and synchronises the stream.  Nothing is kept.
+ * Errors as sim3ba_create / sim3ba_step; the message is read with sim3ba_last_error(NULL). */
+int sim3ba_optimize_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_edges, const float* h_points,
+                         const float* h_conf, const int32_t* h_edges, const int32_t* h_match,
+                         const int32_t* h_fixed_kf, int32_t n_fixed, const sim3ba_params* params,
+                         const double* h_poses_in, int32_t n_iters, double* h_poses_out, double* h_cost,
+                         void* cuda_stream);
+
 /* a8 only: T_i <- Exp(tau_i) T_i with the tau of the last solve. */
 int sim3ba_retract(sim3ba_ctx* ctx);
 
@@ -145,11 +158,20 @@ int sim3ba_get_bookkeeping(sim3ba_ctx* ctx, const int32_t** h_kf_ptr, const int3
  * tests: oracle (H, g) -> GPU solver).  d_H [7N][7N] row-major symmetric double, d_g [7N]. */
 int sim3ba_load_system(sim3ba_ctx* ctx, const double* d_H, const double* d_g);
 
-/* Solver plan (a7).  mode 0 (default): the Cholesky walks only the non-zero 64x64 tiles of L (symbolic
- * tile-level factorisation of the keyframe graph, fill included, computed at create); mode 1: every
- * lower tile (the dense blocked factorisation; also used for systems given by sim3ba_load_system).
- * Both give the same tau up to rounding. */
+/* Solver plan (a7), all giving the same tau up to rounding.
+ * mode 2 (default): band + border block Cholesky ("sparse Cholesky") -- the free keyframes are
+ *   split at create into interior keyframes (independent segments of a temporal chain, block band 3) and
+ *   border keyframes (one endpoint of every longer link: loop closures, inter-agent edges; separator triples
+ *   that cap a segment's length); segments are eliminated at 7x7 granularity in parallel, the Schur complement
+ *   on the border is a small dense system for the tiled Cholesky.  Where the graph does not have that shape
+ *   (a segment touching more than 28 border keyframes, more than 292 border keyframes) mode 2 runs mode 0.
+ * mode 0: the tiled Cholesky walks only the non-zero 64x64 tiles of L (symbolic tile-level factorisation of the
+ *   keyframe graph in temporal order, fill included, computed at create).
+ * mode 1: every lower tile (the dense blocked factorisation; always used for sim3ba_load_system). */
 int sim3ba_set_solver_mode(sim3ba_ctx* ctx, int32_t mode);
+/* Band + border plan of the graph (host output): h_info[0] = 1 if mode 2 applies to this graph, [1] interior
+ * keyframes, [2] segments, [3] border keyframes, [4] longest segment, [5] most border keyframes touched by a segment. */
+int sim3ba_get_bb_info(sim3ba_ctx* ctx, int32_t h_info[6]);
 /* Host outputs (each may be NULL): non-zero tiles of the active plan, lower tiles of the dense plan,
  * flop count of the active plan (factor + both triangular solves, at tile granularity), CTAs of
  * the last persistent solve launch. */

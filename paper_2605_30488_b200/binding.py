@@ -16,10 +16,10 @@ LIB_PATH = os.path.join(_HERE, "libsim3ba.so")
 
 EXPORTS = (
     "sim3ba_default_params", "sim3ba_create", "sim3ba_destroy", "sim3ba_set_params", "sim3ba_set_poses",
-    "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_host",
+    "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_host", "sim3ba_optimize_host",
     "sim3ba_retract", "sim3ba_get_edge_stats", "sim3ba_get_edge_blocks", "sim3ba_get_system",
     "sim3ba_get_update", "sim3ba_get_bookkeeping", "sim3ba_load_system", "sim3ba_get_launch_count",
-    "sim3ba_set_solver_mode", "sim3ba_get_solver_info",
+    "sim3ba_set_solver_mode", "sim3ba_get_solver_info", "sim3ba_get_bb_info",
     "sim3ba_set_profiling", "sim3ba_get_phase_ms", "sim3ba_copy_d2d", "sim3ba_last_error", "sim3ba_version",
 )
 
@@ -61,6 +61,7 @@ def load_library() -> C.CDLL:
         "sim3ba_solve": [vp],
         "sim3ba_step": [vp],
         "sim3ba_step_host": [vp, vp, vp, vp],
+        "sim3ba_optimize_host": [i32, i32, i32, i32, vp, vp, vp, vp, P(i32), i32, P(Params), vp, i32, vp, vp, vp],
         "sim3ba_retract": [vp],
         "sim3ba_get_edge_stats": [vp, P(vp), P(vp), P(vp)],
         "sim3ba_get_edge_blocks": [vp, P(vp)],
@@ -71,6 +72,7 @@ def load_library() -> C.CDLL:
         "sim3ba_get_launch_count": [vp, P(i64)],
         "sim3ba_set_solver_mode": [vp, i32],
         "sim3ba_get_solver_info": [vp, P(i32), P(i32), P(C.c_double), P(i32)],
+        "sim3ba_get_bb_info": [vp, P(i32)],
         "sim3ba_set_profiling": [vp, i32],
         "sim3ba_get_phase_ms": [vp, P(C.c_float)],
         "sim3ba_copy_d2d": [vp, vp, vp, C.c_uint64],
@@ -90,6 +92,23 @@ def load_library() -> C.CDLL:
 def make_params(sigma_ray=0.003, sigma_dist=10.0, huber_k=1.345, conf_min=0.0, lm_lambda=0.0, eps0=1e-6,
                 max_attempts=6) -> Params:
     return Params(sigma_ray, sigma_dist, huber_k, conf_min, lm_lambda, eps0, max_attempts, 0)
+
+
+def optimize_host(points, conf, edges, match, fixed_kf: Sequence[int], params: Optional[Params], height: int, width: int,
+                  poses_in, n_iters: int, poses_out, cost_out=None, stream: int = 0):
+    """sim3ba_optimize_host: the whole job with HOST (CPU, pinned recommended) torch tensors -- graph upload, create,
+    n_iters GN steps, poses (and per-iteration costs) back.  Argument marshalling only."""
+    lib = load_library()
+    for t in (points, conf, edges, match, poses_in, poses_out):
+        assert t.device.type == "cpu" and t.is_contiguous()
+    fk = (C.c_int32 * max(1, len(fixed_kf)))(*fixed_kf)
+    prm = params if params is not None else make_params()
+    rc = lib.sim3ba_optimize_host(points.shape[0], height, width, edges.shape[0], points.data_ptr(), conf.data_ptr(),
+                                  edges.data_ptr(), match.data_ptr(), fk, len(fixed_kf), C.byref(prm), poses_in.data_ptr(),
+                                  n_iters, poses_out.data_ptr(), cost_out.data_ptr() if cost_out is not None else None,
+                                  stream)
+    if rc:
+        raise Sim3BAError(rc, (lib.sim3ba_last_error(None) or b"").decode())
 
 
 class Sim3BA:
@@ -237,6 +256,12 @@ class Sim3BA:
         nt, ntd, fl, gr = C.c_int32(), C.c_int32(), C.c_double(), C.c_int32()
         self._check(self.lib.sim3ba_get_solver_info(self._h, C.byref(nt), C.byref(ntd), C.byref(fl), C.byref(gr)))
         return dict(n_tiles=nt.value, n_tiles_dense=ntd.value, flops=fl.value, grid=gr.value)
+
+    def bb_info(self) -> Dict[str, int]:
+        """Band + border plan of the graph (solver mode 2)."""
+        info = (C.c_int32 * 6)()
+        self._check(self.lib.sim3ba_get_bb_info(self._h, info))
+        return dict(zip(("valid", "n_interior", "n_segments", "n_border", "max_segment", "max_segment_border"), list(info)))
 
     def launch_count(self) -> int:
         n = C.c_int64()

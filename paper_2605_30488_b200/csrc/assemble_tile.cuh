@@ -26,7 +26,7 @@ struct AsmArgs {
 
 __device__ __forceinline__ int tri7(int r, int c) { return r * 7 - r * (r - 1) / 2 + (c - r); }   // r <= c
 
-__device__ __noinline__ double asm_element(const AsmArgs& a, int R, int C, double eps) {
+static __device__ __noinline__ double asm_element(const AsmArgs& a, int R, int C, double eps) {
   if (C > R) return 0.0;
   if (R >= a.n) return (R == C) ? 1.0 : 0.0;
   const int kr = R / 7, kc = C / 7;
@@ -54,7 +54,7 @@ __device__ __noinline__ double asm_element(const AsmArgs& a, int R, int C, doubl
 }
 
 // 256 threads: thread (row = tid / 4, quarter = tid % 4) writes 16 consecutive doubles of its row
-__device__ __noinline__ void assemble_tile(const AsmArgs& a, int ti, int tj, double eps, int tid) {
+static __device__ __noinline__ void assemble_tile(const AsmArgs& a, int ti, int tj, double eps, int tid) {
   const int rr = tid >> 2, q = tid & 3;
   const int R = ti * kNB + rr;
   double* dst = a.L + (size_t)R * a.npad + (size_t)tj * kNB + 16 * q;

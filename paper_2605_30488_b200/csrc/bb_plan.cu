@@ -1,0 +1,180 @@
+// a0 (host): band + border analysis of the keyframe graph for the block (7x7) Cholesky of a7
+// (solver mode 2; layout and roles in sim3ba_internal.cuh, kernel in k_solve_bb.cu).
+//
+// The Sim(3) graph of PAPER.md:108 is, per agent, a temporal chain (edges (k, k+1..k+3)) plus a few
+// long links: loop closures and inter-agent edges.  One endpoint of every long link becomes a BORDER
+// keyframe (greedy vertex cover, the endpoint with more long links first); a chain longer than
+// `lmax` interior keyframes is cut by making the next kBand keyframes border as well (substructuring:
+// the pieces are then independent and are eliminated in parallel).  Integer bookkeeping only.
+#include <stdlib.h>
+
+#include <algorithm>
+#include <utility>
+
+#include "sim3ba_internal.cuh"
+
+namespace sim3ba {
+
+namespace {
+template <class T>
+cudaError_t up(T** dst, const std::vector<T>& src, cudaStream_t s) {
+  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(dst), std::max<size_t>(src.size(), 1) * sizeof(T));
+  if (e != cudaSuccess || src.empty()) return e;
+  return cudaMemcpyAsync(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice, s);
+}
+template <class T>
+cudaError_t dalloc(T** p, size_t count) {
+  return cudaMalloc(reinterpret_cast<void**>(p), std::max<size_t>(count, 1) * sizeof(T));
+}
+}  // namespace
+
+void free_bb_plan(BBPlan& p) {
+  cudaFree(p.seg_ptr); cudaFree(p.seg_bptr); cudaFree(p.seg_bord); cudaFree(p.col_kf); cudaFree(p.col_nb); cudaFree(p.col_ofs);
+  cudaFree(p.col_band); cudaFree(p.col_bpair); cudaFree(p.col_bofs); cudaFree(p.bord_kf); cudaFree(p.bord_sptr);
+  cudaFree(p.bord_seg); cudaFree(p.bord_slot); cudaFree(p.bb_pair); cudaFree(p.colbuf); cudaFree(p.seg_rhs);
+  cudaFree(p.LB); cudaFree(p.rhsB); cudaFree(p.ysolB); cudaFree(p.DinvB); cudaFree(p.tauB);
+  free_plan(p.dense);
+  p = BBPlan();
+}
+
+bool build_bb_plan(Ctx* c, std::string& err) {
+  BBPlan& P = c->plan_bb;
+  P.ready = true;
+  P.valid = false;
+  const int N = c->N;
+  const int n_pairs = (int)c->h_pair_kf.size() / 2;
+  int lmax = 160;
+  if (const char* s = getenv("SIM3BA_BB_LMAX")) lmax = std::max(4, atoi(s));
+
+  enum { FIXED = 0, INTERIOR = 1, BORDER = 2 };
+  std::vector<int> role(N, INTERIOR);
+  for (int k = 0; k < N; ++k) if (c->h_fixed[k]) role[k] = FIXED;
+  // adjacency over the pairs with both endpoints free
+  std::vector<std::vector<std::pair<int32_t, int32_t>>> adj(N);   // (other keyframe, pair index)
+  std::vector<int> longdeg(N, 0);
+  for (int p = 0; p < n_pairs; ++p) {
+    const int hi = c->h_pair_kf[2 * p], lo = c->h_pair_kf[2 * p + 1];
+    if (role[hi] == FIXED || role[lo] == FIXED) continue;
+    adj[hi].push_back({lo, p});
+    adj[lo].push_back({hi, p});
+    if (hi - lo > kBand) { ++longdeg[hi]; ++longdeg[lo]; }
+  }
+  // vertex cover of the long links (pairs are sorted by (hi, lo))
+  for (int p = 0; p < n_pairs; ++p) {
+    const int hi = c->h_pair_kf[2 * p], lo = c->h_pair_kf[2 * p + 1];
+    if (role[hi] == FIXED || role[lo] == FIXED || hi - lo <= kBand) continue;
+    if (role[hi] == BORDER || role[lo] == BORDER) continue;
+    role[longdeg[lo] > longdeg[hi] ? lo : hi] = BORDER;
+  }
+  // segments: runs of interior keyframes in index order; natural cut where no band pair reaches on; forced
+  // cut after lmax keyframes by turning the interior keyframes of the next kBand indices into border
+  std::vector<int32_t> col_kf, seg_ptr(1, 0);
+  {
+    int reach = -1, run = 0, sep_until = -1;
+    for (int u = 0; u < N; ++u) {
+      if (role[u] != INTERIOR) continue;
+      if (u <= sep_until) { role[u] = BORDER; continue; }
+      if (run > 0 && reach < u) { seg_ptr.push_back((int32_t)col_kf.size()); run = 0; }
+      col_kf.push_back(u);
+      ++run;
+      for (auto& nb : adj[u])
+        if (nb.first > u && nb.first - u <= kBand && role[nb.first] == INTERIOR) reach = std::max(reach, (int)nb.first);
+      if (run >= lmax && reach > u) {   // the chain goes on: cut it
+        sep_until = u + kBand;
+        seg_ptr.push_back((int32_t)col_kf.size());
+        run = 0;
+        reach = -1;
+      }
+    }
+    if (run > 0) seg_ptr.push_back((int32_t)col_kf.size());
+  }
+  const int n_int = (int)col_kf.size(), n_seg = (int)seg_ptr.size() - 1;
+  std::vector<int32_t> bord_kf, bidx(N, -1), seg_of(N, -1), pos_of(N, -1);
+  for (int k = 0; k < N; ++k) if (role[k] == BORDER) { bidx[k] = (int32_t)bord_kf.size(); bord_kf.push_back(k); }
+  const int n_bord = (int)bord_kf.size();
+  for (int s = 0; s < n_seg; ++s)
+    for (int q = seg_ptr[s]; q < seg_ptr[s + 1]; ++q) { seg_of[col_kf[q]] = s; pos_of[col_kf[q]] = q; }
+
+  // border keyframes of every segment; structure checks
+  std::vector<int32_t> seg_bptr(1, 0), seg_bord;
+  int max_nb = 0, max_len = 0;
+  for (int s = 0; s < n_seg; ++s) {
+    std::vector<int32_t> b;
+    for (int q = seg_ptr[s]; q < seg_ptr[s + 1]; ++q)
+      for (auto& nb : adj[col_kf[q]]) {
+        const int v = nb.first;
+        if (role[v] == BORDER) b.push_back(bidx[v]);
+        else if (seg_of[v] != s || std::abs(pos_of[v] - q) > kBand) return true;   // not band + border: plan not used
+      }
+    std::sort(b.begin(), b.end());
+    b.erase(std::unique(b.begin(), b.end()), b.end());
+    max_nb = std::max(max_nb, (int)b.size());
+    max_len = std::max(max_len, seg_ptr[s + 1] - seg_ptr[s]);
+    seg_bord.insert(seg_bord.end(), b.begin(), b.end());
+    seg_bptr.push_back((int32_t)seg_bord.size());
+  }
+  if (max_nb > kMaxSegBorder || 7 * n_bord > 2048) return true;   // too much border: the tile plan is the better tool
+
+  // per-column block sources
+  std::vector<int64_t> col_ofs(n_int), col_bofs(n_int);
+  std::vector<int32_t> col_nb(n_int, 0);
+  std::vector<int32_t> col_band((size_t)n_int * kBand, -1), col_bpair;
+  size_t ofs = 0;
+  for (int s = 0; s < n_seg; ++s) {
+    const int nb = seg_bptr[s + 1] - seg_bptr[s];
+    for (int q = seg_ptr[s]; q < seg_ptr[s + 1]; ++q) {
+      const int u = col_kf[q];
+      col_ofs[q] = (int64_t)ofs;
+      col_nb[q] = nb;
+      ofs += ((size_t)(1 + kBand + nb) * 49 + 7 + 1) & ~(size_t)1;   // 16-byte granules
+      col_bofs[q] = (int64_t)col_bpair.size();
+      col_bpair.resize(col_bpair.size() + nb, -1);
+      for (auto& a : adj[u]) {
+        const int v = a.first;
+        if (role[v] == BORDER) {
+          const int slot = (int)(std::lower_bound(seg_bord.begin() + seg_bptr[s], seg_bord.begin() + seg_bptr[s + 1], bidx[v]) -
+                                 (seg_bord.begin() + seg_bptr[s]));
+          col_bpair[(size_t)col_bofs[q] + slot] = a.second;
+        } else if (pos_of[v] > q) {
+          col_band[(size_t)q * kBand + (pos_of[v] - q - 1)] = a.second;
+        }
+      }
+    }
+  }
+  // border side: segments touching a border keyframe, border-border pairs
+  std::vector<int32_t> bord_sptr(n_bord + 1, 0), bord_seg, bord_slot, bb_pair((size_t)n_bord * n_bord, -1);
+  {
+    std::vector<std::vector<std::pair<int32_t, int32_t>>> touch(n_bord);
+    for (int s = 0; s < n_seg; ++s)
+      for (int q = seg_bptr[s]; q < seg_bptr[s + 1]; ++q) touch[seg_bord[q]].push_back({s, q - seg_bptr[s]});
+    for (int b = 0; b < n_bord; ++b) {
+      for (auto& t : touch[b]) { bord_seg.push_back(t.first); bord_slot.push_back(t.second); }
+      bord_sptr[b + 1] = (int32_t)bord_seg.size();
+    }
+    for (int b = 0; b < n_bord; ++b)
+      for (auto& a : adj[bord_kf[b]])
+        if (role[a.first] == BORDER && a.first < bord_kf[b]) bb_pair[(size_t)b * n_bord + bidx[a.first]] = a.second;
+  }
+
+  P.n_int = n_int; P.n_seg = n_seg; P.n_bord = n_bord; P.max_nb = max_nb; P.max_len = max_len;
+  P.npadB = (7 * n_bord + kNB - 1) / kNB * kNB;
+  P.col_doubles = ofs;
+  P.h_seg_ptr = seg_ptr; P.h_seg_bptr = seg_bptr;
+  cudaError_t e = cudaSuccess;
+  auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return e == cudaSuccess; };
+  ok(up(&P.seg_ptr, seg_ptr, c->stream)); ok(up(&P.seg_bptr, seg_bptr, c->stream)); ok(up(&P.seg_bord, seg_bord, c->stream));
+  ok(up(&P.col_kf, col_kf, c->stream)); ok(up(&P.col_nb, col_nb, c->stream)); ok(up(&P.col_ofs, col_ofs, c->stream)); ok(up(&P.col_band, col_band, c->stream));
+  ok(up(&P.col_bpair, col_bpair, c->stream)); ok(up(&P.col_bofs, col_bofs, c->stream)); ok(up(&P.bord_kf, bord_kf, c->stream));
+  ok(up(&P.bord_sptr, bord_sptr, c->stream)); ok(up(&P.bord_seg, bord_seg, c->stream)); ok(up(&P.bord_slot, bord_slot, c->stream));
+  ok(up(&P.bb_pair, bb_pair, c->stream));
+  ok(dalloc(&P.colbuf, ofs)); ok(dalloc(&P.seg_rhs, seg_bord.size() * 7));
+  const size_t nB = (size_t)P.npadB;
+  ok(dalloc(&P.LB, nB * nB)); ok(dalloc(&P.rhsB, nB)); ok(dalloc(&P.ysolB, nB)); ok(dalloc(&P.DinvB, nB)); ok(dalloc(&P.tauB, nB));
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // the host vectors go out of scope
+  if (e != cudaSuccess) { err = std::string("build_bb_plan: ") + cudaGetErrorString(e); return false; }
+  if (P.npadB > 0 && !build_dense_plan(P.npadB / kNB, P.dense, c->stream, err)) return false;
+  P.valid = true;
+  return true;
+}
+
+}  // namespace sim3ba

@@ -41,7 +41,10 @@ constexpr size_t kOffIdx = kOffRdi + sizeof(float2) * (kTilePx / 2);    // int32
 constexpr size_t kOffRing = kOffIdx + sizeof(int32_t) * 2 * kTilePx;    // float4 [kWarps][kStages][64]: gathered X_j in flight
 constexpr size_t kOffBar = kOffRing + sizeof(float4) * kWarps * kStages * 64;          // mbarrier [kWarps][3]
 constexpr size_t kAccSmem = kOffBar + sizeof(uint64_t) * 3 * kWarps;
-constexpr int kAccCtasPerSm = 12 / kWarps;     // 12 warps per SM: bounded by registers (<= 168) and shared memory (18 KB per warp)
+#ifndef SIM3BA_ACC_WARPS_PER_SM
+#define SIM3BA_ACC_WARPS_PER_SM 12
+#endif
+constexpr int kAccCtasPerSm = SIM3BA_ACC_WARPS_PER_SM / kWarps;     // 12 warps per SM: bounded by registers (<= 168) and shared memory (18 KB per warp)
 static_assert(kAccCtasPerSm * (kAccSmem + 1024) <= 227 * 1024, "kAccCtasPerSm CTAs per SM");
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }

@@ -19,348 +19,11 @@
 //   back     L^T tau = y block by block, last to first, over the row lists.
 // Grid-wide barriers are a monotonically increasing global counter (all CTAs are co-resident: the
 // kernel is launched with cudaLaunchCooperativeKernel, with no more CTAs than the widest phase needs).
-#include <cooperative_groups.h>
-
-#include "assemble_tile.cuh"
-#include "sim3ba_internal.cuh"
+#include "solve_tile.cuh"
 
 namespace sim3ba {
 
 namespace {
-
-constexpr int NB = kNB;          // 64
-constexpr int LDD = NB + 1;      // diagonal tile / TRSM tile in shared memory (odd stride: column walks are conflict-free)
-constexpr int LDT = NB + 4;      // DMMA operand tiles (LDT % 16 == 4: fragment loads are conflict-free)
-constexpr int kSolveThreads = 256;
-
-struct SolveArgs {
-  AsmArgs as;
-  double* L; int npad, n, nb;
-  const int32_t *col_ptr, *col_rows, *row_ptr, *row_cols, *tiles; int n_tiles;
-  double *rhs, *ysol, *Dinv, *tau;
-  double eps0; int max_attempts;
-  int32_t* status;               // [0] failure flag of the running attempt, [1] attempts used, [2] ok
-  double* eps_used;
-  unsigned int* bar;
-};
-
-struct Smem {
-  double D[NB * LDD];            // diagonal tile L_kk
-  double A[(NB + 1) * LDT];      // TRSM tile + right-hand-side row (stride LDD) / DMMA operand A (stride LDT)
-  double B[NB * LDT];            // DMMA operand B
-  double y[NB];
-  double dinv[NB];               // 1 / diag(L_kk)
-  double red[256];
-  int flag;
-};
-
-__device__ __forceinline__ unsigned int ld_acquire(const unsigned int* p) {
-  unsigned int v;
-  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-
-__device__ __forceinline__ int ld_flag(const int32_t* p) {
-  int v;
-  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-
-__device__ __forceinline__ void grid_barrier(unsigned int* bar, unsigned int G, unsigned int& gen) {
-  __syncthreads();
-  gen += 1;
-  if (G > 1 && threadIdx.x == 0) {
-    __threadfence();
-    atomicAdd(bar, 1u);
-    const unsigned int target = gen * G;
-    while (ld_acquire(bar) < target) { }
-    __threadfence();
-  }
-  __syncthreads();
-}
-
-__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-
-// ---- rank-8 update shared by POTRF and TRSM -----------------------------------------------------
-// C[r][t0 + j] -= sum_{s<8} C[r][c0 + s] * D[t0 + j][c0 + s]   for the row set of this call, t0 = c0 + 8.
-// Each thread owns a strided 4x4 block: rows r0 + rstep*ii, columns t0 + bj + nblk*jj.
-__device__ __forceinline__ void rank8_block(double* C, int ldc, const double* D, int c0, int r0,
-                                            int rstep, int nr, int bj, int nblk) {
-  const int t0 = c0 + 8;
-  double acc[4][4];
-#pragma unroll
-  for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-    for (int jj = 0; jj < 4; ++jj) acc[ii][jj] = (ii < nr) ? C[(r0 + rstep * ii) * ldc + t0 + bj + nblk * jj] : 0.0;
-#pragma unroll
-  for (int s = 0; s < 8; ++s) {
-    double lr[4], lc[4];
-#pragma unroll
-    for (int ii = 0; ii < 4; ++ii) lr[ii] = (ii < nr) ? C[(r0 + rstep * ii) * ldc + c0 + s] : 0.0;
-#pragma unroll
-    for (int jj = 0; jj < 4; ++jj) lc[jj] = D[(t0 + bj + nblk * jj) * LDD + c0 + s];
-#pragma unroll
-    for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-      for (int jj = 0; jj < 4; ++jj) acc[ii][jj] = fma(-lr[ii], lc[jj], acc[ii][jj]);
-  }
-#pragma unroll
-  for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-    for (int jj = 0; jj < 4; ++jj)
-      if (ii < nr) C[(r0 + rstep * ii) * ldc + t0 + bj + nblk * jj] = acc[ii][jj];
-}
-
-// ---- Cholesky of the 64x64 tile in sm.D (lower triangle; the upper triangle is scratch) ---------
-// Returns false (uniformly) on a pivot that is <= 0 or not finite.
-__device__ bool potrf64(Smem& sm, int tid) {
-  const int lane = tid & 31, warp = tid >> 5;
-  if (tid == 0) sm.flag = 0;
-  for (int pb = 0; pb < 8; ++pb) {
-    const int c0 = 8 * pb;
-    if (warp == 0) {   // micro-panel: rows lane and lane + 32, columns c0 .. c0 + 7, in registers
-      double a0[8], a1[8];
-#pragma unroll
-      for (int t = 0; t < 8; ++t) { a0[t] = sm.D[lane * LDD + c0 + t]; a1[t] = sm.D[(lane + 32) * LDD + c0 + t]; }
-      bool good = true;
-#pragma unroll
-      for (int s = 0; s < 8; ++s) {
-        const int R = c0 + s;
-        const double p = __shfl_sync(0xffffffffu, (R < 32) ? a0[s] : a1[s], R & 31);
-        const bool g = (p > 0.0) && (p < 1.0e300);   // false for NaN, <= 0, inf
-        good = good && g;
-        const double inv = g ? rsqrt(p) : 1.0;
-        a0[s] *= inv;
-        a1[s] *= inv;
-#pragma unroll
-        for (int t = s + 1; t < 8; ++t) {
-          const int Rt = c0 + t;
-          const double lt = __shfl_sync(0xffffffffu, (Rt < 32) ? a0[s] : a1[s], Rt & 31);
-          a0[t] = fma(-a0[s], lt, a0[t]);
-          a1[t] = fma(-a1[s], lt, a1[t]);
-        }
-        if (lane == 0) sm.dinv[R] = inv;
-      }
-#pragma unroll
-      for (int t = 0; t < 8; ++t) { sm.D[lane * LDD + c0 + t] = a0[t]; sm.D[(lane + 32) * LDD + c0 + t] = a1[t]; }
-      if (!good && lane == 0) sm.flag = 1;
-    }
-    __syncthreads();
-    const int nblk = (NB - c0 - 8) >> 2;   // 14, 12, ..., 0
-    if (tid < nblk * nblk) {
-      const int bi = tid / nblk, bj = tid - bi * nblk;
-      rank8_block(sm.D, LDD, sm.D, c0, c0 + 8 + bi, nblk, 4, bj, nblk);
-    }
-    __syncthreads();
-  }
-  return sm.flag == 0;
-}
-
-// ---- X L_kk^T = A for the tile in sm.A (stride LDD), rows 0..nrows-1 plus, if with_rhs, row NB -----
-__device__ void trsm64(Smem& sm, int nrows, bool with_rhs, int tid) {
-  const bool row_thread = (tid < nrows) || (with_rhs && tid == NB);
-  for (int pb = 0; pb < 8; ++pb) {
-    const int c0 = 8 * pb;
-    if (row_thread) {
-      double x[8];
-#pragma unroll
-      for (int t = 0; t < 8; ++t) x[t] = sm.A[tid * LDD + c0 + t];
-#pragma unroll
-      for (int s = 0; s < 8; ++s) {
-        x[s] *= sm.dinv[c0 + s];
-#pragma unroll
-        for (int t = s + 1; t < 8; ++t) x[t] = fma(-x[s], sm.D[(c0 + t) * LDD + c0 + s], x[t]);
-      }
-#pragma unroll
-      for (int t = 0; t < 8; ++t) sm.A[tid * LDD + c0 + t] = x[t];
-    }
-    __syncthreads();
-    const int nblk = (NB - c0 - 8) >> 2;
-    if (nblk > 0) {
-      if (nrows > 0 && tid < 16 * nblk) {
-        const int rg = tid / nblk, bj = tid - rg * nblk;
-        rank8_block(sm.A, LDD, sm.D, c0, rg, 16, 4, bj, nblk);
-      } else if (with_rhs && tid >= 224 && tid < 224 + nblk) {
-        rank8_block(sm.A, LDD, sm.D, c0, NB, 0, 1, tid - 224, nblk);
-      }
-    }
-    __syncthreads();
-  }
-}
-
-// ---- phase A of block column k --------------------------------------------------------------------
-__device__ void panel_phase(const SolveArgs& a, Smem& sm, int k, int G) {
-  const int tid = threadIdx.x;
-  const size_t ld = (size_t)a.npad;
-  const int cbeg = a.col_ptr[k], c = a.col_ptr[k + 1] - cbeg;
-  if (blockIdx.x != 0 && (int)blockIdx.x >= c) return;
-  double* Lkk = a.L + (size_t)k * NB * ld + (size_t)k * NB;
-  for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
-    const int r = idx >> 6, cc = idx & 63;
-    sm.D[r * LDD + cc] = __ldcg(Lkk + r * ld + cc);
-  }
-  __syncthreads();
-  if (!potrf64(sm, tid)) {
-    if (blockIdx.x == 0 && tid == 0) a.status[0] = 1;
-    return;
-  }
-  if (blockIdx.x == 0) {   // the factorised diagonal tile goes back in place (strict upper triangle zero)
-    for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
-      const int r = idx >> 6, cc = idx & 63;
-      Lkk[r * ld + cc] = (cc <= r) ? sm.D[r * LDD + cc] : 0.0;
-    }
-    if (tid < NB) a.Dinv[k * NB + tid] = sm.dinv[tid];
-  }
-  bool have_y = false;
-  int t = blockIdx.x;
-  do {
-    const bool has_tile = t < c;
-    double* Aik = nullptr;
-    int i = 0;
-    if (has_tile) {
-      i = a.col_rows[cbeg + t];
-      Aik = a.L + (size_t)i * NB * ld + (size_t)k * NB;
-      for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
-        const int r = idx >> 6, cc = idx & 63;
-        sm.A[r * LDD + cc] = __ldcg(Aik + r * ld + cc);
-      }
-    }
-    if (!have_y && tid < NB) sm.A[NB * LDD + tid] = __ldcg(a.rhs + k * NB + tid);
-    __syncthreads();
-    trsm64(sm, has_tile ? NB : 0, !have_y, tid);
-    if (!have_y) {
-      if (tid < NB) {
-        const double yv = sm.A[NB * LDD + tid];
-        sm.y[tid] = yv;
-        if (blockIdx.x == 0) a.ysol[k * NB + tid] = yv;
-      }
-      have_y = true;
-      __syncthreads();
-    }
-    if (has_tile) {
-      for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
-        const int r = idx >> 6, cc = idx & 63;
-        Aik[r * ld + cc] = sm.A[r * LDD + cc];
-      }
-      // b_i -= L_ik y_k: four threads per row, 16 columns each
-      const int r = tid >> 2, g = tid & 3;
-      double dot = 0.0;
-#pragma unroll
-      for (int cc = 0; cc < 16; ++cc) dot = fma(sm.A[r * LDD + 16 * g + cc], sm.y[16 * g + cc], dot);
-      dot += __shfl_xor_sync(0xffffffffu, dot, 1);
-      dot += __shfl_xor_sync(0xffffffffu, dot, 2);
-      if (g == 0) a.rhs[i * NB + r] = __ldcg(a.rhs + i * NB + r) - dot;
-    }
-    __syncthreads();
-    t += G;
-  } while (t < c);
-}
-
-// ---- phase B of block column k: C_ij -= L_ik L_jk^T on the FP64 tensor pipe --------------------
-__device__ void update_phase(const SolveArgs& a, Smem& sm, int k, int G) {
-  const int cbeg = a.col_ptr[k], c = a.col_ptr[k + 1] - cbeg;
-  const int ntasks = c * (c + 1) / 2;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int gid = lane >> 2, tig = lane & 3;
-  const int wm = warp & 3, wn = warp >> 2;   // rows 16 wm .. +15, columns 32 wn .. +31
-  const size_t ld = (size_t)a.npad;
-  for (int t = blockIdx.x; t < ntasks; t += G) {
-    int ta = (int)((sqrt(8.0 * (double)t + 1.0) - 1.0) * 0.5);
-    while ((ta + 1) * (ta + 2) / 2 <= t) ++ta;
-    while (ta * (ta + 1) / 2 > t) --ta;
-    const int tb = t - ta * (ta + 1) / 2;
-    const int i = a.col_rows[cbeg + ta], j = a.col_rows[cbeg + tb];
-    const double* Ag = a.L + (size_t)i * NB * ld + (size_t)k * NB;
-    const double* Bg = a.L + (size_t)j * NB * ld + (size_t)k * NB;
-    for (int idx = tid; idx < NB * NB / 2; idx += kSolveThreads) {
-      const int r = idx >> 5, c2 = (idx & 31) * 2;
-      const double2 va = __ldcg(reinterpret_cast<const double2*>(Ag + r * ld + c2));
-      *reinterpret_cast<double2*>(&sm.A[r * LDT + c2]) = va;
-      if (i != j) {
-        const double2 vb = __ldcg(reinterpret_cast<const double2*>(Bg + r * ld + c2));
-        *reinterpret_cast<double2*>(&sm.B[r * LDT + c2]) = vb;
-      }
-    }
-    __syncthreads();
-    const double* Bs = (i != j) ? sm.B : sm.A;
-    double acc[2][4][2];
-#pragma unroll
-    for (int mi = 0; mi < 2; ++mi)
-#pragma unroll
-      for (int ni = 0; ni < 4; ++ni) acc[mi][ni][0] = acc[mi][ni][1] = 0.0;
-#pragma unroll 4
-    for (int kk = 0; kk < NB; kk += 4) {
-      double af[2], bf[4];
-#pragma unroll
-      for (int mi = 0; mi < 2; ++mi) af[mi] = sm.A[(16 * wm + 8 * mi + gid) * LDT + kk + tig];
-#pragma unroll
-      for (int ni = 0; ni < 4; ++ni) bf[ni] = Bs[(32 * wn + 8 * ni + gid) * LDT + kk + tig];
-#pragma unroll
-      for (int mi = 0; mi < 2; ++mi)
-#pragma unroll
-        for (int ni = 0; ni < 4; ++ni) dmma884(acc[mi][ni][0], acc[mi][ni][1], af[mi], bf[ni]);
-    }
-    double* Cg = a.L + (size_t)i * NB * ld + (size_t)j * NB;
-#pragma unroll
-    for (int mi = 0; mi < 2; ++mi)
-#pragma unroll
-      for (int ni = 0; ni < 4; ++ni) {
-        double2* p = reinterpret_cast<double2*>(Cg + (size_t)(16 * wm + 8 * mi + gid) * ld + 32 * wn + 8 * ni + 2 * tig);
-        double2 v = __ldcg(p);
-        v.x -= acc[mi][ni][0];
-        v.y -= acc[mi][ni][1];
-        *p = v;
-      }
-    __syncthreads();
-  }
-}
-
-// backward step for block kb: tau_kb = L_kk^-T y_kb (each participating CTA, redundantly), then
-// y_jb -= L[kb, jb]^T tau_kb for the non-zero tiles of row kb this CTA owns; CTA 0 stores tau_kb.
-__device__ void back_phase(const SolveArgs& a, Smem& sm, int kb, int G) {
-  const int tid = threadIdx.x;
-  const int rbeg = a.row_ptr[kb], rc = a.row_ptr[kb + 1] - rbeg;
-  if (blockIdx.x != 0 && (int)blockIdx.x >= rc) return;
-  const size_t ld = (size_t)a.npad;
-  const double* Lkk = a.L + (size_t)kb * NB * ld + (size_t)kb * NB;
-  for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
-    const int r = idx >> 6, cc = idx & 63;
-    sm.D[r * LDD + cc] = __ldcg(Lkk + r * ld + cc);
-  }
-  if (tid < NB) { sm.y[tid] = __ldcg(a.ysol + kb * NB + tid); sm.dinv[tid] = __ldcg(a.Dinv + kb * NB + tid); }
-  __syncthreads();
-  // D^T x = y, warp 0: lane owns x[lane], x[lane+32]; c from NB-1 down to 0
-  if (tid < 32) {
-    double b0 = sm.y[tid], b1 = sm.y[tid + 32];
-    for (int c = NB - 1; c >= 0; --c) {
-      const double own = (c < 32) ? b0 : b1;
-      const double xc = __shfl_sync(0xffffffffu, own, c & 31) * sm.dinv[c];
-      if (tid == (c & 31)) { if (c < 32) b0 = xc; else b1 = xc; }
-      if (tid < c) b0 -= sm.D[c * LDD + tid] * xc;
-      if (tid + 32 < c) b1 -= sm.D[c * LDD + tid + 32] * xc;
-    }
-    sm.y[tid] = b0;
-    sm.y[tid + 32] = b1;
-  }
-  __syncthreads();
-  if (blockIdx.x == 0 && tid < NB) a.tau[kb * NB + tid] = sm.y[tid];
-  // 256 threads: column c = tid & 63, a quarter of the rows each; the 4 partial sums meet in shared memory
-  const int c = tid & 63, part = tid >> 6;
-  for (int t = blockIdx.x; t < rc; t += G) {
-    const int jb = a.row_cols[rbeg + t];
-    const double* Lkj = a.L + (size_t)kb * NB * ld + (size_t)jb * NB;
-    double acc = 0.0;
-#pragma unroll 4
-    for (int rr = part * 16; rr < part * 16 + 16; ++rr) acc = fma(__ldcg(Lkj + rr * ld + c), sm.y[rr], acc);
-    __syncthreads();
-    sm.red[part * 64 + c] = acc;
-    __syncthreads();
-    if (tid < NB)
-      a.ysol[jb * NB + tid] = __ldcg(a.ysol + jb * NB + tid) - ((sm.red[tid] + sm.red[64 + tid]) + (sm.red[128 + tid] + sm.red[192 + tid]));
-  }
-}
 
 __global__ void __launch_bounds__(kSolveThreads)
 k_assemble_tiles(AsmArgs a, const int32_t* __restrict__ tiles, double eps, int32_t* __restrict__ status) {

@@ -1,0 +1,576 @@
+// Kernels 3+4 of the Sim(3) GN step, band + border variant (solver mode 2): ONE persistent cooperative
+// kernel for damped assembly (a6), block Cholesky, both triangular solves (a7) and the epsilon escalation.
+//
+//   Eq. (7)  PAPER.md:120   (H + lambda diag(H) + eps_r I) tau = -g
+//   PAPER.md:122            eps_r = eps0 * 100^r on factorisation failure, r < max_attempts, else tau = 0
+//   PAPER.md:118            "sparse Cholesky": the pose graph is temporal chains plus a few long links
+//
+// The free keyframes are split on the host (bb_plan.cu) into interior keyframes -- independent
+// SEGMENTS of a chain whose coupling stays inside a block band of kBand -- and BORDER keyframes
+// (one endpoint of every long link, separator triples between segments).  With H = [[A, F^T], [F, C]]
+// (interior first):
+//   phase 0  gather the 7x7 blocks of every interior block column [D | band | border | rhs] and the dense
+//            border block C from the per-edge blocks (no atomics, fixed order), damping fused;
+//   phase 1  one CTA per segment: right-looking block Cholesky at 7x7 granularity, the block columns
+//            streaming through a shared-memory window (cp.async), the right-hand side riding along:
+//            A = L L^T, F <- F L^-T, y = L^-1 b;
+//   phase 2  one CTA per border keyframe: S = C - F F^T (its block row), b_B <- b_B - F y;
+//   phase 3  tiled FP64 Cholesky of the dense S (solve_tile.cuh) -> tau_B;
+//   phase 4  one CTA per segment: tau_A = L^-T (y - F^T tau_B) by block back-substitution.
+// A pivot <= 0 or not finite anywhere fails the attempt; the retry re-assembles with eps * 100.
+#include <stdio.h>
+
+#include "solve_tile.cuh"
+
+namespace sim3ba {
+
+namespace {
+
+constexpr int kWin = 8;            // block columns resident in shared memory per segment (needs > kBand + prefetch distance)
+constexpr int kBackRing = 8;       // [D | band] parts in flight during the back-substitution
+static_assert(kBand == 3, "the trailing update of the border blocks is written out for three band blocks");
+
+#ifdef SIM3BA_BB_STAMPS
+__device__ unsigned long long g_bb_stamps[16];
+#define BB_STAMP(i) do { if (blockIdx.x == 0 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_bb_stamps[i] = t_; } } while (0)
+#else
+#define BB_STAMP(i)
+#endif
+
+struct BBArgs {
+  const double *blocks35, *g;
+  const int32_t *kf_ptr, *kf_edge, *pair_ptr, *pair_edge;
+  double lambda;
+  int n_int, n_seg, n_bord, npadB, slot_doubles, max_len;
+  const int32_t *seg_ptr, *seg_bptr, *seg_bord, *col_kf, *col_nb, *col_band, *col_bpair, *bord_kf, *bord_sptr, *bord_seg, *bord_slot, *bb_pair;
+  const long long *col_ofs, *col_bofs;
+  double *colbuf, *seg_rhs;
+  SolveArgs B;                     // border system (dense tile plan); B.as is unused
+  double* tau;                     // [7 N] of the whole system
+  const uint8_t* fixed; int N;
+  double eps0; int max_attempts;
+  int32_t* status; double* eps_used; unsigned int* bar;
+};
+
+__device__ __forceinline__ int col_stride(int nb) { return ((1 + kBand + nb) * 49 + 7 + 1) & ~1; }
+__device__ __forceinline__ int tri77(int r, int c) { return r <= c ? r * 7 - r * (r - 1) / 2 + (c - r) : c * 7 - c * (c - 1) / 2 + (r - c); }
+
+__device__ __forceinline__ void cp16(void* dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N_>
+__device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
+
+// element (r, c) of the 7x7 block of H between two keyframes joined by pair `pair` (H_ij = -sum A_e), 0 if no pair
+__device__ __forceinline__ double pair_elem(const BBArgs& a, int pair, int r, int c) {
+  if (pair < 0) return 0.0;
+  const int idx = tri77(r, c);
+  double v = 0.0;
+  for (int q = a.pair_ptr[pair]; q < a.pair_ptr[pair + 1]; ++q) v += a.blocks35[(size_t)a.pair_edge[q] * 35 + idx];
+  return -v;
+}
+// element (r, c) of the damped diagonal block of keyframe kf (H_kk = sum over incident edges of A_e)
+__device__ __forceinline__ double diag_elem(const BBArgs& a, int kf, int r, int c, double eps) {
+  const int idx = tri77(r, c);
+  double v = 0.0;
+  for (int p = a.kf_ptr[kf]; p < a.kf_ptr[kf + 1]; ++p) v += a.blocks35[(size_t)a.kf_edge[p] * 35 + idx];
+  if (r == c) v = v * (1.0 + a.lambda) + eps;
+  return v;
+}
+
+// ---- phase 0 ---------------------------------------------------------------------------------------
+__device__ void bb_assemble(const BBArgs& a, double eps, int G) {
+  const int tid = threadIdx.x;
+  for (int c = blockIdx.x; c < a.n_int; c += G) {            // interior block columns, one CTA each
+    const int nb = a.col_nb[c];
+    const int nel = (1 + kBand + nb) * 49 + 7;
+    const int kf = a.col_kf[c];
+    double* col = a.colbuf + a.col_ofs[c];
+    const int32_t* bp = a.col_bpair + a.col_bofs[c];
+    for (int idx = tid; idx < nel; idx += kSolveThreads) {
+      const int blk = idx / 49, e = idx - blk * 49, r = e / 7, cc = e - r * 7;
+      double v;
+      if (blk == 0) v = diag_elem(a, kf, r, cc, eps);
+      else if (blk <= kBand) v = pair_elem(a, a.col_band[c * kBand + blk - 1], r, cc);
+      else if (blk < 1 + kBand + nb) v = pair_elem(a, bp[blk - 1 - kBand], r, cc);
+      else v = -a.g[7 * kf + e];                              // rhs = -g
+      col[idx] = v;
+    }
+  }
+  const int nB = a.npadB, n7 = 7 * a.n_bord;                  // dense border block C (lower tiles, full diagonal tiles)
+  for (long long idx = (long long)blockIdx.x * kSolveThreads + tid; idx < (long long)nB * nB; idx += (long long)G * kSolveThreads) {
+    const int R = (int)(idx / nB), C = (int)(idx - (long long)R * nB);
+    if (C / kNB > R / kNB) continue;
+    double v = 0.0;
+    if (R >= n7 || C >= n7) v = (R == C) ? 1.0 : 0.0;
+    else if (C <= R) {
+      const int kr = R / 7, kc = C / 7, r = R - 7 * kr, cc = C - 7 * kc;
+      v = (kr == kc) ? diag_elem(a, a.bord_kf[kr], r, cc, eps) : pair_elem(a, a.bb_pair[(size_t)kr * a.n_bord + kc], r, cc);
+    }
+    a.B.L[(size_t)R * nB + C] = v;
+    if (C == 0) a.B.rhs[R] = (R < n7) ? -a.g[7 * a.bord_kf[R / 7] + R % 7] : 0.0;
+  }
+}
+
+// ---- phase 1: block Cholesky of one segment -----------------------------------------------------------
+struct SegSmem {
+  double inv[8];        // 1 / diag(L_cc) of the column being eliminated
+  int fail;
+};
+
+__device__ void bb_segment(const BBArgs& a, double* win, double* brhs, SegSmem& ss, int s) {
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int c0 = a.seg_ptr[s], len = a.seg_ptr[s + 1] - c0;
+  const int nb = a.seg_bptr[s + 1] - a.seg_bptr[s];
+  const int stride = col_stride(nb), chunks = stride / 2;
+  const int oB = (1 + kBand) * 49, oR = oB + nb * 49;        // offsets of the border blocks and of the rhs in a column
+  auto load_col = [&](int l) {                                // global -> window slot l % kWin (all threads; caller commits)
+    if (l < len) {
+      const double* src = a.colbuf + a.col_ofs[c0 + l];
+      double* dst = win + (size_t)(l % kWin) * a.slot_doubles;
+      for (int q = tid; q < chunks; q += kSolveThreads) cp16(dst + 2 * q, src + 2 * q);
+    }
+  };
+  for (int q = tid; q < 7 * nb; q += kSolveThreads) brhs[q] = 0.0;
+  if (tid == 0) ss.fail = 0;
+#ifdef SIM3BA_BB_STAMPS
+  long long tk[6] = {0, 0, 0, 0, 0, 0}, tq = clock64(), tn_;
+#define BB_TICK(i) do { tn_ = clock64(); tk[i] += tn_ - tq; tq = tn_; } while (0)
+#else
+#define BB_TICK(i)
+#endif
+  for (int l = 0; l < kWin - 1; ++l) { load_col(l); cp_commit(); }
+  for (int l = 0; l < len; ++l) {
+    BB_TICK(5);
+    load_col(l + kWin - 1);                                   // into the slot of column l - 1 (written back, barrier passed)
+    cp_commit();
+    cp_wait<kWin - 1 - kBand>();                              // columns l .. l + kBand have landed (this thread's part)
+    __syncthreads();
+    double* col = win + (size_t)(l % kWin) * a.slot_doubles;
+    const int nbnd = min(kBand, len - 1 - l);
+    BB_TICK(0);
+    // (a) POTRF of the 7x7 diagonal block: warp 0, lane r holds row r; pivots and columns travel by shuffles
+    if (tid < 32) {
+      double v[7];
+#pragma unroll
+      for (int k = 0; k < 7; ++k) v[k] = (lane < 7) ? col[lane * 7 + k] : 0.0;
+      bool good = true;
+#pragma unroll
+      for (int p = 0; p < 7; ++p) {
+        const double piv = __shfl_sync(0xffffffffu, v[p], p);
+        const bool gd = (piv > 0.0) && (piv < 1.0e300);       // false for NaN, <= 0, inf
+        good = good && gd;
+        const double inv = gd ? rsqrt(piv) : 1.0;
+        v[p] *= inv;
+#pragma unroll
+        for (int t = p + 1; t < 7; ++t) {
+          const double lt = __shfl_sync(0xffffffffu, v[p], t);
+          v[t] = fma(-v[p], lt, v[t]);
+        }
+        if (lane == 0) ss.inv[p] = inv;
+      }
+      if (lane < 7) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) col[lane * 7 + k] = (k <= lane) ? v[k] : 0.0;
+      }
+      if (!good && lane == 0) ss.fail = 1;
+    }
+    __syncthreads();
+    if (ss.fail) break;                                       // uniform: the attempt has failed
+    BB_TICK(1);
+    // (b) TRSM: every row x of [band blocks; border blocks; rhs^T] becomes x L_cc^-T (one thread per row); seven more
+    //     threads do the same to the rows of the identity: row k of L_cc^-T, kept in the strict upper triangle of the
+    //     diagonal block (its diagonal, 1 / L_kk, is already there) for the back-substitution
+    {
+      const int nrows = 7 * (nbnd + nb) + 1;
+      if (tid < nrows) {
+        double* row = (tid < 7 * nbnd) ? col + 49 + tid * 7 : (tid < nrows - 1) ? col + oB + (tid - 7 * nbnd) * 7 : col + oR;
+        double x[7];
+#pragma unroll
+        for (int k = 0; k < 7; ++k) x[k] = row[k];
+#pragma unroll
+        for (int k = 0; k < 7; ++k) {
+#pragma unroll
+          for (int m = 0; m < k; ++m) x[k] = fma(-x[m], col[k * 7 + m], x[k]);
+          x[k] *= ss.inv[k];
+        }
+#pragma unroll
+        for (int k = 0; k < 7; ++k) row[k] = x[k];
+      } else if (tid < nrows + 7) {
+        const int j = tid - nrows;
+        double x[7];
+#pragma unroll
+        for (int k = 0; k < 7; ++k) {
+          x[k] = (k == j) ? 1.0 : 0.0;
+#pragma unroll
+          for (int m = 0; m < k; ++m) x[k] = fma(-x[m], col[k * 7 + m], x[k]);
+          x[k] *= ss.inv[k];
+        }
+#pragma unroll
+        for (int k = 0; k < 7; ++k) if (k > j) col[j * 7 + k] = x[k];
+      }
+    }
+    __syncthreads();
+    BB_TICK(2);
+    // (c) trailing update of the next nbnd block columns (all in the window) and of the border right-hand side.
+    //     The few diagonal / band blocks and the right-hand sides first, by general indexing ...
+    for (int t = 0; t < nbnd; ++t) {
+      double* tc = win + (size_t)((l + 1 + t) % kWin) * a.slot_doubles;
+      const double* Xa = col + 49 + t * 49;                   // L(l + 1 + t, l)
+      const int nblk = 1 + (nbnd - 1 - t);                    // diagonal, later band blocks
+      for (int idx = tid; idx < nblk * 49 + 7; idx += kSolveThreads) {
+        if (idx < nblk * 49) {
+          const int blk = idx / 49, e = idx - blk * 49, r = e / 7, cc = e - r * 7;
+          const double* Xr = (blk == 0) ? Xa : col + 49 + (t + blk) * 49;   // the block whose row r meets row cc of Xa
+          double* dst = (blk == 0) ? tc : tc + 49 + (blk - 1) * 49;
+          double acc = 0.0;
+#pragma unroll
+          for (int k = 0; k < 7; ++k) acc = fma(Xr[r * 7 + k], Xa[cc * 7 + k], acc);
+          dst[e] -= acc;
+        } else {
+          const int r = idx - nblk * 49;
+          double acc = 0.0;
+#pragma unroll
+          for (int k = 0; k < 7; ++k) acc = fma(Xa[r * 7 + k], col[oR + k], acc);
+          tc[oR + r] -= acc;
+        }
+      }
+    }
+    //     ... then the border blocks F(p, l + 1 + t) -= F(p, l) L(l + 1 + t, l)^T: five blocks at a time, thread = one
+    //     element (r, cc) of a block, the rows of the nbnd band blocks it meets held in registers
+    if (tid < 245 && nb > 0 && nbnd > 0) {
+      const int grp = tid / 49, e = tid - grp * 49, r = e / 7, cc = e - r * 7;
+      double xa[kBand][7];
+#pragma unroll
+      for (int t = 0; t < kBand; ++t)
+#pragma unroll
+        for (int k = 0; k < 7; ++k) xa[t][k] = (t < nbnd) ? col[49 + t * 49 + cc * 7 + k] : 0.0;
+      double* t0 = win + (size_t)((l + 1) % kWin) * a.slot_doubles + oB + e;
+      double* t1 = win + (size_t)((l + 2) % kWin) * a.slot_doubles + oB + e;
+      double* t2 = win + (size_t)((l + 3) % kWin) * a.slot_doubles + oB + e;
+      for (int p = grp; p < nb; p += 5) {
+        const double* F = col + oB + p * 49 + r * 7;
+        double f[7];
+#pragma unroll
+        for (int k = 0; k < 7; ++k) f[k] = F[k];
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+#pragma unroll
+        for (int k = 0; k < 7; ++k) { a0 = fma(f[k], xa[0][k], a0); a1 = fma(f[k], xa[1][k], a1); a2 = fma(f[k], xa[2][k], a2); }
+        t0[p * 49] -= a0;
+        if (nbnd > 1) t1[p * 49] -= a1;
+        if (nbnd > 2) t2[p * 49] -= a2;
+      }
+    }
+    for (int q = tid; q < 7 * nb; q += kSolveThreads) {       // sum_c F_c y_c, in column order
+      double acc = 0.0;
+#pragma unroll
+      for (int k = 0; k < 7; ++k) acc = fma(col[oB + q * 7 + k], col[oR + k], acc);
+      brhs[q] += acc;
+    }
+    BB_TICK(3);
+    // (d) the finished column goes back: L_cc (reciprocal pivots on its diagonal), L band, F L^-T, y
+    {
+      double* dstg = a.colbuf + a.col_ofs[c0 + l];
+      for (int q = tid; q < stride; q += kSolveThreads) {
+        double v = col[q];
+        if (q < 49 && (q % 8) == 0) v = ss.inv[q / 8];
+        dstg[q] = v;
+      }
+    }
+    __syncthreads();
+  }
+  cp_wait<0>();
+  __syncthreads();
+#ifdef SIM3BA_BB_STAMPS
+  BB_TICK(4);
+  if (blockIdx.x == 0 && tid == 0) for (int i = 0; i < 6; ++i) g_bb_stamps[8 + i] = (unsigned long long)tk[i];
+#endif
+  if (ss.fail) { if (tid == 0) a.status[0] = 1; return; }
+  double* out = a.seg_rhs + (size_t)a.seg_bptr[s] * 7;
+  for (int q = tid; q < 7 * nb; q += kSolveThreads) out[q] = brhs[q];
+  __syncthreads();
+}
+
+// ---- phase 2: block row of the Schur complement on one border keyframe ---------------------------------
+// For every segment (s, slot p) touching the keyframe: S(b, q) -= sum_c F_c(p) F_c(q)^T for the border keyframes q <= p of
+// the segment, b_B(b) -= sum_c F_c(p) y_c.  The border parts of the block columns stream through shared memory in chunks
+// of kSchurCols columns (cp.async, double-buffered); a thread owns up to kSchurOut elements of the block row.
+constexpr int kSchurCols = 4;
+constexpr int kSchurOut = (kMaxSegBorder * 49 + kSolveThreads - 1) / kSolveThreads;
+constexpr int kSchurPart = (kMaxSegBorder * 49 + 1) & ~1;   // doubles of one column's border part in the buffer
+
+__device__ void bb_schur_row(const BBArgs& a, double* buf, int b) {
+  const int tid = threadIdx.x;
+  const int nB = a.npadB;
+  const int oB = (1 + kBand) * 49;
+  for (int t = a.bord_sptr[b]; t < a.bord_sptr[b + 1]; ++t) {
+    const int s = a.bord_seg[t], p = a.bord_slot[t];
+    const int c0 = a.seg_ptr[s], len = a.seg_ptr[s + 1] - c0;
+    const int32_t* sb = a.seg_bord + a.seg_bptr[s];
+    const int nout = (p + 1) * 49, chunks16 = (nout + 1) / 2;   // 16-byte chunks of a column's blocks 0 .. p
+    int offP[kSchurOut], offQ[kSchurOut];
+    double acc[kSchurOut];
+#pragma unroll
+    for (int j = 0; j < kSchurOut; ++j) {
+      const int o = tid + j * kSolveThreads;
+      const int q = o / 49, e = o - q * 49, r = e / 7, cc = e - r * 7;
+      offP[j] = (o < nout) ? p * 49 + r * 7 : -1;
+      offQ[j] = q * 49 + cc * 7;
+      acc[j] = 0.0;
+    }
+    auto stage = [&](int ch) {                                  // columns ch * kSchurCols ... -> buffer ch & 1
+      double* dst = buf + (size_t)(ch & 1) * kSchurCols * kSchurPart;
+      for (int w = 0; w < kSchurCols; ++w) {
+        const int l = ch * kSchurCols + w;
+        if (l < len) {
+          const double* src = a.colbuf + a.col_ofs[c0 + l] + oB;
+          for (int q = tid; q < chunks16; q += kSolveThreads) cp16(dst + w * kSchurPart + 2 * q, src + 2 * q);
+        }
+      }
+    };
+    const int nch = (len + kSchurCols - 1) / kSchurCols;
+    stage(0);
+    cp_commit();
+    for (int ch = 0; ch < nch; ++ch) {
+      if (ch + 1 < nch) stage(ch + 1);
+      cp_commit();
+      cp_wait<1>();
+      __syncthreads();
+      const double* src = buf + (size_t)(ch & 1) * kSchurCols * kSchurPart;
+      const int ncol = min(kSchurCols, len - ch * kSchurCols);
+      for (int w = 0; w < ncol; ++w) {
+        const double* F = src + w * kSchurPart;
+#pragma unroll
+        for (int j = 0; j < kSchurOut; ++j) {
+          if (offP[j] >= 0) {
+            double v = acc[j];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) v = fma(F[offP[j] + k], F[offQ[j] + k], v);
+            acc[j] = v;
+          }
+        }
+      }
+      __syncthreads();                                          // the buffer is restaged two chunks later
+    }
+#pragma unroll
+    for (int j = 0; j < kSchurOut; ++j) {
+      if (offP[j] >= 0) {
+        const int o = tid + j * kSolveThreads;
+        const int q = o / 49, e = o - q * 49, r = e / 7, cc = e - r * 7;
+        double* dst = a.B.L + (size_t)(7 * b + r) * nB + 7 * sb[q] + cc;
+        *dst = __ldcg(dst) - acc[j];
+      }
+    }
+    if (tid < 7) a.B.rhs[7 * b + tid] = __ldcg(a.B.rhs + 7 * b + tid) - __ldcg(a.seg_rhs + (size_t)(a.seg_bptr[s] + p) * 7 + tid);
+    __syncthreads();                                            // the next segment maps the blocks to other threads
+  }
+}
+
+// ---- phase 4: back-substitution of one segment ------------------------------------------------------------
+__device__ void bb_back(const BBArgs& a, double* ring, double* z, double* tb, int s) {
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int c0 = a.seg_ptr[s], len = a.seg_ptr[s + 1] - c0;
+  const int nb = a.seg_bptr[s + 1] - a.seg_bptr[s];
+  const int oB = (1 + kBand) * 49, oR = oB + nb * 49;
+  const int32_t* sb = a.seg_bord + a.seg_bptr[s];
+  for (int q = tid; q < 7 * nb; q += kSolveThreads) tb[q] = __ldcg(a.B.tau + 7 * sb[q / 7] + q % 7);
+  __syncthreads();
+  for (int q = tid; q < 7 * len; q += kSolveThreads) {        // z_c = y_c - F_c^T tau_B, all columns at once
+    const int l = q / 7, k = q - 7 * l;
+    const double* col = a.colbuf + a.col_ofs[c0 + l];
+    double acc = __ldcg(col + oR + k);
+    for (int pr = 0; pr < 7 * nb; ++pr) acc = fma(-__ldcg(col + oB + pr * 7 + k), tb[pr], acc);
+    z[q] = acc;
+  }
+  __syncthreads();
+  if (tid < 32) {                                             // the chain itself: one warp, lane k owns component k
+    constexpr int part = (1 + kBand) * 49;                    // [D | band] doubles of a column (even: 16-byte chunks)
+    auto load = [&](int l) {
+      if (l >= 0) {
+        const double* src = a.colbuf + a.col_ofs[c0 + l];
+        double* dst = ring + (size_t)(l % kBackRing) * part;
+        for (int q = lane; q < part / 2; q += 32) cp16(dst + 2 * q, src + 2 * q);
+      }
+    };
+    for (int l = len - 1; l > len - kBackRing; --l) { load(l); cp_commit(); }
+    for (int l = len - 1; l >= 0; --l) {
+      load(l - kBackRing + 1);
+      cp_commit();
+      cp_wait<kBackRing - 1>();
+      __syncwarp();
+      const double* col = ring + (size_t)(l % kBackRing) * part;
+      const int nbnd = min(kBand, len - 1 - l);
+      // s = z_l - sum_t L(l+1+t, l)^T tau_{l+1+t}: lane 8 t + k takes band block t, component k
+      const int t = lane >> 3, k = lane & 7;
+      double part_sum = 0.0;
+      if (t < nbnd && k < 7) {
+        const double* X = col + 49 + t * 49;
+        const double* tn = z + 7 * (l + 1 + t);               // tau of column l + 1 + t (already final)
+#pragma unroll
+        for (int r = 0; r < 7; ++r) part_sum = fma(X[r * 7 + k], tn[r], part_sum);
+      }
+      const double p1 = __shfl_down_sync(0xffffffffu, part_sum, 8), p2 = __shfl_down_sync(0xffffffffu, part_sum, 16);
+      double sk = (lane < 7) ? z[7 * l + lane] - ((part_sum + p1) + p2) : 0.0;
+      // x = L_cc^-T s: row k of L_cc^-T sits in row k of the diagonal block, columns k .. 6
+      double xk = 0.0;
+#pragma unroll
+      for (int m = 0; m < 7; ++m) {
+        const double sm_ = __shfl_sync(0xffffffffu, sk, m);
+        if (lane < 7 && m >= lane) xk = fma(col[lane * 7 + m], sm_, xk);
+      }
+      sk = xk;
+      __syncwarp();
+      if (lane < 7) {
+        z[7 * l + lane] = sk;
+        a.tau[7 * a.col_kf[c0 + l] + lane] = sk;
+      }
+      __syncwarp();
+    }
+    cp_wait<0>();
+  }
+  __syncthreads();
+}
+
+__global__ void __launch_bounds__(kSolveThreads, 1)
+k_solve_bb(BBArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Smem& sm = *reinterpret_cast<Smem*>(smem_raw);              // phase 3 view
+  double* win = reinterpret_cast<double*>(smem_raw);          // phase 1 / 4 view
+  const int G = gridDim.x, tid = threadIdx.x;
+  double* brhs = win + (size_t)kWin * a.slot_doubles;         // [7 kMaxSegBorder]
+  SegSmem& ss = *reinterpret_cast<SegSmem*>(brhs + 7 * kMaxSegBorder);
+  unsigned int gen = 0;
+  bool solved = false;
+  double eps = a.eps0;
+  const int nbB = a.npadB / kNB;
+  int r = 0;
+  for (; r < a.max_attempts; ++r, eps *= 100.0) {
+    BB_STAMP(0);
+    bb_assemble(a, eps, G);
+    if (blockIdx.x == 0 && tid == 0) a.status[0] = 0;
+    grid_barrier(a.bar, G, gen);
+    BB_STAMP(1);
+    for (int s = blockIdx.x; s < a.n_seg; s += G) bb_segment(a, win, brhs, ss, s);
+    BB_STAMP(2);
+    grid_barrier(a.bar, G, gen);
+    BB_STAMP(3);
+    bool failed = ld_flag(a.status) != 0;
+    if (!failed && nbB > 0) {
+      for (int b = blockIdx.x; b < a.n_bord; b += G) bb_schur_row(a, win, b);
+      grid_barrier(a.bar, G, gen);
+      BB_STAMP(4);
+      for (int k = 0; k < nbB; ++k) {                         // tiled Cholesky of S, forward solve riding along
+        panel_phase(a.B, sm, k, G);
+        if (a.B.col_ptr[k + 1] > a.B.col_ptr[k]) {
+          grid_barrier(a.bar, G, gen);
+          if (ld_flag(a.status) != 0) { failed = true; break; }
+          update_phase(a.B, sm, k, G);
+          grid_barrier(a.bar, G, gen);
+        }
+      }
+      if (!failed) {
+        grid_barrier(a.bar, G, gen);
+        failed = ld_flag(a.status) != 0;
+      }
+      if (!failed) {
+        for (int kb = nbB - 1; kb >= 0; --kb) {
+          back_phase(a.B, sm, kb, G);
+          if (a.B.row_ptr[kb + 1] > a.B.row_ptr[kb]) grid_barrier(a.bar, G, gen);
+        }
+      }
+    }
+    if (failed) {
+      grid_barrier(a.bar, G, gen);   // everybody has seen the flag before it is cleared again
+      continue;
+    }
+    grid_barrier(a.bar, G, gen);     // tau_B is final
+    BB_STAMP(5);
+    {
+      double* ring = win;
+      double* z = win + (size_t)kBackRing * (1 + kBand) * 49;
+      double* tb = z + 7 * a.max_len;
+      for (int s = blockIdx.x; s < a.n_seg; s += G) bb_back(a, ring, z, tb, s);
+      for (int q = blockIdx.x * kSolveThreads + tid; q < 7 * a.n_bord; q += G * kSolveThreads)
+        a.tau[7 * a.bord_kf[q / 7] + q % 7] = __ldcg(a.B.tau + q);
+    }
+    BB_STAMP(6);
+    solved = true;
+    break;
+  }
+  if (!solved) {   // all attempts failed: zero update
+    for (int idx = blockIdx.x * kSolveThreads + tid; idx < 7 * a.N; idx += G * kSolveThreads) a.tau[idx] = 0.0;
+  }
+  if (blockIdx.x == 0 && tid == 0) {
+    a.status[1] = solved ? r + 1 : a.max_attempts;
+    a.status[2] = solved ? 1 : 0;
+    a.status[0] = solved ? 0 : 1;
+    *a.eps_used = solved ? eps : nan("");
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_solve_bb(Ctx* c) {
+  BBPlan& P = c->plan_bb;
+  static int max_blocks_per_sm = -1, num_sms = 0;
+  static size_t smem_set = 0;
+  const int slot = ((1 + kBand + P.max_nb) * 49 + 7 + 1) & ~1;
+  const size_t smem_seg = ((size_t)kWin * slot + 7 * kMaxSegBorder) * sizeof(double) + sizeof(SegSmem);
+  const size_t smem_back = ((size_t)kBackRing * (1 + kBand) * 49 + 7 * (size_t)P.max_len + 7 * kMaxSegBorder) * sizeof(double);
+  const size_t smem_schur = (size_t)2 * kSchurCols * kSchurPart * sizeof(double);
+  const size_t smem = std::max({sizeof(Smem), smem_seg, smem_back, smem_schur});
+  if (max_blocks_per_sm < 0 || smem > smem_set) {
+    cudaError_t e = cudaFuncSetAttribute(k_solve_bb, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&max_blocks_per_sm, k_solve_bb, kSolveThreads, smem);
+    if (e != cudaSuccess) return e;
+    if (max_blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
+    smem_set = smem;
+  }
+  const SolvePlan& D = P.dense;
+  // enough CTAs for the widest phase: a few block columns each in the assembly, one per segment / border keyframe / tile task
+  long long want = std::max<long long>({(long long)P.n_seg, (long long)P.n_bord, (long long)D.max_upd, (long long)D.max_col,
+                                        (long long)(P.n_int + 3) / 4, 1LL});
+  const int G = (int)std::min<long long>(want, (long long)num_sms * std::min(max_blocks_per_sm, 1));
+  BBArgs a{};
+  a.blocks35 = c->blocks35; a.g = c->g; a.kf_ptr = c->kf_ptr; a.kf_edge = c->kf_edge; a.pair_ptr = c->pair_ptr; a.pair_edge = c->pair_edge;
+  a.lambda = c->prm.lm_lambda;
+  a.n_int = P.n_int; a.n_seg = P.n_seg; a.n_bord = P.n_bord; a.npadB = P.npadB; a.slot_doubles = slot; a.max_len = P.max_len;
+  a.seg_ptr = P.seg_ptr; a.seg_bptr = P.seg_bptr; a.seg_bord = P.seg_bord; a.col_kf = P.col_kf; a.col_nb = P.col_nb; a.col_band = P.col_band;
+  a.col_bpair = P.col_bpair; a.bord_kf = P.bord_kf; a.bord_sptr = P.bord_sptr; a.bord_seg = P.bord_seg; a.bord_slot = P.bord_slot;
+  a.bb_pair = P.bb_pair; a.col_ofs = reinterpret_cast<const long long*>(P.col_ofs); a.col_bofs = reinterpret_cast<const long long*>(P.col_bofs);
+  a.colbuf = P.colbuf; a.seg_rhs = P.seg_rhs;
+  SolveArgs& B = a.B;
+  B.L = P.LB; B.npad = P.npadB; B.n = 7 * P.n_bord; B.nb = P.npadB / kNB;
+  B.col_ptr = D.col_ptr; B.col_rows = D.col_rows; B.row_ptr = D.row_ptr; B.row_cols = D.row_cols; B.tiles = D.tiles; B.n_tiles = D.n_tiles;
+  B.rhs = P.rhsB; B.ysol = P.ysolB; B.Dinv = P.DinvB; B.tau = P.tauB;
+  B.eps0 = c->prm.eps0; B.max_attempts = c->prm.max_attempts; B.status = c->fail_flag; B.eps_used = c->d_eps_used; B.bar = c->bar;
+  a.tau = c->tau; a.fixed = c->fixed_mask; a.N = c->N;
+  a.eps0 = c->prm.eps0; a.max_attempts = c->prm.max_attempts; a.status = c->fail_flag; a.eps_used = c->d_eps_used; a.bar = c->bar;
+  cudaError_t e = cudaMemsetAsync(c->bar, 0, sizeof(unsigned int), c->stream);
+  if (e != cudaSuccess) return e;
+  if (c->profiling) cudaEventRecord(c->ev[4], c->stream);
+  void* args[] = {&a};
+  e = cudaLaunchCooperativeKernel((const void*)k_solve_bb, dim3(G), dim3(kSolveThreads), args, smem, c->stream);
+  c->launches += 1;
+  c->last_solve_grid = G;
+#ifdef SIM3BA_BB_STAMPS
+  {
+    cudaStreamSynchronize(c->stream);
+    unsigned long long st[16];
+    cudaMemcpyFromSymbol(st, g_bb_stamps, sizeof(st));
+    fprintf(stderr, "[bb] G=%d seg=%d bord=%d maxlen=%d | asm %.1f seg %.1f (bar %.1f) schur %.1f border-chol %.1f back %.1f us\n", G, P.n_seg, P.n_bord,
+            P.max_len, (st[1] - st[0]) * 1e-3, (st[2] - st[1]) * 1e-3, (st[3] - st[2]) * 1e-3, (st[4] - st[3]) * 1e-3, (st[5] - st[4]) * 1e-3,
+            (st[6] - st[5]) * 1e-3);
+    fprintf(stderr, "[bbseg] cycles of CTA 0 thread 0, last segment: wait %llu potrf %llu trsm %llu update %llu writeback %llu other %llu\n", st[8], st[9],
+            st[10], st[11], st[12] , st[13]);
+  }
+#endif
+  return e;
+}
+
+}  // namespace sim3ba

@@ -90,7 +90,7 @@ void free_all(Ctx* c) {
   cudaFree(c->kf_ptr); cudaFree(c->kf_edge); cudaFree(c->pair_kf); cudaFree(c->pair_ptr); cudaFree(c->pair_edge);
   cudaFree(c->partials); cudaFree(c->blocks35); cudaFree(c->edge_cost); cudaFree(c->n_valid); cudaFree(c->checksum);
   cudaFree(c->Hd); cudaFree(c->L); cudaFree(c->g); cudaFree(c->rhs); cudaFree(c->ysol); cudaFree(c->Dinv); cudaFree(c->pairhi_ptr);
-  free_plan(c->plan_sparse); free_plan(c->plan_dense);
+  free_plan(c->plan_sparse); free_plan(c->plan_dense); free_bb_plan(c->plan_bb);
   cudaFree(c->tau); cudaFree(c->total_cost); cudaFree(c->fail_flag); cudaFree(c->d_eps_used); cudaFree(c->bar);
   if (c->h_flag) cudaFreeHost(c->h_flag);
   if (c->h_scalar) cudaFreeHost(c->h_scalar);
@@ -112,7 +112,10 @@ int build_blocks(Ctx* c) {
 // a6 (damped, into L) + a7 with the escalation of PAPER.md:122: one persistent kernel, no host sync
 int solve_impl(Ctx* c) {
   mark(c, 3);
-  CU(launch_solve(c));
+  // mode 2 (default): band + border block Cholesky where the graph has that shape, else the tile-sparse plan;
+  // a caller-supplied dense system (sim3ba_load_system) always takes the dense tile plan
+  if (c->solver_mode == 2 && !c->dense_loaded && c->plan_bb.valid) CU(launch_solve_bb(c));
+  else CU(launch_solve(c));
   mark(c, 5);
   c->solved = true;
   c->status_stale = true;
@@ -260,6 +263,7 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
   {
     std::string perr;
     if (!build_plan(c, false, c->plan_sparse, perr)) return bail(SIM3BA_ERR_CUDA, perr);
+    if (!build_bb_plan(c, perr)) return bail(SIM3BA_ERR_CUDA, perr);
   }
   CUB(launch_pack(c, d_points, d_conf));
   CUB(cudaStreamSynchronize(c->stream));
@@ -372,6 +376,62 @@ int sim3ba_step_host(sim3ba_ctx* h, const double* h_in, double* h_out, double* h
   return SIM3BA_OK;
 }
 
+int sim3ba_optimize_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_edges, const float* h_points,
+                         const float* h_conf, const int32_t* h_edges, const int32_t* h_match, const int32_t* h_fixed_kf,
+                         int32_t n_fixed, const sim3ba_params* params, const double* h_poses_in, int32_t n_iters,
+                         double* h_poses_out, double* h_cost, void* cuda_stream) {
+  Ctx* c = nullptr;   // errors before / outside a context go to the thread-local create error
+  if (n_kf <= 0 || height <= 0 || width <= 0 || n_edges < 0 || n_iters < 0 || (int64_t)height * width > (1 << 28))
+    return fail(c, SIM3BA_ERR_INVALID_ARG, "non-positive or oversized dimensions");
+  if (!h_points || !h_conf || (n_edges > 0 && (!h_edges || !h_match)) || !h_poses_in || !h_poses_out)
+    return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL host pointer");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t NHW = (size_t)n_kf * height * width, EHW = (size_t)n_edges * height * width;
+  float *d_points = nullptr, *d_conf = nullptr;
+  int32_t *d_edges = nullptr, *d_match = nullptr;
+  sim3ba_ctx* h = nullptr;
+  int rc = SIM3BA_OK;
+  auto cleanup = [&]() {
+    if (h) sim3ba_destroy(h);
+    cudaFree(d_points); cudaFree(d_conf); cudaFree(d_edges); cudaFree(d_match);
+  };
+#define CUJ(call)                                                       \
+  do {                                                                  \
+    cudaError_t e_ = (call);                                            \
+    if (e_ != cudaSuccess) {                                            \
+      cleanup();                                                        \
+      return cuda_fail(nullptr, e_, #call);                             \
+    }                                                                   \
+  } while (0)
+  CUJ(dev_alloc(&d_points, 3 * NHW));
+  CUJ(dev_alloc(&d_conf, NHW));
+  CUJ(dev_alloc(&d_edges, 2 * (size_t)n_edges));
+  CUJ(dev_alloc(&d_match, EHW));
+  CUJ(cudaMemcpyAsync(d_points, h_points, 3 * NHW * sizeof(float), cudaMemcpyHostToDevice, st));
+  CUJ(cudaMemcpyAsync(d_conf, h_conf, NHW * sizeof(float), cudaMemcpyHostToDevice, st));
+  if (n_edges > 0) {
+    CUJ(cudaMemcpyAsync(d_edges, h_edges, 2 * (size_t)n_edges * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    CUJ(cudaMemcpyAsync(d_match, h_match, EHW * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  }
+  rc = sim3ba_create(&h, n_kf, height, width, n_edges, d_points, d_conf, d_edges, d_match, h_fixed_kf, n_fixed, params, cuda_stream);
+  if (rc) { h = nullptr; cleanup(); return rc; }
+  c = &h->c;
+  const size_t pose_bytes = (size_t)8 * n_kf * sizeof(double);
+  cudaError_t ce = cudaMemcpyAsync(c->poses, h_poses_in, pose_bytes, cudaMemcpyHostToDevice, st);
+  for (int it = 0; it < n_iters && ce == cudaSuccess && rc == SIM3BA_OK; ++it) {
+    rc = sim3ba_step(h);
+    if (rc == SIM3BA_OK && h_cost) ce = cudaMemcpyAsync(h_cost + it, c->total_cost, sizeof(double), cudaMemcpyDeviceToHost, st);
+  }
+  if (ce == cudaSuccess && rc == SIM3BA_OK) ce = cudaMemcpyAsync(h_poses_out, c->poses, pose_bytes, cudaMemcpyDeviceToHost, st);
+  if (ce == cudaSuccess && rc == SIM3BA_OK) ce = cudaStreamSynchronize(st);
+  if (rc != SIM3BA_OK) g_create_error = c->err;
+  cleanup();
+  if (rc != SIM3BA_OK) return rc;
+  if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "sim3ba_optimize_host");
+#undef CUJ
+  return SIM3BA_OK;
+}
+
 int sim3ba_get_edge_stats(sim3ba_ctx* h, const int32_t** nv, const uint64_t** chk, const double** cost) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
@@ -441,7 +501,7 @@ int sim3ba_load_system(sim3ba_ctx* h, const double* d_H, const double* d_g) {
 int sim3ba_set_solver_mode(sim3ba_ctx* h, int32_t mode) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
-  if (mode != 0 && mode != 1) return fail(c, SIM3BA_ERR_INVALID_ARG, "solver mode must be 0 (tile-sparse) or 1 (dense)");
+  if (mode < 0 || mode > 2) return fail(c, SIM3BA_ERR_INVALID_ARG, "solver mode must be 0 (tile-sparse), 1 (dense) or 2 (band + border)");
   c->solver_mode = mode;
   return SIM3BA_OK;
 }
@@ -460,6 +520,13 @@ int sim3ba_get_solver_info(sim3ba_ctx* h, int32_t* n_tiles, int32_t* n_tiles_den
   if (n_tiles_dense) *n_tiles_dense = nb * (nb + 1) / 2;
   if (flops) *flops = plan.flops;
   if (grid) *grid = c->last_solve_grid;
+  return SIM3BA_OK;
+}
+
+int sim3ba_get_bb_info(sim3ba_ctx* h, int32_t info[6]) {
+  if (!h || !info) return SIM3BA_ERR_INVALID_ARG;
+  const BBPlan& P = h->c.plan_bb;
+  info[0] = P.valid ? 1 : 0; info[1] = P.n_int; info[2] = P.n_seg; info[3] = P.n_bord; info[4] = P.max_len; info[5] = P.max_nb;
   return SIM3BA_OK;
 }
 

@@ -40,6 +40,44 @@ struct SolvePlan {
   bool ready = false;
 };
 
+// Band + border plan of the block (7x7) Cholesky (a7, solver mode 2), built once per graph on the host (a0).
+// Free keyframes are split into BORDER keyframes -- one endpoint of every edge longer than kBand in keyframe
+// index (loop closures, inter-agent links), plus separator triples that cap the length of a chain -- and
+// INTERIOR keyframes, which form independent SEGMENTS: runs in temporal order whose coupling stays inside a
+// block band of kBand.  A segment is eliminated sequentially by one CTA at 7x7 granularity (block column =
+// diagonal block, <= kBand band blocks, one block per border keyframe of the segment); the Schur
+// complement on the border keyframes is a small dense system for the tile Cholesky; the interior
+// update follows by back-substitution.  Same tau as the tile plans up to rounding.
+constexpr int kBand = 3;          // block band of a chain (edges (k, k+1..k+3))
+constexpr int kMaxSegBorder = 28; // border keyframes one segment may touch (else the plan is not used)
+struct BBPlan {
+  bool ready = false, valid = false;
+  int n_int = 0, n_seg = 0, n_bord = 0, max_nb = 0, max_len = 0;
+  int npadB = 0;                  // padded size of the border system (multiple of kNB), 0 if no border
+  size_t col_doubles = 0;         // doubles of all interior block columns
+  // device arrays
+  int32_t *seg_ptr = nullptr;     // [n_seg+1] interior columns of a segment (indices into col_*)
+  int32_t *seg_bptr = nullptr;    // [n_seg+1] into seg_bord
+  int32_t *seg_bord = nullptr;    // border keyframes of a segment, as border indices (ascending)
+  int32_t *col_kf = nullptr;      // [n_int] keyframe of an interior column
+  int32_t *col_nb = nullptr;      // [n_int] border keyframes of the column's segment
+  int64_t *col_ofs = nullptr;     // [n_int] offset (doubles) of the column in colbuf
+  int32_t *col_band = nullptr;    // [n_int][kBand] pair index of block (column c + 1 + a, column c), -1 if none / outside
+  int32_t *col_bpair = nullptr;   // [sum len * nb] pair index of block (border keyframe, column), -1 if none
+  int64_t *col_bofs = nullptr;    // [n_int] offset into col_bpair
+  int32_t *bord_kf = nullptr;     // [n_bord] keyframe of a border index (ascending)
+  int32_t *bord_sptr = nullptr;   // [n_bord+1] segments touching a border keyframe ...
+  int32_t *bord_seg = nullptr;    //   ... segment id
+  int32_t *bord_slot = nullptr;   //   ... position of the keyframe in the segment's border list
+  int32_t *bb_pair = nullptr;     // [n_bord][n_bord] pair index of block (border a, border b), b < a, -1 if none
+  // device work buffers
+  double *colbuf = nullptr;       // interior block columns: [D 49][band kBand*49][border nb*49][rhs 7] per column
+  double *seg_rhs = nullptr;      // [sum nb * 7] per-segment contribution sum_c F_c y_c to the border right-hand side
+  double *LB = nullptr, *rhsB = nullptr, *ysolB = nullptr, *DinvB = nullptr, *tauB = nullptr;
+  SolvePlan dense;                // dense tile plan of the border system
+  std::vector<int32_t> h_seg_ptr, h_seg_bptr;
+};
+
 struct Ctx {
   int N = 0, H = 0, W = 0, HW = 0, E = 0, n = 0, npad = 0, chunks = 0, n_pairs = 0;
   cudaStream_t stream = nullptr;
@@ -59,7 +97,8 @@ struct Ctx {
   int32_t* pairhi_ptr = nullptr;   // [N+1] first pair whose larger keyframe is >= k (pairs are sorted by (hi, lo))
   std::vector<int32_t> h_edges, h_kf_ptr, h_kf_edge, h_pair_kf, h_pair_ptr, h_pair_edge, h_pairhi_ptr;
   SolvePlan plan_sparse, plan_dense;
-  int solver_mode = 0;             // 0: tile-sparse plan of the graph, 1: dense plan (every lower tile)
+  BBPlan plan_bb;
+  int solver_mode = 2;             // 0: tile-sparse plan of the graph, 1: dense plan (every lower tile), 2: band + border (falls back to 0)
   std::vector<uint8_t> h_fixed;
   // per-edge results
   double* partials = nullptr;      // [E][chunks * warps per CTA][kPartialStride]: one record per (edge, 512-pixel slice)
@@ -101,6 +140,10 @@ cudaError_t launch_load_gradient(Ctx* c, const double* d_g);
 cudaError_t launch_solve(Ctx* c);                        // kernels 3+4: tile assembly (damped), then the persistent Cholesky / solves / eps retry
 bool build_plan(Ctx* c, bool dense, SolvePlan& plan, std::string& err);   // host symbolic factorisation + upload
 void free_plan(SolvePlan& plan);
+bool build_dense_plan(int nb, SolvePlan& plan, cudaStream_t stream, std::string& err);   // every lower tile of an nb x nb tile grid
+bool build_bb_plan(Ctx* c, std::string& err);          // host band + border analysis + upload; plan_bb.valid says whether it applies
+void free_bb_plan(BBPlan& plan);
+cudaError_t launch_solve_bb(Ctx* c);                     // kernels 3+4, band + border variant (solver mode 2)
 cudaError_t launch_retract(Ctx* c);                      // kernel 5
 
 }  // namespace sim3ba

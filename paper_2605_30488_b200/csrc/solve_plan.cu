@@ -24,32 +24,9 @@ void free_plan(SolvePlan& p) {
   p = SolvePlan();
 }
 
-bool build_plan(Ctx* c, bool dense, SolvePlan& plan, std::string& err) {
-  const int nb = c->npad / kNB;
-  std::vector<std::vector<int32_t>> col(nb);
-  if (dense) {
-    for (int k = 0; k < nb; ++k)
-      for (int i = k + 1; i < nb; ++i) col[k].push_back(i);
-  } else {
-    auto add = [&](int ti, int tj) { if (ti > tj) col[tj].push_back(ti); };
-    for (int k = 0; k < c->N; ++k) {                       // a diagonal block may straddle two tiles
-      if (c->h_fixed[k]) continue;
-      add((7 * k + 6) / kNB, (7 * k) / kNB);
-    }
-    const int P = (int)c->h_pair_kf.size() / 2;
-    for (int p = 0; p < P; ++p) {
-      const int hi = c->h_pair_kf[2 * p], lo = c->h_pair_kf[2 * p + 1];
-      if (c->h_fixed[hi] || c->h_fixed[lo]) continue;
-      for (int a = 0; a < 2; ++a)
-        for (int b = 0; b < 2; ++b) add((7 * hi + 6 * a) / kNB, (7 * lo + 6 * b) / kNB);
-    }
-    for (int k = 0; k < nb; ++k) {                         // symbolic factorisation (fill-in)
-      auto& v = col[k];
-      std::sort(v.begin(), v.end());
-      v.erase(std::unique(v.begin(), v.end()), v.end());
-      if (v.size() > 1) col[v[0]].insert(col[v[0]].end(), v.begin() + 1, v.end());
-    }
-  }
+namespace {
+// column lists (rows i > k with a non-zero tile (i, k)) -> row lists, tile list, flop count; upload
+bool finish_plan(int nb, const std::vector<std::vector<int32_t>>& col, SolvePlan& plan, cudaStream_t stream, std::string& err) {
   plan.nb = nb;
   plan.h_col_ptr.assign(nb + 1, 0);
   plan.h_col_rows.clear();
@@ -77,14 +54,52 @@ bool build_plan(Ctx* c, bool dense, SolvePlan& plan, std::string& err) {
   }
   plan.n_tiles = (int)plan.h_tiles.size() / 2;
   cudaError_t e;
-  if ((e = up(&plan.col_ptr, plan.h_col_ptr, c->stream)) != cudaSuccess || (e = up(&plan.col_rows, plan.h_col_rows, c->stream)) != cudaSuccess ||
-      (e = up(&plan.row_ptr, plan.h_row_ptr, c->stream)) != cudaSuccess || (e = up(&plan.row_cols, plan.h_row_cols, c->stream)) != cudaSuccess ||
-      (e = up(&plan.tiles, plan.h_tiles, c->stream)) != cudaSuccess || (e = cudaStreamSynchronize(c->stream)) != cudaSuccess) {
+  if ((e = up(&plan.col_ptr, plan.h_col_ptr, stream)) != cudaSuccess || (e = up(&plan.col_rows, plan.h_col_rows, stream)) != cudaSuccess ||
+      (e = up(&plan.row_ptr, plan.h_row_ptr, stream)) != cudaSuccess || (e = up(&plan.row_cols, plan.h_row_cols, stream)) != cudaSuccess ||
+      (e = up(&plan.tiles, plan.h_tiles, stream)) != cudaSuccess || (e = cudaStreamSynchronize(stream)) != cudaSuccess) {
     err = std::string("build_plan: ") + cudaGetErrorString(e);
     return false;
   }
   plan.ready = true;
   return true;
+}
+
+}  // namespace
+
+bool build_plan(Ctx* c, bool dense, SolvePlan& plan, std::string& err) {
+  const int nb = c->npad / kNB;
+  std::vector<std::vector<int32_t>> col(nb);
+  if (dense) {
+    for (int k = 0; k < nb; ++k)
+      for (int i = k + 1; i < nb; ++i) col[k].push_back(i);
+  } else {
+    auto add = [&](int ti, int tj) { if (ti > tj) col[tj].push_back(ti); };
+    for (int k = 0; k < c->N; ++k) {                       // a diagonal block may straddle two tiles
+      if (c->h_fixed[k]) continue;
+      add((7 * k + 6) / kNB, (7 * k) / kNB);
+    }
+    const int P = (int)c->h_pair_kf.size() / 2;
+    for (int p = 0; p < P; ++p) {
+      const int hi = c->h_pair_kf[2 * p], lo = c->h_pair_kf[2 * p + 1];
+      if (c->h_fixed[hi] || c->h_fixed[lo]) continue;
+      for (int a = 0; a < 2; ++a)
+        for (int b = 0; b < 2; ++b) add((7 * hi + 6 * a) / kNB, (7 * lo + 6 * b) / kNB);
+    }
+    for (int k = 0; k < nb; ++k) {                         // symbolic factorisation (fill-in)
+      auto& v = col[k];
+      std::sort(v.begin(), v.end());
+      v.erase(std::unique(v.begin(), v.end()), v.end());
+      if (v.size() > 1) col[v[0]].insert(col[v[0]].end(), v.begin() + 1, v.end());
+    }
+  }
+  return finish_plan(nb, col, plan, c->stream, err);
+}
+
+bool build_dense_plan(int nb, SolvePlan& plan, cudaStream_t stream, std::string& err) {
+  std::vector<std::vector<int32_t>> col(nb);
+  for (int k = 0; k < nb; ++k)
+    for (int i = k + 1; i < nb; ++i) col[k].push_back(i);
+  return finish_plan(nb, col, plan, stream, err);
 }
 
 }  // namespace sim3ba

@@ -129,6 +129,34 @@ def test_free_running_matches_oracle(k):
     ba.close()
 
 
+def test_optimize_host_equals_stepping_and_odd_image_size():
+    """sim3ba_optimize_host (host buffers in, poses out) runs the very same kernels as create + n x step; the image
+    size 37 x 29 has HW % 4 != 0, so the match indices take the non-TMA staging path of kernel 1."""
+    import torch
+    from paper_2605_30488_b200 import optimize_host
+    from tests.gpu_common import gpu_params
+    for spec in (reduced(2), CONFIGS[2].scaled(kf_per_agent=6, height=37, width=29, n_scene=3_000)):
+        g = make_graph(spec)
+        prm = oracle_params("config")
+        ba = make_solver(g, prm)
+        check_system(ba, g, g.poses_init, prm, tag=f"hw={g.hw}")
+        set_poses(ba, g.poses_init)
+        costs = []
+        for _ in range(3):
+            ba.step()
+            costs.append(ba.update()[3])
+        ref = ba.get_poses().cpu().numpy()
+        ba.close()
+        h_out = torch.empty((g.n_kf, 8), dtype=torch.float64).pin_memory()
+        h_cost = torch.empty((3,), dtype=torch.float64).pin_memory()
+        optimize_host(torch.from_numpy(g.points).pin_memory(), torch.from_numpy(g.conf).pin_memory(),
+                      torch.from_numpy(g.edges).contiguous(), torch.from_numpy(g.match).pin_memory(), g.fixed_kf,
+                      gpu_params(prm), g.spec.height, g.spec.width, torch.from_numpy(g.poses_init.copy()), 3, h_out, h_cost,
+                      torch.cuda.current_stream().cuda_stream)
+        assert np.array_equal(h_out.numpy(), ref)
+        assert np.array_equal(h_cost.numpy(), np.asarray(costs))
+
+
 def test_step_equals_build_solve_retract_and_is_deterministic():
     g = make_graph(reduced(2))
     prm = oracle_params("config")
@@ -201,6 +229,72 @@ def test_epsilon_escalation_and_zero_update_on_gpu():
     ba.load_system(torch.from_numpy(H).cuda(), torch.from_numpy(gg).cuda())
     ba.solve()
     assert ba.update()[1] == 6
+    ba.close()
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_solver_modes_agree(k, monkeypatch):
+    """a7 three ways -- band + border block Cholesky (mode 2, default), tile-sparse (0), dense tiles (1) -- on the same
+    built system: same attempts / eps, tau within 1e-6 of each other (different elimination orders on cond ~ 1e8
+    systems) and each within the north_star 1e-3 of the oracle.  Mode 2 also with short segments (separators)."""
+    g = make_config(1) if k == 1 else make_graph(reduced(k))
+    prm = oracle_params("config")
+    sysm = orc.build_system(g.poses_init, g.points, g.conf, g.edges, g.match, prm)
+    sol = orc.solve(sysm.H, sysm.g, g.fixed_kf, prm)
+    tau_floor = 1e-6 * np.sqrt(sol.tau.size)
+    taus = {}
+    for tag, mode, lmax in (("bb", 2, None), ("bb-short", 2, "5"), ("tile", 0, None), ("dense", 1, None)):
+        if lmax is None:
+            monkeypatch.delenv("SIM3BA_BB_LMAX", raising=False)
+        else:
+            monkeypatch.setenv("SIM3BA_BB_LMAX", lmax)
+        ba = make_solver(g, prm)
+        info = ba.bb_info()
+        assert info["valid"] == 1 and info["n_interior"] + info["n_border"] == g.n_kf - len(g.fixed_kf)
+        if lmax is not None:
+            assert info["max_segment"] <= 5
+        ba.set_solver_mode(mode)
+        set_poses(ba, g.poses_init)
+        ba.build_system()
+        ba.solve()
+        tau, attempts, eps, _ = ba.update()
+        taus[tag] = tau.cpu().numpy()
+        assert attempts == sol.attempts and eps == sol.eps_used, tag
+        assert rel(taus[tag], sol.tau, tau_floor) <= TOL_TAU, tag
+        for kf in g.fixed_kf:
+            assert np.all(taus[tag][7 * kf:7 * kf + 7] == 0.0)
+        ba.close()
+    for tag in ("bb-short", "tile", "dense"):
+        assert rel(taus[tag], taus["bb"], tau_floor) <= 1e-6, tag
+
+
+def test_band_border_zero_information_keyframe_and_all_attempts_fail():
+    """A keyframe none of whose edges has a valid match has a zero diagonal block: with eps0 > 0 its update is 0 and the
+    rest matches the oracle; with eps0 = 0 every attempt meets a zero pivot -> tau = 0, attempts = max."""
+    g = make_config(1, height=40, width=60)
+    lone = 3
+    for e in range(g.n_edges):
+        if lone in g.edges[e]:
+            g.match[e, :] = -1
+    prm = oracle_params("config")
+    ba = make_solver(g, prm)
+    assert ba.bb_info()["valid"] == 1
+    sysm, sol = check_system(ba, g, g.poses_init, prm, "lone keyframe")
+    tau = ba.update()[0].cpu().numpy()
+    assert np.all(tau[7 * lone:7 * lone + 7] == 0.0)
+    ba.close()
+    prm0 = oracle_params("config", eps0=0.0)
+    ba = make_solver(g, prm0)
+    set_poses(ba, g.poses_init)
+    ba.build_system()
+    ba.solve()
+    tau, attempts, eps, _ = ba.update()
+    ref = orc.solve(sysm.H, sysm.g, g.fixed_kf, prm0)
+    assert attempts == ref.attempts == prm0.max_attempts and np.isnan(eps)
+    assert np.all(tau.cpu().numpy() == 0.0) and np.all(ref.tau == 0.0)
+    before = ba.get_poses().cpu().numpy()
+    ba.step()
+    assert np.array_equal(before, ba.get_poses().cpu().numpy())
     ba.close()
 
 
