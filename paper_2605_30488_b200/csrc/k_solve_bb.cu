@@ -115,73 +115,84 @@ __device__ void bb_assemble(const BBArgs& a, double eps, int G) {
 
 // ---- phase 1: block Cholesky of one segment -----------------------------------------------------------
 struct SegSmem {
-  double inv[8];        // 1 / diag(L_cc) of the column being eliminated
+  double inv[2][8];     // 1 / diag(L_cc) of the column being eliminated (parity of the column) and of the next one
   int fail;
 };
 
+// 1 / sqrt(p) to full double precision from the fp32 MUFU estimate and two Newton steps (relative error 2e-7 -> 6e-14
+// -> 5e-27 before rounding); pivots outside the comfortable fp32 range take the library routine
+__device__ __forceinline__ double fast_rsqrt(double p) {
+  const float pf = (float)p;
+  if (!(pf > 1e-30f && pf < 1e30f)) return rsqrt(p);
+  float rf;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rf) : "f"(pf));
+  double y = (double)rf;
+  const double h = 0.5 * p;
+  y = y * fma(-h * y, y, 1.5);
+  y = y * fma(-h * y, y, 1.5);
+  return y;
+}
+
+// Cholesky of the 7x7 diagonal block at `col` by one warp: lane r holds row r, pivots and columns travel by shuffles.
+// Leaves L (lower triangle, zeros above) in the block and the reciprocal pivots in inv[]; returns false on a bad pivot.
+__device__ __forceinline__ bool potrf7_warp(double* col, double* inv, int lane) {
+  double v[7];
+#pragma unroll
+  for (int k = 0; k < 7; ++k) v[k] = (lane < 7) ? col[lane * 7 + k] : 0.0;
+  bool good = true;
+#pragma unroll
+  for (int p = 0; p < 7; ++p) {
+    const double piv = __shfl_sync(0xffffffffu, v[p], p);
+    const bool gd = (piv > 0.0) && (piv < 1.0e300);           // false for NaN, <= 0, inf
+    good = good && gd;
+    const double iv = gd ? fast_rsqrt(piv) : 1.0;
+    v[p] *= iv;
+#pragma unroll
+    for (int t = p + 1; t < 7; ++t) {
+      const double lt = __shfl_sync(0xffffffffu, v[p], t);
+      v[t] = fma(-v[p], lt, v[t]);
+    }
+    if (lane == 0) inv[p] = iv;
+  }
+  if (lane < 7) {
+#pragma unroll
+    for (int k = 0; k < 7; ++k) col[lane * 7 + k] = (k <= lane) ? v[k] : 0.0;
+  }
+  return good;
+}
+
+// Right-looking block Cholesky of segment s with one column of look-ahead: while warps 1..7 apply the trailing update of
+// column l and write it back, warp 0 finishes the diagonal block of column l + 1 and factorises it, so the serial chain
+// per column is  TRSM(l) -> max(update(l), POTRF(l + 1)).
 __device__ void bb_segment(const BBArgs& a, double* win, double* brhs, SegSmem& ss, int s) {
-  const int tid = threadIdx.x, lane = tid & 31;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int c0 = a.seg_ptr[s], len = a.seg_ptr[s + 1] - c0;
   const int nb = a.seg_bptr[s + 1] - a.seg_bptr[s];
   const int stride = col_stride(nb), chunks = stride / 2;
   const int oB = (1 + kBand) * 49, oR = oB + nb * 49;        // offsets of the border blocks and of the rhs in a column
+  auto slot = [&](int l) -> double* { return win + (size_t)(l % kWin) * a.slot_doubles; };
   auto load_col = [&](int l) {                                // global -> window slot l % kWin (all threads; caller commits)
     if (l < len) {
       const double* src = a.colbuf + a.col_ofs[c0 + l];
-      double* dst = win + (size_t)(l % kWin) * a.slot_doubles;
+      double* dst = slot(l);
       for (int q = tid; q < chunks; q += kSolveThreads) cp16(dst + 2 * q, src + 2 * q);
     }
   };
   for (int q = tid; q < 7 * nb; q += kSolveThreads) brhs[q] = 0.0;
   if (tid == 0) ss.fail = 0;
-#ifdef SIM3BA_BB_STAMPS
-  long long tk[6] = {0, 0, 0, 0, 0, 0}, tq = clock64(), tn_;
-#define BB_TICK(i) do { tn_ = clock64(); tk[i] += tn_ - tq; tq = tn_; } while (0)
-#else
-#define BB_TICK(i)
-#endif
   for (int l = 0; l < kWin - 1; ++l) { load_col(l); cp_commit(); }
+  cp_wait<kWin - 2>();                                        // column 0 has landed
+  __syncthreads();
+  if (warp == 0 && !potrf7_warp(slot(0), ss.inv[0], lane) && lane == 0) ss.fail = 1;
+  __syncthreads();
   for (int l = 0; l < len; ++l) {
-    BB_TICK(5);
-    load_col(l + kWin - 1);                                   // into the slot of column l - 1 (written back, barrier passed)
-    cp_commit();
-    cp_wait<kWin - 1 - kBand>();                              // columns l .. l + kBand have landed (this thread's part)
-    __syncthreads();
-    double* col = win + (size_t)(l % kWin) * a.slot_doubles;
-    const int nbnd = min(kBand, len - 1 - l);
-    BB_TICK(0);
-    // (a) POTRF of the 7x7 diagonal block: warp 0, lane r holds row r; pivots and columns travel by shuffles
-    if (tid < 32) {
-      double v[7];
-#pragma unroll
-      for (int k = 0; k < 7; ++k) v[k] = (lane < 7) ? col[lane * 7 + k] : 0.0;
-      bool good = true;
-#pragma unroll
-      for (int p = 0; p < 7; ++p) {
-        const double piv = __shfl_sync(0xffffffffu, v[p], p);
-        const bool gd = (piv > 0.0) && (piv < 1.0e300);       // false for NaN, <= 0, inf
-        good = good && gd;
-        const double inv = gd ? rsqrt(piv) : 1.0;
-        v[p] *= inv;
-#pragma unroll
-        for (int t = p + 1; t < 7; ++t) {
-          const double lt = __shfl_sync(0xffffffffu, v[p], t);
-          v[t] = fma(-v[p], lt, v[t]);
-        }
-        if (lane == 0) ss.inv[p] = inv;
-      }
-      if (lane < 7) {
-#pragma unroll
-        for (int k = 0; k < 7; ++k) col[lane * 7 + k] = (k <= lane) ? v[k] : 0.0;
-      }
-      if (!good && lane == 0) ss.fail = 1;
-    }
-    __syncthreads();
     if (ss.fail) break;                                       // uniform: the attempt has failed
-    BB_TICK(1);
+    double* col = slot(l);
+    const double* inv = ss.inv[l & 1];
+    const int nbnd = min(kBand, len - 1 - l);
     // (b) TRSM: every row x of [band blocks; border blocks; rhs^T] becomes x L_cc^-T (one thread per row); seven more
     //     threads do the same to the rows of the identity: row k of L_cc^-T, kept in the strict upper triangle of the
-    //     diagonal block (its diagonal, 1 / L_kk, is already there) for the back-substitution
+    //     diagonal block (its diagonal, 1 / L_kk, goes there at write-back) for the back-substitution
     {
       const int nrows = 7 * (nbnd + nb) + 1;
       if (tid < nrows) {
@@ -193,7 +204,7 @@ __device__ void bb_segment(const BBArgs& a, double* win, double* brhs, SegSmem& 
         for (int k = 0; k < 7; ++k) {
 #pragma unroll
           for (int m = 0; m < k; ++m) x[k] = fma(-x[m], col[k * 7 + m], x[k]);
-          x[k] *= ss.inv[k];
+          x[k] *= inv[k];
         }
 #pragma unroll
         for (int k = 0; k < 7; ++k) row[k] = x[k];
@@ -205,23 +216,43 @@ __device__ void bb_segment(const BBArgs& a, double* win, double* brhs, SegSmem& 
           x[k] = (k == j) ? 1.0 : 0.0;
 #pragma unroll
           for (int m = 0; m < k; ++m) x[k] = fma(-x[m], col[k * 7 + m], x[k]);
-          x[k] *= ss.inv[k];
+          x[k] *= inv[k];
         }
 #pragma unroll
         for (int k = 0; k < 7; ++k) if (k > j) col[j * 7 + k] = x[k];
       }
     }
+    load_col(l + kWin - 1);                                   // into the slot of column l - 1 (written back, barrier passed)
+    cp_commit();
+    cp_wait<kWin - 1 - kBand>();                              // columns l .. l + kBand have landed (this thread's part)
     __syncthreads();
-    BB_TICK(2);
-    // (c) trailing update of the next nbnd block columns (all in the window) and of the border right-hand side.
-    //     The few diagonal / band blocks and the right-hand sides first, by general indexing ...
-    for (int t = 0; t < nbnd; ++t) {
-      double* tc = win + (size_t)((l + 1 + t) % kWin) * a.slot_doubles;
-      const double* Xa = col + 49 + t * 49;                   // L(l + 1 + t, l)
-      const int nblk = 1 + (nbnd - 1 - t);                    // diagonal, later band blocks
-      for (int idx = tid; idx < nblk * 49 + 7; idx += kSolveThreads) {
-        if (idx < nblk * 49) {
-          const int blk = idx / 49, e = idx - blk * 49, r = e / 7, cc = e - r * 7;
+    // (c) trailing update of the next nbnd block columns (all in the window)
+    if (warp == 0) {
+      if (nbnd > 0) {                                         // D(l + 1) -= L(l + 1, l) L(l + 1, l)^T, then its Cholesky
+        double* tc = slot(l + 1);
+        const double* Xa = col + 49;
+        for (int e = lane; e < 49; e += 32) {
+          const int r = e / 7, cc = e - r * 7;
+          double acc = 0.0;
+#pragma unroll
+          for (int k = 0; k < 7; ++k) acc = fma(Xa[r * 7 + k], Xa[cc * 7 + k], acc);
+          tc[e] -= acc;
+        }
+        __syncwarp();
+        if (!potrf7_warp(tc, ss.inv[(l + 1) & 1], lane) && lane == 0) ss.fail = 1;
+      }
+    } else {
+      const int wt = tid - 32;                                // 0 .. 223
+      constexpr int kWT = kSolveThreads - 32;
+      // the few diagonal / band blocks (all but D(l + 1)) and the right-hand sides, by general indexing
+      const int nbt = nbnd * (nbnd + 1) / 2;
+      for (int idx = 49 + wt; idx < nbt * 49 + 7 * nbnd; idx += kWT) {
+        if (idx < nbt * 49) {
+          const int bt = idx / 49, e = idx - bt * 49, r = e / 7, cc = e - r * 7;
+          int t = 0, blk = bt;
+          while (blk >= nbnd - t) { blk -= nbnd - t; ++t; }
+          double* tc = slot(l + 1 + t);
+          const double* Xa = col + 49 + t * 49;               // L(l + 1 + t, l)
           const double* Xr = (blk == 0) ? Xa : col + 49 + (t + blk) * 49;   // the block whose row r meets row cc of Xa
           double* dst = (blk == 0) ? tc : tc + 49 + (blk - 1) * 49;
           double acc = 0.0;
@@ -229,52 +260,50 @@ __device__ void bb_segment(const BBArgs& a, double* win, double* brhs, SegSmem& 
           for (int k = 0; k < 7; ++k) acc = fma(Xr[r * 7 + k], Xa[cc * 7 + k], acc);
           dst[e] -= acc;
         } else {
-          const int r = idx - nblk * 49;
+          const int j = idx - nbt * 49, t = j / 7, r = j - 7 * t;
+          const double* Xa = col + 49 + t * 49;
           double acc = 0.0;
 #pragma unroll
           for (int k = 0; k < 7; ++k) acc = fma(Xa[r * 7 + k], col[oR + k], acc);
-          tc[oR + r] -= acc;
+          slot(l + 1 + t)[oR + r] -= acc;
         }
       }
-    }
-    //     ... then the border blocks F(p, l + 1 + t) -= F(p, l) L(l + 1 + t, l)^T: five blocks at a time, thread = one
-    //     element (r, cc) of a block, the rows of the nbnd band blocks it meets held in registers
-    if (tid < 245 && nb > 0 && nbnd > 0) {
-      const int grp = tid / 49, e = tid - grp * 49, r = e / 7, cc = e - r * 7;
-      double xa[kBand][7];
+      // the border blocks F(p, l + 1 + t) -= F(p, l) L(l + 1 + t, l)^T: four blocks at a time, thread = one element
+      // (r, cc) of a block, the rows of the nbnd band blocks it meets held in registers
+      if (wt < 196 && nb > 0 && nbnd > 0) {
+        const int grp = wt / 49, e = wt - grp * 49, r = e / 7, cc = e - r * 7;
+        double xa[kBand][7];
 #pragma unroll
-      for (int t = 0; t < kBand; ++t)
+        for (int t = 0; t < kBand; ++t)
 #pragma unroll
-        for (int k = 0; k < 7; ++k) xa[t][k] = (t < nbnd) ? col[49 + t * 49 + cc * 7 + k] : 0.0;
-      double* t0 = win + (size_t)((l + 1) % kWin) * a.slot_doubles + oB + e;
-      double* t1 = win + (size_t)((l + 2) % kWin) * a.slot_doubles + oB + e;
-      double* t2 = win + (size_t)((l + 3) % kWin) * a.slot_doubles + oB + e;
-      for (int p = grp; p < nb; p += 5) {
-        const double* F = col + oB + p * 49 + r * 7;
-        double f[7];
+          for (int k = 0; k < 7; ++k) xa[t][k] = (t < nbnd) ? col[49 + t * 49 + cc * 7 + k] : 0.0;
+        double* t0 = slot(l + 1) + oB + e;
+        double* t1 = slot(l + 2) + oB + e;
+        double* t2 = slot(l + 3) + oB + e;
+        for (int p = grp; p < nb; p += 4) {
+          const double* F = col + oB + p * 49 + r * 7;
+          double f[7];
 #pragma unroll
-        for (int k = 0; k < 7; ++k) f[k] = F[k];
-        double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+          for (int k = 0; k < 7; ++k) f[k] = F[k];
+          double a0 = 0.0, a1 = 0.0, a2 = 0.0;
 #pragma unroll
-        for (int k = 0; k < 7; ++k) { a0 = fma(f[k], xa[0][k], a0); a1 = fma(f[k], xa[1][k], a1); a2 = fma(f[k], xa[2][k], a2); }
-        t0[p * 49] -= a0;
-        if (nbnd > 1) t1[p * 49] -= a1;
-        if (nbnd > 2) t2[p * 49] -= a2;
+          for (int k = 0; k < 7; ++k) { a0 = fma(f[k], xa[0][k], a0); a1 = fma(f[k], xa[1][k], a1); a2 = fma(f[k], xa[2][k], a2); }
+          t0[p * 49] -= a0;
+          if (nbnd > 1) t1[p * 49] -= a1;
+          if (nbnd > 2) t2[p * 49] -= a2;
+        }
       }
-    }
-    for (int q = tid; q < 7 * nb; q += kSolveThreads) {       // sum_c F_c y_c, in column order
-      double acc = 0.0;
+      for (int q = wt; q < 7 * nb; q += kWT) {                // sum_c F_c y_c, in column order
+        double acc = 0.0;
 #pragma unroll
-      for (int k = 0; k < 7; ++k) acc = fma(col[oB + q * 7 + k], col[oR + k], acc);
-      brhs[q] += acc;
-    }
-    BB_TICK(3);
-    // (d) the finished column goes back: L_cc (reciprocal pivots on its diagonal), L band, F L^-T, y
-    {
+        for (int k = 0; k < 7; ++k) acc = fma(col[oB + q * 7 + k], col[oR + k], acc);
+        brhs[q] += acc;
+      }
+      // (d) the finished column goes back: L_cc (reciprocal pivots on its diagonal, L_cc^-T above it), L band, F L^-T, y
       double* dstg = a.colbuf + a.col_ofs[c0 + l];
-      for (int q = tid; q < stride; q += kSolveThreads) {
+      for (int q = wt; q < stride; q += kWT) {
         double v = col[q];
-        if (q < 49 && (q % 8) == 0) v = ss.inv[q / 8];
+        if (q < 49 && (q % 8) == 0) v = inv[q / 8];
         dstg[q] = v;
       }
     }
@@ -282,10 +311,6 @@ __device__ void bb_segment(const BBArgs& a, double* win, double* brhs, SegSmem& 
   }
   cp_wait<0>();
   __syncthreads();
-#ifdef SIM3BA_BB_STAMPS
-  BB_TICK(4);
-  if (blockIdx.x == 0 && tid == 0) for (int i = 0; i < 6; ++i) g_bb_stamps[8 + i] = (unsigned long long)tk[i];
-#endif
   if (ss.fail) { if (tid == 0) a.status[0] = 1; return; }
   double* out = a.seg_rhs + (size_t)a.seg_bptr[s] * 7;
   for (int q = tid; q < 7 * nb; q += kSolveThreads) out[q] = brhs[q];
@@ -295,31 +320,28 @@ __device__ void bb_segment(const BBArgs& a, double* win, double* brhs, SegSmem& 
 // ---- phase 2: block row of the Schur complement on one border keyframe ---------------------------------
 // For every segment (s, slot p) touching the keyframe: S(b, q) -= sum_c F_c(p) F_c(q)^T for the border keyframes q <= p of
 // the segment, b_B(b) -= sum_c F_c(p) y_c.  The border parts of the block columns stream through shared memory in chunks
-// of kSchurCols columns (cp.async, double-buffered); a thread owns up to kSchurOut elements of the block row.
+// of kSchurCols columns (cp.async, double-buffered).  A 7x7 block product F_c(p) F_c(q)^T is two DMMA.8x8x4 (rows and
+// k padded to 8 with zeros); warp w owns the blocks q = w, w + 8, ... and sums over the columns in order.
 constexpr int kSchurCols = 4;
-constexpr int kSchurOut = (kMaxSegBorder * 49 + kSolveThreads - 1) / kSolveThreads;
+constexpr int kSchurPairs = (kMaxSegBorder + 7) / 8;        // blocks per warp
 constexpr int kSchurPart = (kMaxSegBorder * 49 + 1) & ~1;   // doubles of one column's border part in the buffer
 
 __device__ void bb_schur_row(const BBArgs& a, double* buf, int b) {
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int gid = lane >> 2, tig = lane & 3;
   const int nB = a.npadB;
   const int oB = (1 + kBand) * 49;
+  const bool v0 = gid < 7, v1 = gid < 7 && tig < 3;           // fragment elements inside the 7x7 block
+  const int f0 = gid * 7 + tig, f1 = gid * 7 + 4 + tig;
   for (int t = a.bord_sptr[b]; t < a.bord_sptr[b + 1]; ++t) {
     const int s = a.bord_seg[t], p = a.bord_slot[t];
     const int c0 = a.seg_ptr[s], len = a.seg_ptr[s + 1] - c0;
     const int32_t* sb = a.seg_bord + a.seg_bptr[s];
-    const int nout = (p + 1) * 49, chunks16 = (nout + 1) / 2;   // 16-byte chunks of a column's blocks 0 .. p
-    int offP[kSchurOut], offQ[kSchurOut];
-    double acc[kSchurOut];
+    const int chunks16 = ((p + 1) * 49 + 1) / 2;              // 16-byte chunks of a column's blocks 0 .. p
+    double acc[kSchurPairs][2];
 #pragma unroll
-    for (int j = 0; j < kSchurOut; ++j) {
-      const int o = tid + j * kSolveThreads;
-      const int q = o / 49, e = o - q * 49, r = e / 7, cc = e - r * 7;
-      offP[j] = (o < nout) ? p * 49 + r * 7 : -1;
-      offQ[j] = q * 49 + cc * 7;
-      acc[j] = 0.0;
-    }
-    auto stage = [&](int ch) {                                  // columns ch * kSchurCols ... -> buffer ch & 1
+    for (int j = 0; j < kSchurPairs; ++j) acc[j][0] = acc[j][1] = 0.0;
+    auto stage = [&](int ch) {                                // columns ch * kSchurCols ... -> buffer ch & 1
       double* dst = buf + (size_t)(ch & 1) * kSchurCols * kSchurPart;
       for (int w = 0; w < kSchurCols; ++w) {
         const int l = ch * kSchurCols + w;
@@ -341,29 +363,30 @@ __device__ void bb_schur_row(const BBArgs& a, double* buf, int b) {
       const int ncol = min(kSchurCols, len - ch * kSchurCols);
       for (int w = 0; w < ncol; ++w) {
         const double* F = src + w * kSchurPart;
+        const double a0 = v0 ? F[p * 49 + f0] : 0.0, a1 = v1 ? F[p * 49 + f1] : 0.0;
 #pragma unroll
-        for (int j = 0; j < kSchurOut; ++j) {
-          if (offP[j] >= 0) {
-            double v = acc[j];
-#pragma unroll
-            for (int k = 0; k < 7; ++k) v = fma(F[offP[j] + k], F[offQ[j] + k], v);
-            acc[j] = v;
+        for (int j = 0; j < kSchurPairs; ++j) {
+          const int q = warp + 8 * j;
+          if (q <= p) {
+            const double b0 = v0 ? F[q * 49 + f0] : 0.0, b1 = v1 ? F[q * 49 + f1] : 0.0;
+            dmma884(acc[j][0], acc[j][1], a0, b0);
+            dmma884(acc[j][0], acc[j][1], a1, b1);
           }
         }
       }
-      __syncthreads();                                          // the buffer is restaged two chunks later
+      __syncthreads();                                        // the buffer is restaged two chunks later
     }
 #pragma unroll
-    for (int j = 0; j < kSchurOut; ++j) {
-      if (offP[j] >= 0) {
-        const int o = tid + j * kSolveThreads;
-        const int q = o / 49, e = o - q * 49, r = e / 7, cc = e - r * 7;
-        double* dst = a.B.L + (size_t)(7 * b + r) * nB + 7 * sb[q] + cc;
-        *dst = __ldcg(dst) - acc[j];
+    for (int j = 0; j < kSchurPairs; ++j) {
+      const int q = warp + 8 * j;
+      if (q <= p && gid < 7) {
+        double* dst = a.B.L + (size_t)(7 * b + gid) * nB + 7 * sb[q] + 2 * tig;
+        dst[0] = __ldcg(dst) - acc[j][0];
+        if (tig < 3) dst[1] = __ldcg(dst + 1) - acc[j][1];
       }
     }
     if (tid < 7) a.B.rhs[7 * b + tid] = __ldcg(a.B.rhs + 7 * b + tid) - __ldcg(a.seg_rhs + (size_t)(a.seg_bptr[s] + p) * 7 + tid);
-    __syncthreads();                                            // the next segment maps the blocks to other threads
+    __syncthreads();                                          // a later segment may map the same block to another warp
   }
 }
 
@@ -566,8 +589,6 @@ cudaError_t launch_solve_bb(Ctx* c) {
     fprintf(stderr, "[bb] G=%d seg=%d bord=%d maxlen=%d | asm %.1f seg %.1f (bar %.1f) schur %.1f border-chol %.1f back %.1f us\n", G, P.n_seg, P.n_bord,
             P.max_len, (st[1] - st[0]) * 1e-3, (st[2] - st[1]) * 1e-3, (st[3] - st[2]) * 1e-3, (st[4] - st[3]) * 1e-3, (st[5] - st[4]) * 1e-3,
             (st[6] - st[5]) * 1e-3);
-    fprintf(stderr, "[bbseg] cycles of CTA 0 thread 0, last segment: wait %llu potrf %llu trsm %llu update %llu writeback %llu other %llu\n", st[8], st[9],
-            st[10], st[11], st[12] , st[13]);
   }
 #endif
   return e;
