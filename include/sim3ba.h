@@ -119,6 +119,18 @@ int sim3ba_optimize_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_
                          const double* h_poses_in, int32_t n_iters, double* h_poses_out, double* h_cost,
                          void* cuda_stream);
 
+/* Gauge synchronisation of two map components before their first joint solve.
+ * Over the valid matches (m, n) of edge `edge` = (i, j) of the graph -- the validity rule of the GN step -- the matched
+ * points are lifted into the two world frames with the CURRENT poses, x = T_WCi X_i[m], y = T_WCj X_j[n], and
+ * (s*, R*, t*) = argmin sum |x - (s R y + t)|^2 (Eq. (3)) is found in closed form (Eq. (4), Umeyama; FP64).  With fewer
+ * than n_c_min correspondences (paper: 64) T* = T_WCi T_WCj^-1 instead.  T* is then left-multiplied onto the poses of
+ * the n_moving keyframes h_moving_kf (host array; the component of j).  moving_is_i != 0 swaps the roles: the similarity
+ * maps x onto y (fallback T_WCj T_WCi^-1) and is meant for the component of i.  Host outputs, each may be NULL:
+ * h_T [8] = T* in the pose layout (t, q_xyzw, s), *h_n_c = number of correspondences, *h_fallback = 1 if the endpoint
+ * transform was used.  Synchronises the stream.  Errors: INVALID_ARG (edge / keyframe out of range), CUDA, ALLOC. */
+int sim3ba_gauge_sync(sim3ba_ctx* ctx, int32_t edge, const int32_t* h_moving_kf, int32_t n_moving, int32_t moving_is_i,
+                      int32_t n_c_min, double* h_T, int32_t* h_n_c, int32_t* h_fallback);
+
 /* a8 only: T_i <- Exp(tau_i) T_i with the tau of the last solve. */
 int sim3ba_retract(sim3ba_ctx* ctx);
 

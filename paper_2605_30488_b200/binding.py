@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libsim3ba.so")
 
 EXPORTS = (
     "sim3ba_default_params", "sim3ba_create", "sim3ba_destroy", "sim3ba_set_params", "sim3ba_set_poses",
-    "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_host", "sim3ba_optimize_host",
+    "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_host", "sim3ba_optimize_host", "sim3ba_gauge_sync",
     "sim3ba_retract", "sim3ba_get_edge_stats", "sim3ba_get_edge_blocks", "sim3ba_get_system",
     "sim3ba_get_update", "sim3ba_get_bookkeeping", "sim3ba_load_system", "sim3ba_get_launch_count",
     "sim3ba_set_solver_mode", "sim3ba_get_solver_info", "sim3ba_get_bb_info",
@@ -62,6 +62,7 @@ def load_library() -> C.CDLL:
         "sim3ba_step": [vp],
         "sim3ba_step_host": [vp, vp, vp, vp],
         "sim3ba_optimize_host": [i32, i32, i32, i32, vp, vp, vp, vp, P(i32), i32, P(Params), vp, i32, vp, vp, vp],
+        "sim3ba_gauge_sync": [vp, i32, P(i32), i32, i32, i32, P(C.c_double), P(i32), P(i32)],
         "sim3ba_retract": [vp],
         "sim3ba_get_edge_stats": [vp, P(vp), P(vp), P(vp)],
         "sim3ba_get_edge_blocks": [vp, P(vp)],
@@ -190,6 +191,15 @@ class Sim3BA:
 
     def step(self):
         self._check(self.lib.sim3ba_step(self._h))
+
+    def gauge_sync(self, edge: int, moving_kf: Sequence[int], moving_is_i: bool = False, n_c_min: int = 64):
+        """sim3ba_gauge_sync on the current poses; returns (T* as an 8-vector pose, N_c, fallback used)."""
+        mk = (C.c_int32 * max(1, len(moving_kf)))(*[int(k) for k in moving_kf])
+        T = (C.c_double * 8)()
+        nc, fb = C.c_int32(), C.c_int32()
+        self._check(self.lib.sim3ba_gauge_sync(self._h, int(edge), mk, len(moving_kf), int(bool(moving_is_i)), int(n_c_min), T,
+                                               C.byref(nc), C.byref(fb)))
+        return np.array(list(T)), nc.value, bool(fb.value)
 
     def retract(self):
         self._check(self.lib.sim3ba_retract(self._h))

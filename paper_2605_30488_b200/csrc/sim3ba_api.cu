@@ -432,6 +432,36 @@ int sim3ba_optimize_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_
   return SIM3BA_OK;
 }
 
+int sim3ba_gauge_sync(sim3ba_ctx* h, int32_t edge, const int32_t* h_moving_kf, int32_t n_moving, int32_t moving_is_i,
+                      int32_t n_c_min, double* h_T, int32_t* h_n_c, int32_t* h_fallback) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (edge < 0 || edge >= c->E) return fail(c, SIM3BA_ERR_INVALID_ARG, "edge index out of range");
+  if (n_moving < 0 || (n_moving > 0 && !h_moving_kf) || n_c_min < 1) return fail(c, SIM3BA_ERR_INVALID_ARG, "bad moving list or n_c_min");
+  for (int k = 0; k < n_moving; ++k)
+    if (h_moving_kf[k] < 0 || h_moving_kf[k] >= c->N) return fail(c, SIM3BA_ERR_INVALID_ARG, "moving keyframe out of range");
+  const int grid = gauge_sync_grid(c->HW);
+  double* d_work = nullptr;
+  int32_t* d_moving = nullptr;
+  CU(dev_alloc(&d_work, (size_t)gauge_sync_work_doubles(grid)));
+  cudaError_t e = dev_alloc(&d_moving, (size_t)n_moving);
+  if (e == cudaSuccess && n_moving > 0)
+    e = cudaMemcpyAsync(d_moving, h_moving_kf, (size_t)n_moving * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess) e = launch_gauge_sync(c, edge, d_moving, n_moving, moving_is_i != 0, n_c_min, d_work, grid);
+  double res[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(res, d_work + (size_t)gauge_sync_work_doubles(grid) - 10, sizeof(res), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // also keeps h_moving_kf / the temporaries alive long enough
+  cudaFree(d_work);
+  cudaFree(d_moving);
+  if (e != cudaSuccess) return cuda_fail(c, e, "sim3ba_gauge_sync");
+  if (h_T) memcpy(h_T, res, 8 * sizeof(double));
+  if (h_n_c) *h_n_c = (int32_t)res[8];
+  if (h_fallback) *h_fallback = (int32_t)res[9];
+  c->built = false; c->solved = false;   // the poses changed
+  return SIM3BA_OK;
+}
+
 int sim3ba_get_edge_stats(sim3ba_ctx* h, const int32_t** nv, const uint64_t** chk, const double** cost) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;

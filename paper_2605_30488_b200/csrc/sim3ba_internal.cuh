@@ -145,5 +145,9 @@ bool build_bb_plan(Ctx* c, std::string& err);          // host band + border ana
 void free_bb_plan(BBPlan& plan);
 cudaError_t launch_solve_bb(Ctx* c);                     // kernels 3+4, band + border variant (solver mode 2)
 cudaError_t launch_retract(Ctx* c);                      // kernel 5
+// gauge synchronisation (NEXT-2): moments of edge e -> T* (Umeyama / endpoint fallback) -> applied to the moving keyframes
+cudaError_t launch_gauge_sync(Ctx* c, int e, const int32_t* d_moving, int n_moving, int moving_is_i, int n_c_min, double* d_work, int grid);
+int gauge_sync_grid(int HW);
+int gauge_sync_work_doubles(int grid);
 
 }  // namespace sim3ba
