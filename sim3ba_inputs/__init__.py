@@ -5,4 +5,5 @@ pixel-match maps shaped like the five workloads of BASELINE.json (DESIGN.md "Inp
 contains none of the method's arithmetic (no residual, Jacobian, normal equations, Sim(3) Exp/Log,
 solve) and imports neither ``oracle/`` nor the CUDA package.
 """
-from .graphs import CONFIGS, Graph, GraphSpec, make_graph, make_config, PRESETS  # noqa: F401
+from .graphs import (CONFIGS, DepthInputs, Graph, GraphSpec, PRESETS, clean_variant, make_config, make_depth_inputs,  # noqa: F401
+                     make_graph)

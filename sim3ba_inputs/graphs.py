@@ -386,6 +386,52 @@ def make_config(k: int, **scaled) -> Graph:
     return make_graph(spec)
 
 
+@dataclass
+class DepthInputs:
+    """Inputs of the segment-level structure refinement: labels, 4-adjacent pairs, Delta_gh."""
+    labels: np.ndarray        # [N, HW] int32, segment label of a pixel inside its keyframe, < 0 = excluded
+    n_seg: int                # segments per keyframe (segment id = k * n_seg + label)
+    pairs: np.ndarray         # [P, 2] int32, unordered 4-adjacent segment pairs (g, h) of every keyframe, as segment ids
+    delta: np.ndarray         # [P] float64, reference log-range difference averaged at the shared boundary
+    anchor_kf: np.ndarray     # keyframes whose segments stay fixed
+
+
+def make_depth_inputs(g: Graph, grid=None, drop_frac: float = 0.02) -> DepthInputs:
+    """Stands in for the SLIC segmentation of PAPER.md:126: a rows x cols grid of rectangular segments per keyframe (config
+    5: 4 x 8 = 32), a seeded fraction of pixels excluded (label -1, "low confidence"), the 4-adjacent pairs of the grid and
+    Delta_gh = mean over the pixel pairs straddling the shared boundary of log|X_p| - log|X_p'| (p in g, p' in h)."""
+    r, c = grid if grid is not None else (g.spec.n_segments if g.spec.n_segments[0] > 0 else (4, 8))
+    H, W = g.spec.height, g.spec.width
+    rr = (np.arange(H) * r // H)[:, None]
+    cc = (np.arange(W) * c // W)[None, :]
+    lab2 = (rr * c + cc).astype(np.int32)                                # [H, W]
+    labels = np.repeat(lab2.reshape(1, -1), g.n_kf, axis=0).copy()
+    for k in range(g.n_kf):
+        rng = _rng(g.spec.seed, 9, k)
+        labels[k, rng.random(H * W) < drop_frac] = -1
+    logd = np.log(np.maximum(np.linalg.norm(g.points.astype(np.float64), axis=2), 1e-12)).reshape(g.n_kf, H, W)
+    pairs, delta = [], []
+    for k in range(g.n_kf):
+        for a in range(r * c):
+            ar, ac = divmod(a, c)
+            for b in ((ar, ac + 1), (ar + 1, ac)):
+                if b[0] >= r or b[1] >= c:
+                    continue
+                bl = b[0] * c + b[1]
+                if b[1] == ac + 1:      # vertical boundary: pixel columns x, x + 1 with labels a, bl
+                    rows = np.flatnonzero(rr[:, 0] == ar)
+                    x = int(np.flatnonzero(cc[0, :] == ac)[-1])
+                    d = logd[k, rows, x] - logd[k, rows, x + 1]
+                else:                   # horizontal boundary: pixel rows y, y + 1
+                    y = int(np.flatnonzero(rr[:, 0] == ar)[-1])
+                    cols = np.flatnonzero(cc[0, :] == ac)
+                    d = logd[k, y, cols] - logd[k, y + 1, cols]
+                pairs.append((k * r * c + a, k * r * c + bl))
+                delta.append(float(np.mean(d)))
+    return DepthInputs(labels=labels, n_seg=r * c, pairs=np.asarray(pairs, dtype=np.int32).reshape(-1, 2),
+                       delta=np.asarray(delta, dtype=np.float64), anchor_kf=g.fixed_kf.copy())
+
+
 def clean_variant(spec: GraphSpec) -> GraphSpec:
     """Noise-free, outlier-free variant (pins: zero residual/gradient at ground truth)."""
     return replace(spec, sigma_n=0.0, p_out=0.0)
