@@ -131,6 +131,37 @@ int sim3ba_optimize_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_
 int sim3ba_gauge_sync(sim3ba_ctx* ctx, int32_t edge, const int32_t* h_moving_kf, int32_t n_moving, int32_t moving_is_i,
                       int32_t n_c_min, double* h_T, int32_t* h_n_c, int32_t* h_fallback);
 
+/* ---- Segment-level structure refinement with the poses held fixed (Eq. (8)-(10); SURVEY 8(f)
+ * NEXT-1; BASELINE config 5 "pose-depth alternation").  One log-scale eta_g per segment g of a keyframe:
+ * X(eta_g) = exp(eta_g) X_init (Eq. (8)); data term Eq. (9) over the graph's valid matches whose two pixels carry a
+ * label, 3-D point residual sqrt(q) [T_ij X_j(eta) - X_i(eta)] / sigma_point with per-component Huber; boundary term
+ * ((eta_g - eta_h) + Delta_gh)^2 over the given pairs and prior eta_g^2 (Eq. (10), conventions D1-D5 of DESIGN.md
+ * section 10); per iteration the independent steps Delta eta_g = -g_g / ((1 + lambda_lm) H_gg) with the Jacobi diagonal
+ * H_gg, clipped to eta_max; segments of the anchor keyframes stay fixed. ---- */
+typedef struct {
+  float  sigma_point;      /* paper 0.05 */
+  float  huber_k;          /* kappa on the whitened residual; not restated for Eq. (9): 1.345 */
+  double lambda_smooth;    /* paper 1 */
+  double lambda_prior;     /* paper 1 (> 0) */
+  double lambda_lm;        /* paper 0.05 */
+  double eta_max;          /* paper 0.5 */
+} sim3ba_depth_params;
+int sim3ba_depth_default_params(sim3ba_depth_params* p);
+/* n_iters iterations at the context's CURRENT poses on its packed pointmaps.  d_labels [N][HW] int32 DEVICE: label of a
+ * pixel inside its keyframe, 0 <= label < n_seg <= 64, < 0 = excluded pixel; segment id = keyframe * n_seg + label.
+ * h_pairs [n_pairs][2] HOST segment ids (g, h) of the 4-adjacent pairs, h_delta [n_pairs] HOST Delta_gh,
+ * h_anchor_kf HOST list of keyframes whose segments stay fixed.  d_eta [N * n_seg] double DEVICE, in/out (caller
+ * owned; start from zeros for eta = 0).  h_cost HOST [n_iters] or NULL: the objective at the start of each iteration.
+ * Synchronises the stream.  Errors: INVALID_ARG, CUDA, ALLOC. */
+int sim3ba_depth_refine(sim3ba_ctx* ctx, const int32_t* d_labels, int32_t n_seg, const int32_t* h_pairs, const double* h_delta,
+                        int32_t n_pairs, const int32_t* h_anchor_kf, int32_t n_anchor, const sim3ba_depth_params* p,
+                        int32_t n_iters, double* d_eta, double* h_cost);
+/* The other half of the alternation: re-packs the context's pointmaps from the caller's pristine d_points [N][HW][3],
+ * d_conf [N][HW] (as in sim3ba_create) with every labelled pixel scaled by exp(eta) of its segment, so that the next
+ * sim3ba_step sees the refined structure.  Asynchronous on the context's stream. */
+int sim3ba_apply_depth(sim3ba_ctx* ctx, const float* d_points, const float* d_conf, const int32_t* d_labels, int32_t n_seg,
+                       const double* d_eta);
+
 /* a8 only: T_i <- Exp(tau_i) T_i with the tau of the last solve. */
 int sim3ba_retract(sim3ba_ctx* ctx);
 

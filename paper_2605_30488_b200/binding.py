@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libsim3ba.so")
 
 EXPORTS = (
     "sim3ba_default_params", "sim3ba_create", "sim3ba_destroy", "sim3ba_set_params", "sim3ba_set_poses",
-    "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_host", "sim3ba_optimize_host", "sim3ba_gauge_sync",
+    "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_host", "sim3ba_optimize_host", "sim3ba_gauge_sync", "sim3ba_depth_default_params", "sim3ba_depth_refine", "sim3ba_apply_depth",
     "sim3ba_retract", "sim3ba_get_edge_stats", "sim3ba_get_edge_blocks", "sim3ba_get_system",
     "sim3ba_get_update", "sim3ba_get_bookkeeping", "sim3ba_load_system", "sim3ba_get_launch_count",
     "sim3ba_set_solver_mode", "sim3ba_get_solver_info", "sim3ba_get_bb_info",
@@ -28,6 +28,11 @@ class Params(C.Structure):
     _fields_ = [("sigma_ray", C.c_float), ("sigma_dist", C.c_float), ("huber_k", C.c_float),
                 ("conf_min", C.c_float), ("lm_lambda", C.c_double), ("eps0", C.c_double),
                 ("max_attempts", C.c_int32), ("reserved", C.c_int32)]
+
+
+class DepthParams(C.Structure):
+    _fields_ = [("sigma_point", C.c_float), ("huber_k", C.c_float), ("lambda_smooth", C.c_double),
+                ("lambda_prior", C.c_double), ("lambda_lm", C.c_double), ("eta_max", C.c_double)]
 
 
 class Sim3BAError(RuntimeError):
@@ -63,6 +68,9 @@ def load_library() -> C.CDLL:
         "sim3ba_step_host": [vp, vp, vp, vp],
         "sim3ba_optimize_host": [i32, i32, i32, i32, vp, vp, vp, vp, P(i32), i32, P(Params), vp, i32, vp, vp, vp],
         "sim3ba_gauge_sync": [vp, i32, P(i32), i32, i32, i32, P(C.c_double), P(i32), P(i32)],
+        "sim3ba_depth_default_params": [P(DepthParams)],
+        "sim3ba_depth_refine": [vp, vp, i32, P(i32), P(C.c_double), i32, P(i32), i32, P(DepthParams), i32, vp, P(C.c_double)],
+        "sim3ba_apply_depth": [vp, vp, vp, vp, i32, vp],
         "sim3ba_retract": [vp],
         "sim3ba_get_edge_stats": [vp, P(vp), P(vp), P(vp)],
         "sim3ba_get_edge_blocks": [vp, P(vp)],
@@ -200,6 +208,30 @@ class Sim3BA:
         self._check(self.lib.sim3ba_gauge_sync(self._h, int(edge), mk, len(moving_kf), int(bool(moving_is_i)), int(n_c_min), T,
                                                C.byref(nc), C.byref(fb)))
         return np.array(list(T)), nc.value, bool(fb.value)
+
+    def depth_refine(self, labels, n_seg: int, pairs: np.ndarray, delta: np.ndarray, anchor_kf: Sequence[int], eta, n_iters: int = 10,
+                     params: Optional[DepthParams] = None):
+        """sim3ba_depth_refine: labels int32 [N,HW] and eta float64 [N*n_seg] are CUDA tensors (eta updated in place);
+        pairs [P,2] int32 / delta [P] float64 are NumPy host arrays.  Returns the objective at the start of each iteration."""
+        t = self._torch
+        assert labels.is_cuda and labels.dtype == t.int32 and labels.is_contiguous() and tuple(labels.shape) == (self.N, self.HW)
+        assert eta.is_cuda and eta.dtype == t.float64 and eta.is_contiguous() and eta.numel() == self.N * n_seg
+        prm = params
+        if prm is None:
+            prm = DepthParams()
+            self._check(self.lib.sim3ba_depth_default_params(C.byref(prm)))
+        pr = np.ascontiguousarray(pairs, dtype=np.int32).reshape(-1, 2)
+        dl = np.ascontiguousarray(delta, dtype=np.float64).reshape(-1)
+        ak = (C.c_int32 * max(1, len(anchor_kf)))(*[int(k) for k in anchor_kf])
+        cost = (C.c_double * max(1, n_iters))()
+        self._check(self.lib.sim3ba_depth_refine(self._h, labels.data_ptr(), int(n_seg), pr.ctypes.data_as(C.POINTER(C.c_int32)),
+                                                 dl.ctypes.data_as(C.POINTER(C.c_double)), pr.shape[0], ak, len(anchor_kf), C.byref(prm),
+                                                 int(n_iters), eta.data_ptr(), cost))
+        return np.array(list(cost)[:n_iters])
+
+    def apply_depth(self, points, conf, labels, n_seg: int, eta):
+        """sim3ba_apply_depth: re-pack the pointmaps scaled by exp(eta) of each pixel's segment."""
+        self._check(self.lib.sim3ba_apply_depth(self._h, points.data_ptr(), conf.data_ptr(), labels.data_ptr(), int(n_seg), eta.data_ptr()))
 
     def retract(self):
         self._check(self.lib.sim3ba_retract(self._h))

@@ -462,6 +462,42 @@ int sim3ba_gauge_sync(sim3ba_ctx* h, int32_t edge, const int32_t* h_moving_kf, i
   return SIM3BA_OK;
 }
 
+int sim3ba_depth_default_params(sim3ba_depth_params* p) {
+  if (!p) return SIM3BA_ERR_INVALID_ARG;
+  p->sigma_point = 0.05f; p->huber_k = 1.345f; p->lambda_smooth = 1.0; p->lambda_prior = 1.0; p->lambda_lm = 0.05; p->eta_max = 0.5;
+  return SIM3BA_OK;
+}
+
+int sim3ba_depth_refine(sim3ba_ctx* h, const int32_t* d_labels, int32_t n_seg, const int32_t* h_pairs, const double* h_delta,
+                        int32_t n_pairs, const int32_t* h_anchor_kf, int32_t n_anchor, const sim3ba_depth_params* p, int32_t n_iters,
+                        double* d_eta, double* h_cost) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (!d_labels || !d_eta || !p || n_seg < 1 || n_seg > depth_max_segments() || n_iters < 0 || n_pairs < 0 || n_anchor < 0 ||
+      (n_pairs > 0 && (!h_pairs || !h_delta)) || (n_anchor > 0 && !h_anchor_kf))
+    return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL pointer, or n_seg outside 1..64, or a negative count");
+  if (!(p->sigma_point > 0.f) || !(p->huber_k > 0.f) || p->lambda_smooth < 0.0 || !(p->lambda_prior > 0.0) || p->lambda_lm < 0.0 ||
+      !(p->eta_max > 0.0))
+    return fail(c, SIM3BA_ERR_INVALID_ARG, "invalid depth params (sigma, kappa, lambda_prior, eta_max > 0; lambda_smooth, lambda_lm >= 0)");
+  const int n_total = c->N * n_seg;
+  for (int q = 0; q < 2 * n_pairs; ++q)
+    if (h_pairs[q] < 0 || h_pairs[q] >= n_total) return fail(c, SIM3BA_ERR_INVALID_ARG, "segment id of a boundary pair out of range");
+  for (int k = 0; k < n_anchor; ++k)
+    if (h_anchor_kf[k] < 0 || h_anchor_kf[k] >= c->N) return fail(c, SIM3BA_ERR_INVALID_ARG, "anchor keyframe out of range");
+  CU(run_depth_refine(c, d_labels, n_seg, h_pairs, h_delta, n_pairs, h_anchor_kf, n_anchor, *p, n_iters, d_eta, h_cost));
+  return SIM3BA_OK;
+}
+
+int sim3ba_apply_depth(sim3ba_ctx* h, const float* d_points, const float* d_conf, const int32_t* d_labels, int32_t n_seg,
+                       const double* d_eta) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  if (!d_points || !d_conf || !d_labels || !d_eta || n_seg < 1) return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL pointer or n_seg < 1");
+  CU(launch_depth_apply(c, d_points, d_conf, d_labels, n_seg, d_eta));
+  c->built = false; c->solved = false;   // the pointmaps changed
+  return SIM3BA_OK;
+}
+
 int sim3ba_get_edge_stats(sim3ba_ctx* h, const int32_t** nv, const uint64_t** chk, const double** cost) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;

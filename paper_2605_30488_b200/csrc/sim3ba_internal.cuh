@@ -149,5 +149,10 @@ cudaError_t launch_retract(Ctx* c);                      // kernel 5
 cudaError_t launch_gauge_sync(Ctx* c, int e, const int32_t* d_moving, int n_moving, int moving_is_i, int n_c_min, double* d_work, int grid);
 int gauge_sync_grid(int HW);
 int gauge_sync_work_doubles(int grid);
+// segment-level depth refinement with poses fixed (NEXT-1)
+cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const int32_t* h_pairs, const double* h_delta, int n_pairs,
+                             const int32_t* h_anchor, int n_anchor, const sim3ba_depth_params& p, int n_iters, double* d_eta, double* h_cost);
+cudaError_t launch_depth_apply(Ctx* c, const float* d_points, const float* d_conf, const int32_t* d_labels, int n_seg, const double* d_eta);
+int depth_max_segments();
 
 }  // namespace sim3ba
