@@ -3,6 +3,7 @@ multi-rank logic is bench.py's aggregation -- job time = MAX over ranks, job uni
 reference arm's "rank 0 alone prints" rule.  No GPU, no oracle arithmetic."""
 import json
 import os
+import re
 import socket
 import subprocess
 import sys
@@ -44,7 +45,7 @@ def test_aggregate_is_max_time_sum_units_world2(tmp_path):
     script.write_text(WORKER.format(root=ROOT))
     r = _torchrun(2, [str(script)])
     assert r.returncode == 0, r.stderr[-2000:]
-    rows = [json.loads(ln) for ln in r.stdout.splitlines() if ln.startswith("{")]
+    rows = [json.loads(m) for m in re.findall(r"\{[^{}]*\}", r.stdout)]   # the two ranks may share a line
     assert sorted(x["rank"] for x in rows) == [0, 1]
     for x in rows:
         assert x["world"] == 2
