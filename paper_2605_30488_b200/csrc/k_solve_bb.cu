@@ -338,20 +338,20 @@ __device__ void bb_schur_row(const BBArgs& a, double* buf, int b) {
     const int c0 = a.seg_ptr[s], len = a.seg_ptr[s + 1] - c0;
     const int32_t* sb = a.seg_bord + a.seg_bptr[s];
     const int chunks16 = ((p + 1) * 49 + 1) / 2;              // 16-byte chunks of a column's blocks 0 .. p
+    const int part = 2 * chunks16;                            // doubles of one column in the buffer
+    const int ccols = min(64, (kSchurCols * kSchurPart) / part);   // columns per chunk: the narrower the row, the more
     double acc[kSchurPairs][2];
 #pragma unroll
     for (int j = 0; j < kSchurPairs; ++j) acc[j][0] = acc[j][1] = 0.0;
     auto stage = [&](int ch) {                                // columns ch * kSchurCols ... -> buffer ch & 1
       double* dst = buf + (size_t)(ch & 1) * kSchurCols * kSchurPart;
-      for (int w = 0; w < kSchurCols; ++w) {
-        const int l = ch * kSchurCols + w;
-        if (l < len) {
-          const double* src = a.colbuf + a.col_ofs[c0 + l] + oB;
-          for (int q = tid; q < chunks16; q += kSolveThreads) cp16(dst + w * kSchurPart + 2 * q, src + 2 * q);
-        }
+      const int l0 = ch * ccols, nl = min(ccols, len - l0);
+      for (int q = tid; q < nl * chunks16; q += kSolveThreads) {
+        const int w = q / chunks16, qq = q - w * chunks16;
+        cp16(dst + w * part + 2 * qq, a.colbuf + a.col_ofs[c0 + l0 + w] + oB + 2 * qq);
       }
     };
-    const int nch = (len + kSchurCols - 1) / kSchurCols;
+    const int nch = (len + ccols - 1) / ccols;
     stage(0);
     cp_commit();
     for (int ch = 0; ch < nch; ++ch) {
@@ -360,9 +360,9 @@ __device__ void bb_schur_row(const BBArgs& a, double* buf, int b) {
       cp_wait<1>();
       __syncthreads();
       const double* src = buf + (size_t)(ch & 1) * kSchurCols * kSchurPart;
-      const int ncol = min(kSchurCols, len - ch * kSchurCols);
+      const int ncol = min(ccols, len - ch * ccols);
       for (int w = 0; w < ncol; ++w) {
-        const double* F = src + w * kSchurPart;
+        const double* F = src + w * part;
         const double a0 = v0 ? F[p * 49 + f0] : 0.0, a1 = v1 ? F[p * 49 + f1] : 0.0;
 #pragma unroll
         for (int j = 0; j < kSchurPairs; ++j) {
@@ -388,6 +388,56 @@ __device__ void bb_schur_row(const BBArgs& a, double* buf, int b) {
     if (tid < 7) a.B.rhs[7 * b + tid] = __ldcg(a.B.rhs + 7 * b + tid) - __ldcg(a.seg_rhs + (size_t)(a.seg_bptr[s] + p) * 7 + tid);
     __syncthreads();                                          // a later segment may map the same block to another warp
   }
+}
+
+// ---- phase 3, border system of at most one tile (7 n_bord <= 64): unblocked Cholesky and both solves in shared memory
+// by CTA 0 (the tiled path costs two grid barriers and a 64-pivot tile for what is here a 14 x 14 system).
+__device__ void bb_small_border(const BBArgs& a, Smem& sm, int n7) {
+  const int tid = threadIdx.x;
+  const int nB = a.npadB;
+  for (int idx = tid; idx < n7 * n7; idx += kSolveThreads) {
+    const int r = idx / n7, c = idx - r * n7;
+    if (c <= r) sm.D[r * LDD + c] = __ldcg(a.B.L + (size_t)r * nB + c);
+  }
+  if (tid < n7) sm.y[tid] = __ldcg(a.B.rhs + tid);
+  if (tid == 0) sm.flag = 0;
+  __syncthreads();
+  for (int p = 0; p < n7; ++p) {
+    const double piv = sm.D[p * LDD + p];
+    const bool gd = (piv > 0.0) && (piv < 1.0e300);
+    if (!gd) { if (tid == 0) sm.flag = 1; break; }             // uniform: everybody reads the same pivot
+    const double inv = rsqrt(piv);
+    __syncthreads();                                           // the pivot has been read by all
+    for (int r = p + tid; r < n7; r += kSolveThreads) sm.D[r * LDD + p] *= inv;
+    if (tid == 0) sm.dinv[p] = inv;
+    __syncthreads();
+    const int m = n7 - p - 1;
+    for (int idx = tid; idx < m * m; idx += kSolveThreads) {
+      const int r = p + 1 + idx / m, c = p + 1 + idx % m;
+      if (c <= r) sm.D[r * LDD + c] = fma(-sm.D[r * LDD + p], sm.D[c * LDD + p], sm.D[r * LDD + c]);
+    }
+    __syncthreads();
+  }
+  __syncthreads();
+  if (sm.flag) { if (tid == 0) a.status[0] = 1; return; }
+  if (tid < 32) {                                              // L y = b, then L^T x = y: lanes own rows tid, tid + 32
+    double b0 = tid < n7 ? sm.y[tid] : 0.0, b1 = tid + 32 < n7 ? sm.y[tid + 32] : 0.0;
+    for (int c = 0; c < n7; ++c) {
+      const double yc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * sm.dinv[c];
+      if (tid == (c & 31)) { if (c < 32) b0 = yc; else b1 = yc; }
+      if (tid > c && tid < n7) b0 -= sm.D[tid * LDD + c] * yc;
+      if (tid + 32 > c && tid + 32 < n7) b1 -= sm.D[(tid + 32) * LDD + c] * yc;
+    }
+    for (int c = n7 - 1; c >= 0; --c) {
+      const double xc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * sm.dinv[c];
+      if (tid == (c & 31)) { if (c < 32) b0 = xc; else b1 = xc; }
+      if (tid < c) b0 -= sm.D[c * LDD + tid] * xc;
+      if (tid + 32 < c) b1 -= sm.D[c * LDD + tid + 32] * xc;
+    }
+    if (tid < n7) a.B.tau[tid] = b0;
+    if (tid + 32 < n7) a.B.tau[tid + 32] = b1;
+  }
+  __syncthreads();
 }
 
 // ---- phase 4: back-substitution of one segment ------------------------------------------------------------
@@ -483,6 +533,11 @@ k_solve_bb(BBArgs a) {
       for (int b = blockIdx.x; b < a.n_bord; b += G) bb_schur_row(a, win, b);
       grid_barrier(a.bar, G, gen);
       BB_STAMP(4);
+      if (nbB == 1) {                                         // one tile: direct solve by CTA 0
+        if (blockIdx.x == 0) bb_small_border(a, sm, 7 * a.n_bord);
+        grid_barrier(a.bar, G, gen);
+        failed = ld_flag(a.status) != 0;
+      } else {
       for (int k = 0; k < nbB; ++k) {                         // tiled Cholesky of S, forward solve riding along
         panel_phase(a.B, sm, k, G);
         if (a.B.col_ptr[k + 1] > a.B.col_ptr[k]) {
@@ -501,6 +556,7 @@ k_solve_bb(BBArgs a) {
           back_phase(a.B, sm, kb, G);
           if (a.B.row_ptr[kb + 1] > a.B.row_ptr[kb]) grid_barrier(a.bar, G, gen);
         }
+      }
       }
     }
     if (failed) {
