@@ -35,17 +35,19 @@ constexpr int kSlots = kPartialStride;         // 40 reduction slots (layout: si
 constexpr int kAccSlots = 37;                  // slots that carry floating-point sums
 
 // shared-memory carve-up of k_accumulate (dynamic); every array is sliced per warp
-constexpr size_t kOffXi = 0;                                            // float4 [kWarps][kWarpPx], re-laid as lane pairs
-constexpr size_t kOffRdi = kOffXi + sizeof(float4) * kTilePx;           // float2 [kWarps][kWarpPx / 2] (1/|X_A|, 1/|X_B|)
-constexpr size_t kOffIdx = kOffRdi + sizeof(float2) * (kTilePx / 2);    // int32 [kWarps][2][kWarpPx]
-constexpr size_t kOffRing = kOffIdx + sizeof(int32_t) * 2 * kTilePx;    // float4 [kWarps][kStages][64]: gathered X_j in flight
-constexpr size_t kOffBar = kOffRing + sizeof(float4) * kWarps * kStages * 64;          // mbarrier [kWarps][3]
-constexpr size_t kAccSmem = kOffBar + sizeof(uint64_t) * 3 * kWarps;
+// one contiguous region per warp, so that every shared-memory address of the pair loop is (warp base + lane * size) + constant
+constexpr size_t kOffXi = 0;                                            // float4 [kWarpPx], re-laid as lane pairs
+constexpr size_t kOffRdi = kOffXi + sizeof(float4) * kWarpPx;           // float2 [kWarpPx / 2] (1/|X_A|, 1/|X_B|)
+constexpr size_t kOffIdx = kOffRdi + sizeof(float2) * (kWarpPx / 2);    // int32 [2][kWarpPx]
+constexpr size_t kOffRing = kOffIdx + sizeof(int32_t) * 2 * kWarpPx;    // float4 [kStages][64]: gathered X_j in flight
+constexpr size_t kOffBar = kOffRing + sizeof(float4) * kStages * 64;    // mbarrier [3]
+constexpr size_t kWarpBytes = (kOffBar + sizeof(uint64_t) * 3 + 127) / 128 * 128;
+constexpr size_t kAccSmem = kWarpBytes * kWarps;
 #ifndef SIM3BA_ACC_WARPS_PER_SM
 #define SIM3BA_ACC_WARPS_PER_SM 12
 #endif
 constexpr int kAccCtasPerSm = SIM3BA_ACC_WARPS_PER_SM / kWarps;     // 12 warps per SM: bounded by registers (<= 168) and shared memory (18 KB per warp)
-static_assert(kAccCtasPerSm * (kAccSmem + 1024) <= 227 * 1024, "kAccCtasPerSm CTAs per SM");
+static_assert(kAccCtasPerSm * (kAccSmem + 1024) <= 228 * 1024, "kAccCtasPerSm CTAs per SM (228 KB of shared memory per SM, 1 KB reserved per CTA)");
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -251,11 +253,12 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
              const double* __restrict__ edgeT, double* __restrict__ partials, int HW, int tiles, int idx_tma, DevParams prm) {
   extern __shared__ __align__(128) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  float4* s_Xi = reinterpret_cast<float4*>(smem + kOffXi) + warp * kWarpPx;          // this warp's slice, re-laid as lane pairs
-  float2* s_rdi = reinterpret_cast<float2*>(smem + kOffRdi) + warp * (kWarpPx / 2);
-  float4* s_ring = reinterpret_cast<float4*>(smem + kOffRing) + warp * (kStages * 64);   // [kStages][64], slot = pair % kStages
-  int32_t* s_idx = reinterpret_cast<int32_t*>(smem + kOffIdx) + warp * (2 * kWarpPx);  // [2][kWarpPx], double-buffered over edges
-  uint64_t* s_bar = reinterpret_cast<uint64_t*>(smem + kOffBar) + warp * 3;           // [0] X_i slice, [1], [2] index buffers
+  unsigned char* wb = smem + warp * kWarpBytes;                               // this warp's region
+  float4* s_Xi = reinterpret_cast<float4*>(wb + kOffXi);                      // the warp's slice, re-laid as lane pairs
+  float2* s_rdi = reinterpret_cast<float2*>(wb + kOffRdi);
+  float4* s_ring = reinterpret_cast<float4*>(wb + kOffRing);                  // [kStages][64], slot = pair % kStages
+  int32_t* s_idx = reinterpret_cast<int32_t*>(wb + kOffIdx);                  // [2][kWarpPx], double-buffered over edges
+  uint64_t* s_bar = reinterpret_cast<uint64_t*>(wb + kOffBar);                // [0] X_i slice, [1], [2] index buffers
 
   const int g = blockIdx.x / tiles, tile = blockIdx.x - g * tiles;
   const int i = grp_kf[g];
