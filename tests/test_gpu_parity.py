@@ -341,3 +341,64 @@ def test_config2_full_size_sampled_edges():
     ba = make_solver(g, prm)
     check_system(ba, g, g.poses_init, prm, "C2-full")
     ba.close()
+
+
+def test_config4_full_size_sampled_edges_and_solver_property():
+    """BASELINE configs[3] at full size (1000 keyframes, 3036 edges, 7000 x 7000 system, the launch configuration bench.py
+    times): the match set of EVERY edge bit-exact against the validity rule written out in NumPy, the 7x7 blocks of a sample of
+    edges (first, last, every inter-agent tenth, a stride through the chains) against the oracle, and the update tau against
+    SciPy's dense Cholesky of the system assembled in NumPy from the GPU's own per-edge blocks (decomposition: a1-a5 vs the
+    oracle on samples, a6-a7 vs a library solve on the whole system)."""
+    import scipy.linalg
+    g = make_config(4)
+    prm = oracle_params("config")
+    ba = make_solver(g, prm)
+    set_poses(ba, g.poses_init)
+    ba.build_system()
+    ba.solve()
+    nv, chk, _ = (t.cpu().numpy() for t in ba.edge_stats())
+    blk = ba.edge_blocks().cpu().numpy()
+    tau, attempts, eps, _ = ba.update()
+    tau = tau.cpu().numpy()
+    HW = g.hw
+    for e in range(g.n_edges):                                 # R12, typed out: 0 <= n < HW, c_i[m] > c_min, c_j[n] > c_min
+        i, j = g.edges[e]
+        n = g.match[e].astype(np.int64)
+        m = np.flatnonzero((n >= 0) & (n < HW))
+        m = m[(g.conf[i, m] > prm.conf_min) & (g.conf[j, n[m]] > prm.conf_min)]
+        assert nv[e] == m.size, e
+        with np.errstate(over="ignore"):
+            ref = np.sum(m.astype(np.uint64) * np.uint64(HW) + n[m].astype(np.uint64), dtype=np.uint64)
+        assert chk.view(np.uint64)[e] == ref, e
+    inter = np.flatnonzero(g.edge_kind == 2)
+    sample = sorted(set([0, g.n_edges - 1] + list(inter[::10]) + list(range(5, g.n_edges, 211))))
+    sysm = orc.build_system(g.poses_init, g.points, g.conf, g.edges, g.match, prm, edge_subset=sample)
+    ref = blocks35_from_oracle(sysm)
+    for e in sample:
+        assert rel(blk[e, :28], ref[e, :28]) <= TOL_BLOCK, e
+        assert rel(blk[e, 28:], ref[e, 28:], FLOOR_G * np.linalg.norm(sysm.edge_b_abs[e])) <= TOL_BLOCK, e
+    # a6 + a7 on the whole system: assemble H, g from the GPU's blocks (two diagonal, one off-diagonal block per edge,
+    # PAPER.md:118), delete the gauge rows (PAPER.md:108), eps_0 on the diagonal (Eq. (7)), library Cholesky
+    n = 7 * g.n_kf
+    H, gg = np.zeros((n, n)), np.zeros(n)
+    iu = np.triu_indices(7)
+    for e in range(g.n_edges):
+        i, j = (int(v) for v in g.edges[e])
+        A = np.zeros((7, 7))
+        A[iu] = blk[e, :28]
+        A = A + A.T - np.diag(np.diag(A))
+        si, sj = slice(7 * i, 7 * i + 7), slice(7 * j, 7 * j + 7)
+        H[si, si] += A
+        H[sj, sj] += A
+        H[si, sj] -= A
+        H[sj, si] -= A
+        gg[sj] += blk[e, 28:]
+        gg[si] -= blk[e, 28:]
+    fr = free_idx(g)
+    Hf = H[np.ix_(fr, fr)] + prm.eps0 * np.eye(fr.size)
+    ref_tau = np.zeros(n)
+    ref_tau[fr] = -scipy.linalg.cho_solve(scipy.linalg.cho_factor(Hf, lower=True), gg[fr])
+    assert attempts == 1 and eps == prm.eps0
+    assert rel(tau, ref_tau) <= 1e-6
+    assert ba.bb_info()["valid"] == 1
+    ba.close()
