@@ -67,9 +67,24 @@ __global__ void k_damp_copy(double* __restrict__ dst, const double* __restrict__
   dst[(size_t)r * npad + c] = v;
 }
 
-__global__ void k_gradient(double* __restrict__ g, const double* __restrict__ blocks35, const int32_t* __restrict__ edges,
-                           const int32_t* __restrict__ kf_ptr, const int32_t* __restrict__ kf_edge,
-                           const uint8_t* __restrict__ fixed, int N) {
+// g from the per-edge b_e (gather over the keyframe -> edge CSR); the last block sums the per-edge robust costs instead
+__global__ void __launch_bounds__(128)
+k_gradient_cost(double* __restrict__ g, const double* __restrict__ blocks35, const int32_t* __restrict__ edges,
+                const int32_t* __restrict__ kf_ptr, const int32_t* __restrict__ kf_edge, const uint8_t* __restrict__ fixed, int N,
+                const double* __restrict__ edge_cost, int E, double* __restrict__ total) {
+  if (blockIdx.x == gridDim.x - 1) {
+    __shared__ double s[128];
+    double v = 0.0;
+    for (int e = threadIdx.x; e < E; e += 128) v += edge_cost[e];
+    s[threadIdx.x] = v;
+    __syncthreads();
+    for (int o = 64; o > 0; o >>= 1) {
+      if (threadIdx.x < o) s[threadIdx.x] += s[threadIdx.x + o];
+      __syncthreads();
+    }
+    if (threadIdx.x == 0) *total = s[0];
+    return;
+  }
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= 7 * N) return;
   const int k = idx / 7, comp = idx % 7;
@@ -82,19 +97,6 @@ __global__ void k_gradient(double* __restrict__ g, const double* __restrict__ bl
     }
   }
   g[idx] = v;
-}
-
-__global__ void __launch_bounds__(256) k_sum_cost(const double* __restrict__ edge_cost, int E, double* __restrict__ total) {
-  __shared__ double s[256];
-  double v = 0.0;
-  for (int e = threadIdx.x; e < E; e += 256) v += edge_cost[e];
-  s[threadIdx.x] = v;
-  __syncthreads();
-  for (int o = 128; o > 0; o >>= 1) {
-    if (threadIdx.x < o) s[threadIdx.x] += s[threadIdx.x + o];
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) *total = s[0];
 }
 
 __global__ void k_load_gradient(double* __restrict__ g, const double* __restrict__ src, const uint8_t* __restrict__ fixed, int n) {
@@ -121,12 +123,9 @@ cudaError_t launch_assemble(Ctx* c, double* dst, double lambda, double eps, bool
 }
 
 cudaError_t launch_gradient(Ctx* c) {
-  k_gradient<<<(7 * c->N + 127) / 128, 128, 0, c->stream>>>(c->g, c->blocks35, c->edges, c->kf_ptr, c->kf_edge,
-                                                            c->fixed_mask, c->N);
-  cudaError_t err = cudaGetLastError();
-  if (err != cudaSuccess) return err;
-  k_sum_cost<<<1, 256, 0, c->stream>>>(c->edge_cost, c->E, c->total_cost);
-  c->launches += 2;
+  k_gradient_cost<<<(7 * c->N + 127) / 128 + 1, 128, 0, c->stream>>>(c->g, c->blocks35, c->edges, c->kf_ptr, c->kf_edge, c->fixed_mask, c->N,
+                                                                     c->edge_cost, c->E, c->total_cost);
+  ++c->launches;
   return cudaGetLastError();
 }
 
