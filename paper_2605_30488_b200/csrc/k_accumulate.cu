@@ -30,7 +30,8 @@ static_assert(kTilePx == 16 * kAccThreads, "precision plan: <= 16 fp32 terms per
 constexpr int kPairs = kTilePx / (2 * kAccThreads);   // match pairs per thread and edge
 constexpr int kWarps = kAccThreads / 32;
 constexpr int kWarpPx = kTilePx / kWarps;      // contiguous pixels owned by one warp (64 per pair: A = 64 p + lane, B = A + 32)
-constexpr int kStages = 4;                     // ring of gathered X_j pairs per warp: gathers run kStages - 1 pairs ahead
+constexpr int kStages = 3;                     // ring of gathered X_j pairs per warp: gathers run kStages - 1 pairs ahead (a 4th
+                                               // stage would push twelve one-warp CTAs 24 bytes past the 228 KB of an SM)
 constexpr int kSlots = kPartialStride;         // 40 reduction slots (layout: sim3ba_internal.cuh)
 constexpr int kAccSlots = 37;                  // slots that carry floating-point sums
 

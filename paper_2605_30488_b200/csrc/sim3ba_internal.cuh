@@ -11,7 +11,8 @@
 
 namespace sim3ba {
 
-constexpr int kAccThreads = 64;      // accumulate CTA: two independent warps
+constexpr int kAccThreads = 32;      // accumulate CTA: ONE warp -- warps are independent workers, so the finest CTA gives the block
+                                     // scheduler the finest grain (a two-warp CTA holds its slot until the slower warp is done)
 constexpr int kTilePx = 16 * kAccThreads;   // pixels of a keyframe handled by one accumulate CTA (512 contiguous per warp)
 // doubles per (edge, 512-pixel warp slice) partial record: [0..27] upper triangle of M = sum J_xi^T Omega J_xi (row-major,
 // r <= c; (3,6), (4,6), (5,6) are structurally zero), [28..34] c = sum J_xi^T Omega e, [35] sum w r^2,
