@@ -30,8 +30,9 @@ static_assert(kTilePx == 16 * kAccThreads, "precision plan: <= 16 fp32 terms per
 constexpr int kPairs = kTilePx / (2 * kAccThreads);   // match pairs per thread and edge
 constexpr int kWarps = kAccThreads / 32;
 constexpr int kWarpPx = kTilePx / kWarps;      // contiguous pixels owned by one warp (64 per pair: A = 64 p + lane, B = A + 32)
-constexpr int kStages = 3;                     // ring of gathered X_j pairs per warp: gathers run kStages - 1 pairs ahead (a 4th
-                                               // stage would push twelve one-warp CTAs 24 bytes past the 228 KB of an SM)
+constexpr int kStages = 2;                     // ring of gathered X_j pairs per warp: gathers run kStages - 1 pairs ahead.  Two stages
+                                               // (15.4 KB + 1 KB reserved per one-warp CTA) let 13 warps share the 228 KB of an SM; three
+                                               // stages with 12 warps measured 3-5 % slower
 constexpr int kSlots = kPartialStride;         // 40 reduction slots (layout: sim3ba_internal.cuh)
 constexpr int kAccSlots = 37;                  // slots that carry floating-point sums
 
@@ -45,9 +46,9 @@ constexpr size_t kOffBar = kOffRing + sizeof(float4) * kStages * 64;    // mbarr
 constexpr size_t kWarpBytes = (kOffBar + sizeof(uint64_t) * 3 + 127) / 128 * 128;
 constexpr size_t kAccSmem = kWarpBytes * kWarps;
 #ifndef SIM3BA_ACC_WARPS_PER_SM
-#define SIM3BA_ACC_WARPS_PER_SM 12
+#define SIM3BA_ACC_WARPS_PER_SM 13
 #endif
-constexpr int kAccCtasPerSm = SIM3BA_ACC_WARPS_PER_SM / kWarps;     // 12 warps per SM: bounded by registers (<= 168) and shared memory (18 KB per warp)
+constexpr int kAccCtasPerSm = SIM3BA_ACC_WARPS_PER_SM / kWarps;     // warps per SM: bounded by registers (<= 152) and shared memory
 static_assert(kAccCtasPerSm * (kAccSmem + 1024) <= 228 * 1024, "kAccCtasPerSm CTAs per SM (228 KB of shared memory per SM, 1 KB reserved per CTA)");
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }

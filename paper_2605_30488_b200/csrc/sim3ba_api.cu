@@ -391,10 +391,20 @@ int sim3ba_optimize_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_
   int32_t *d_edges = nullptr, *d_match = nullptr;
   sim3ba_ctx* h = nullptr;
   int rc = SIM3BA_OK;
+  // the graph buffers come from the device's stream-ordered pool, kept warm between jobs (no map / unmap per job)
+  {
+    int dev = 0;
+    cudaMemPool_t pool;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+      uint64_t keep = UINT64_MAX;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+  }
   auto cleanup = [&]() {
-    if (h) sim3ba_destroy(h);
-    cudaFree(d_points); cudaFree(d_conf); cudaFree(d_edges); cudaFree(d_match);
+    if (h) sim3ba_destroy(h);                                   // synchronises the stream
+    cudaFreeAsync(d_points, st); cudaFreeAsync(d_conf, st); cudaFreeAsync(d_edges, st); cudaFreeAsync(d_match, st);
   };
+  auto pool_alloc = [&](void** ptr, size_t bytes) { return cudaMallocAsync(ptr, std::max<size_t>(bytes, 16), st); };
 #define CUJ(call)                                                       \
   do {                                                                  \
     cudaError_t e_ = (call);                                            \
@@ -403,10 +413,10 @@ int sim3ba_optimize_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_
       return cuda_fail(nullptr, e_, #call);                             \
     }                                                                   \
   } while (0)
-  CUJ(dev_alloc(&d_points, 3 * NHW));
-  CUJ(dev_alloc(&d_conf, NHW));
-  CUJ(dev_alloc(&d_edges, 2 * (size_t)n_edges));
-  CUJ(dev_alloc(&d_match, EHW));
+  CUJ(pool_alloc(reinterpret_cast<void**>(&d_points), 3 * NHW * sizeof(float)));
+  CUJ(pool_alloc(reinterpret_cast<void**>(&d_conf), NHW * sizeof(float)));
+  CUJ(pool_alloc(reinterpret_cast<void**>(&d_edges), 2 * (size_t)n_edges * sizeof(int32_t)));
+  CUJ(pool_alloc(reinterpret_cast<void**>(&d_match), EHW * sizeof(int32_t)));
   CUJ(cudaMemcpyAsync(d_points, h_points, 3 * NHW * sizeof(float), cudaMemcpyHostToDevice, st));
   CUJ(cudaMemcpyAsync(d_conf, h_conf, NHW * sizeof(float), cudaMemcpyHostToDevice, st));
   if (n_edges > 0) {
