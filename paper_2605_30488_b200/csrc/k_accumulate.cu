@@ -30,23 +30,23 @@ static_assert(kTilePx == 16 * kAccThreads, "precision plan: <= 16 fp32 terms per
 constexpr int kPairs = kTilePx / (2 * kAccThreads);   // match pairs per thread and edge
 constexpr int kWarps = kAccThreads / 32;
 constexpr int kWarpPx = kTilePx / kWarps;      // contiguous pixels owned by one warp (64 per pair: A = 64 p + lane, B = A + 32)
-constexpr int kStages = 2;                     // ring of gathered X_j pairs per warp: gathers run kStages - 1 pairs ahead.  Two stages
-                                               // (15.4 KB + 1 KB reserved per one-warp CTA) let 13 warps share the 228 KB of an SM; three
-                                               // stages with 12 warps measured 3-5 % slower
+constexpr int kStages = 2;                     // ring of gathered X_j pairs per warp: gathers run kStages - 1 pairs ahead.  Two stages and
+                                               // no stored 1/|X_i| (14.1 KB + 1 KB reserved per one-warp CTA) let 14 warps share the 228 KB
+                                               // of an SM.  Measured on C2: 12 warps / 3 stages 177.6 us, 13 / 2 171.3, 14 / 2 165.8; 16 warps
+                                               // with the index buffer refilled in halves 167.8 (not kept)
 constexpr int kSlots = kPartialStride;         // 40 reduction slots (layout: sim3ba_internal.cuh)
 constexpr int kAccSlots = 37;                  // slots that carry floating-point sums
 
 // shared-memory carve-up of k_accumulate (dynamic); every array is sliced per warp
 // one contiguous region per warp, so that every shared-memory address of the pair loop is (warp base + lane * size) + constant
 constexpr size_t kOffXi = 0;                                            // float4 [kWarpPx], re-laid as lane pairs
-constexpr size_t kOffRdi = kOffXi + sizeof(float4) * kWarpPx;           // float2 [kWarpPx / 2] (1/|X_A|, 1/|X_B|)
-constexpr size_t kOffIdx = kOffRdi + sizeof(float2) * (kWarpPx / 2);    // int32 [2][kWarpPx]
+constexpr size_t kOffIdx = kOffXi + sizeof(float4) * kWarpPx;           // int32 [2][kWarpPx]
 constexpr size_t kOffRing = kOffIdx + sizeof(int32_t) * 2 * kWarpPx;    // float4 [kStages][64]: gathered X_j in flight
 constexpr size_t kOffBar = kOffRing + sizeof(float4) * kStages * 64;    // mbarrier [3]
 constexpr size_t kWarpBytes = (kOffBar + sizeof(uint64_t) * 3 + 127) / 128 * 128;
 constexpr size_t kAccSmem = kWarpBytes * kWarps;
 #ifndef SIM3BA_ACC_WARPS_PER_SM
-#define SIM3BA_ACC_WARPS_PER_SM 13
+#define SIM3BA_ACC_WARPS_PER_SM 14
 #endif
 constexpr int kAccCtasPerSm = SIM3BA_ACC_WARPS_PER_SM / kWarps;     // warps per SM: bounded by registers (<= 152) and shared memory
 static_assert(kAccCtasPerSm * (kAccSmem + 1024) <= 228 * 1024, "kAccCtasPerSm CTAs per SM (228 KB of shared memory per SM, 1 KB reserved per CTA)");
@@ -257,7 +257,6 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   unsigned char* wb = smem + warp * kWarpBytes;                               // this warp's region
   float4* s_Xi = reinterpret_cast<float4*>(wb + kOffXi);                      // the warp's slice, re-laid as lane pairs
-  float2* s_rdi = reinterpret_cast<float2*>(wb + kOffRdi);
   float4* s_ring = reinterpret_cast<float4*>(wb + kOffRing);                  // [kStages][64], slot = pair % kStages
   int32_t* s_idx = reinterpret_cast<int32_t*>(wb + kOffIdx);                  // [2][kWarpPx], double-buffered over edges
   uint64_t* s_bar = reinterpret_cast<uint64_t*>(wb + kOffBar);                // [0] X_i slice, [1], [2] index buffers
@@ -302,18 +301,14 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
   if (n_e > 0) issue_idx(0);
   if (npx > 0) mbar_wait(s_bar, 0);
   // Pair p of a lane = pixels A = 64 p + lane and B = A + 32 of the slice.  Re-lay the two staged float4 in place as
-  // lane pairs, (xA, xB, yA, yB) in A's slot and (zA, zB, wA, wB) in B's, and keep (1/|X_A|, 1/|X_B|):
-  // everything the edges leaving i share.  Thread-private slots: no synchronisation needed.
+  // lane pairs, (xA, xB, yA, yB) in A's slot and (zA, zB, wA, wB) in B's: what the edges leaving i share.
+  // Thread-private slots: no synchronisation needed.
 #pragma unroll 2
   for (int p = 0; p < kPairs; ++p) {
     const int pa = 64 * p + lane, pb = pa + 32;
     const float4 A = s_Xi[pa], B = s_Xi[pb];
-    const float da2 = fmaxf(fmaf(A.x, A.x, fmaf(A.y, A.y, A.z * A.z)), 1e-20f);
-    const float db2 = fmaxf(fmaf(B.x, B.x, fmaf(B.y, B.y, B.z * B.z)), 1e-20f);
-    const float ra = rsq(da2), rb = rsq(db2);
     s_Xi[pa] = make_float4(A.x, B.x, A.y, B.y);
     s_Xi[pb] = make_float4(A.z, B.z, A.w, B.w);
-    s_rdi[32 * p + lane] = make_float2(ra, rb);
   }
 
   // Gathers: per-lane 16-byte cp.async into the warp's ring, kStages - 1 pairs ahead of the arithmetic, flat over the
@@ -382,7 +377,12 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
       const bool vA = (XA0.w >= 0.f) && (P1.z >= 0.f), vB = (XA1.w >= 0.f) && (P1.w >= 0.f);
       if (__any_sync(0xffffffffu, vA || vB)) {               // whole invalid bands are skipped warp-uniformly
         const float4 P0 = s_Xi[pa];                          // (xA, xB, yA, yB)
-        const float2 rdi = s_rdi[32 * p + lane];
+        f2 rdi;                                              // 1 / |X_i|, recomputed per edge: a stored copy would cost the 14th warp
+        {
+          const f2 d2i = fma2(make_float2(P0.x, P0.y), make_float2(P0.x, P0.y), fma2(make_float2(P0.z, P0.w), make_float2(P0.z, P0.w),
+                              make_float2(P1.x, P1.y) * make_float2(P1.x, P1.y)));
+          rdi = make_float2(rsq(fmaxf(d2i.x, 1e-20f)), rsq(fmaxf(d2i.y, 1e-20f)));
+        }
         f2 del0, del1, del2;
         delta(XA0, P0.x, P0.z, P1.x, del0.x, del1.x, del2.x);
         delta(XA1, P0.y, P0.w, P1.y, del0.y, del1.y, del2.y);
