@@ -4,8 +4,9 @@
 // The Sim(3) graph of PAPER.md:108 is, per agent, a temporal chain (edges (k, k+1..k+3)) plus a few
 // long links: loop closures and inter-agent edges.  One endpoint of every long link becomes a BORDER
 // keyframe (greedy vertex cover, the endpoint with more long links first); a chain longer than
-// `lmax` interior keyframes is cut by making the next kBand keyframes border as well (substructuring:
+// `lmax` (about 2 sqrt(N)) interior keyframes is cut by making the next kBand keyframes border as well (substructuring:
 // the pieces are then independent and are eliminated in parallel).  Integer bookkeeping only.
+#include <math.h>
 #include <stdlib.h>
 
 #include <algorithm>
@@ -43,7 +44,12 @@ bool build_bb_plan(Ctx* c, std::string& err) {
   P.valid = false;
   const int N = c->N;
   const int n_pairs = (int)c->h_pair_kf.size() / 2;
-  int lmax = 160;
+  // Longest segment.  A segment costs ~2 us per keyframe, sequentially; every cut adds kBand keyframes to the dense border
+  // system, which costs ~35 us per 64 rows: the two balance near lmax ~ 2 sqrt(free keyframes) (measured on the BASELINE
+  // graphs: 200 keyframes best at 16-32, 1000 at 50-60, 2000 at 80-100).  SIM3BA_BB_LMAX overrides (tests, experiments).
+  int n_free = 0;
+  for (int k = 0; k < N; ++k) n_free += c->h_fixed[k] ? 0 : 1;
+  int lmax = std::max(12, std::min(160, (int)(2.0 * sqrt((double)n_free) + 0.5)));
   if (const char* s = getenv("SIM3BA_BB_LMAX")) lmax = std::max(4, atoi(s));
 
   enum { FIXED = 0, INTERIOR = 1, BORDER = 2 };
