@@ -119,20 +119,6 @@ struct SegSmem {
   int fail;
 };
 
-// 1 / sqrt(p) to full double precision from the fp32 MUFU estimate and two Newton steps (relative error 2e-7 -> 6e-14
-// -> 5e-27 before rounding); pivots outside the comfortable fp32 range take the library routine
-__device__ __forceinline__ double fast_rsqrt(double p) {
-  const float pf = (float)p;
-  if (!(pf > 1e-30f && pf < 1e30f)) return rsqrt(p);
-  float rf;
-  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rf) : "f"(pf));
-  double y = (double)rf;
-  const double h = 0.5 * p;
-  y = y * fma(-h * y, y, 1.5);
-  y = y * fma(-h * y, y, 1.5);
-  return y;
-}
-
 // Cholesky of the 7x7 diagonal block at `col` by one warp: lane r holds row r, pivots and columns travel by shuffles.
 // Leaves L (lower triangle, zeros above) in the block and the reciprocal pivots in inv[]; returns false on a bad pivot.
 __device__ __forceinline__ bool potrf7_warp(double* col, double* inv, int lane) {

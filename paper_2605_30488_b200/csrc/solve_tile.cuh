@@ -65,111 +65,135 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// ---- rank-8 update shared by POTRF and TRSM -----------------------------------------------------
-// C[r][t0 + j] -= sum_{s<8} C[r][c0 + s] * D[t0 + j][c0 + s]   for the row set of this call, t0 = c0 + 8.
-// Each thread owns a strided 4x4 block: rows r0 + rstep*ii, columns t0 + bj + nblk*jj.
-__device__ __forceinline__ void rank8_block(double* C, int ldc, const double* D, int c0, int r0,
-                                            int rstep, int nr, int bj, int nblk) {
-  const int t0 = c0 + 8;
-  double acc[4][4];
-#pragma unroll
-  for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-    for (int jj = 0; jj < 4; ++jj) acc[ii][jj] = (ii < nr) ? C[(r0 + rstep * ii) * ldc + t0 + bj + nblk * jj] : 0.0;
-#pragma unroll
-  for (int s = 0; s < 8; ++s) {
-    double lr[4], lc[4];
-#pragma unroll
-    for (int ii = 0; ii < 4; ++ii) lr[ii] = (ii < nr) ? C[(r0 + rstep * ii) * ldc + c0 + s] : 0.0;
-#pragma unroll
-    for (int jj = 0; jj < 4; ++jj) lc[jj] = D[(t0 + bj + nblk * jj) * LDD + c0 + s];
-#pragma unroll
-    for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-      for (int jj = 0; jj < 4; ++jj) acc[ii][jj] = fma(-lr[ii], lc[jj], acc[ii][jj]);
-  }
-#pragma unroll
-  for (int ii = 0; ii < 4; ++ii)
-#pragma unroll
-    for (int jj = 0; jj < 4; ++jj)
-      if (ii < nr) C[(r0 + rstep * ii) * ldc + t0 + bj + nblk * jj] = acc[ii][jj];
+// 1 / sqrt(p) to full double precision from the fp32 MUFU estimate and two Newton steps (relative error 2e-7 -> 6e-14
+// -> 5e-27 before rounding); pivots outside the comfortable fp32 range take the library routine
+__device__ __forceinline__ double fast_rsqrt(double p) {
+  const float pf = (float)p;
+  if (!(pf > 1e-30f && pf < 1e30f)) return rsqrt(p);
+  float rf;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rf) : "f"(pf));
+  double y = (double)rf;
+  const double h = 0.5 * p;
+  y = y * fma(-h * y, y, 1.5);
+  y = y * fma(-h * y, y, 1.5);
+  return y;
+}
+
+// ---- rank-8 update on the FP64 tensor pipe ----------------------------------------------------------
+// C[rb + i][cb + j] -= sum_{s<8} X[rb + i][c0 + s] * D[cb + j][c0 + s], i, j < 8: one warp, two DMMA.8x8x4.
+// X (stride ldx) holds the rows being updated, D (stride LDD) the factorised panel; C lives in X.
+__device__ __forceinline__ void rank8_dmma(double* X, int ldx, const double* D, int c0, int rb, int cb, int lane) {
+  const int gid = lane >> 2, tig = lane & 3;
+  double* cp = X + (rb + gid) * ldx + cb + 2 * tig;
+  double v0 = cp[0], v1 = cp[1];
+  const double* ap = X + (rb + gid) * ldx + c0 + tig;
+  const double* bp = D + (cb + gid) * LDD + c0 + tig;
+  dmma884(v0, v1, -ap[0], bp[0]);
+  dmma884(v0, v1, -ap[4], bp[4]);
+  cp[0] = v0;
+  cp[1] = v1;
 }
 
 // ---- Cholesky of the 64x64 tile in sm.D (lower triangle; the upper triangle is scratch) ---------
 // Returns false (uniformly) on a pivot that is <= 0 or not finite.  Only the first npan 8-column micro-panels are
-// factorised: the rows behind them are identity padding (pivot 1, nothing to eliminate).
+// factorised: the rows behind them are identity padding (pivot 1, nothing to eliminate).  Per micro-panel: the 8x8
+// diagonal block by ONE thread in registers (no shuffles on the 8-pivot chain), the rows below it by one thread each
+// against that block, the trailing matrix by rank-8 DMMA updates (lower block pairs spread over the warps).
 __device__ bool potrf64(Smem& sm, int tid, int npan) {
   const int lane = tid & 31, warp = tid >> 5;
   if (tid == 0) sm.flag = 0;
   if (tid >= 8 * npan && tid < NB) sm.dinv[tid] = 1.0;
+  __syncthreads();
   for (int pb = 0; pb < npan; ++pb) {
     const int c0 = 8 * pb;
-    if (warp == 0) {   // micro-panel: rows lane and lane + 32, columns c0 .. c0 + 7, in registers
-      double a0[8], a1[8];
+    if (tid == 0) {
+      double a[8][8];
 #pragma unroll
-      for (int t = 0; t < 8; ++t) { a0[t] = sm.D[lane * LDD + c0 + t]; a1[t] = sm.D[(lane + 32) * LDD + c0 + t]; }
+      for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int c = 0; c <= r; ++c) a[r][c] = sm.D[(c0 + r) * LDD + c0 + c];
       bool good = true;
 #pragma unroll
-      for (int s = 0; s < 8; ++s) {
-        const int R = c0 + s;
-        const double p = __shfl_sync(0xffffffffu, (R < 32) ? a0[s] : a1[s], R & 31);
-        const bool g = (p > 0.0) && (p < 1.0e300);   // false for NaN, <= 0, inf
+      for (int p = 0; p < 8; ++p) {
+        const double piv = a[p][p];
+        const bool g = (piv > 0.0) && (piv < 1.0e300);   // false for NaN, <= 0, inf
         good = good && g;
-        const double inv = g ? rsqrt(p) : 1.0;
-        a0[s] *= inv;
-        a1[s] *= inv;
+        const double inv = g ? fast_rsqrt(piv) : 1.0;
+        sm.dinv[c0 + p] = inv;
 #pragma unroll
-        for (int t = s + 1; t < 8; ++t) {
-          const int Rt = c0 + t;
-          const double lt = __shfl_sync(0xffffffffu, (Rt < 32) ? a0[s] : a1[s], Rt & 31);
-          a0[t] = fma(-a0[s], lt, a0[t]);
-          a1[t] = fma(-a1[s], lt, a1[t]);
-        }
-        if (lane == 0) sm.dinv[R] = inv;
+        for (int r = p; r < 8; ++r) a[r][p] *= inv;
+#pragma unroll
+        for (int c = p + 1; c < 8; ++c)
+#pragma unroll
+          for (int r = c; r < 8; ++r) a[r][c] = fma(-a[r][p], a[c][p], a[r][c]);
       }
 #pragma unroll
-      for (int t = 0; t < 8; ++t) { sm.D[lane * LDD + c0 + t] = a0[t]; sm.D[(lane + 32) * LDD + c0 + t] = a1[t]; }
-      if (!good && lane == 0) sm.flag = 1;
+      for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int c = 0; c <= r; ++c) sm.D[(c0 + r) * LDD + c0 + c] = a[r][c];
+      if (!good) sm.flag = 1;
     }
     __syncthreads();
-    const int nblk = (NB - c0 - 8) >> 2;   // 14, 12, ..., 0
-    if (tid < nblk * nblk) {
-      const int bi = tid / nblk, bj = tid - bi * nblk;
-      rank8_block(sm.D, LDD, sm.D, c0, c0 + 8 + bi, nblk, 4, bj, nblk);
+    const int below = NB - c0 - 8;                       // rows under the diagonal block
+    if (tid < below) {                                   // x L11^T = a, one row per thread
+      double* row = sm.D + (c0 + 8 + tid) * LDD + c0;
+      double x[8];
+#pragma unroll
+      for (int t = 0; t < 8; ++t) x[t] = row[t];
+#pragma unroll
+      for (int s = 0; s < 8; ++s) {
+#pragma unroll
+        for (int m = 0; m < s; ++m) x[s] = fma(-x[m], sm.D[(c0 + s) * LDD + c0 + m], x[s]);
+        x[s] *= sm.dinv[c0 + s];
+      }
+#pragma unroll
+      for (int t = 0; t < 8; ++t) row[t] = x[t];
+    }
+    __syncthreads();
+    const int nb8 = below >> 3;                          // 8x8 blocks per side of the trailing matrix
+    for (int t = warp; t < nb8 * (nb8 + 1) / 2; t += kSolveThreads / 32) {
+      int bi = 0, rem = t;
+      while (rem > bi) { rem -= bi + 1; ++bi; }          // t -> (bi, bj = rem), bj <= bi
+      rank8_dmma(sm.D, LDD, sm.D, c0, c0 + 8 + 8 * bi, c0 + 8 + 8 * rem, lane);
     }
     __syncthreads();
   }
-  __syncthreads();
   return sm.flag == 0;
 }
 
 // ---- X L_kk^T = A for the tile in sm.A (stride LDD), rows 0..nrows-1 plus, if with_rhs, row NB -----
+// Per micro-panel: every row against the 8x8 diagonal block of L_kk (one thread per row), then the remaining columns of
+// the rows by rank-8 DMMA updates (the right-hand-side row by plain FMAs).
 __device__ void trsm64(Smem& sm, int nrows, bool with_rhs, int tid, int npan) {
+  const int lane = tid & 31, warp = tid >> 5;
   const bool row_thread = (tid < nrows) || (with_rhs && tid == NB);
   for (int pb = 0; pb < npan; ++pb) {   // the columns behind the first npan micro-panels belong to padding rows: X stays 0 there
     const int c0 = 8 * pb;
     if (row_thread) {
+      double* row = sm.A + tid * LDD + c0;
       double x[8];
 #pragma unroll
-      for (int t = 0; t < 8; ++t) x[t] = sm.A[tid * LDD + c0 + t];
+      for (int t = 0; t < 8; ++t) x[t] = row[t];
 #pragma unroll
       for (int s = 0; s < 8; ++s) {
-        x[s] *= sm.dinv[c0 + s];
 #pragma unroll
-        for (int t = s + 1; t < 8; ++t) x[t] = fma(-x[s], sm.D[(c0 + t) * LDD + c0 + s], x[t]);
+        for (int m = 0; m < s; ++m) x[s] = fma(-x[m], sm.D[(c0 + s) * LDD + c0 + m], x[s]);
+        x[s] *= sm.dinv[c0 + s];
       }
 #pragma unroll
-      for (int t = 0; t < 8; ++t) sm.A[tid * LDD + c0 + t] = x[t];
+      for (int t = 0; t < 8; ++t) row[t] = x[t];
     }
     __syncthreads();
-    const int nblk = (NB - c0 - 8) >> 2;
-    if (nblk > 0) {
-      if (nrows > 0 && tid < 16 * nblk) {
-        const int rg = tid / nblk, bj = tid - rg * nblk;
-        rank8_block(sm.A, LDD, sm.D, c0, rg, 16, 4, bj, nblk);
-      } else if (with_rhs && tid >= 224 && tid < 224 + nblk) {
-        rank8_block(sm.A, LDD, sm.D, c0, NB, 0, 1, tid - 224, nblk);
-      }
+    const int nc8 = (NB - c0 - 8) >> 3;                  // 8-column blocks still to update
+    if (nrows > 0)
+      for (int t = warp; t < (NB / 8) * nc8; t += kSolveThreads / 32)
+        rank8_dmma(sm.A, LDD, sm.D, c0, 8 * (t / nc8), c0 + 8 + 8 * (t % nc8), lane);
+    if (with_rhs && tid >= 192 && tid < 192 + 8 * nc8) {  // the right-hand-side row (warps 6, 7: last in the DMMA round-robin)
+      const int c = c0 + 8 + (tid - 192);
+      double acc = sm.A[NB * LDD + c];
+#pragma unroll
+      for (int s = 0; s < 8; ++s) acc = fma(-sm.A[NB * LDD + c0 + s], sm.D[c * LDD + c0 + s], acc);
+      sm.A[NB * LDD + c] = acc;
     }
     __syncthreads();
   }
