@@ -119,34 +119,6 @@ struct SegSmem {
   int fail;
 };
 
-// Cholesky of the 7x7 diagonal block at `col` by one warp: lane r holds row r, pivots and columns travel by shuffles.
-// Leaves L (lower triangle, zeros above) in the block and the reciprocal pivots in inv[]; returns false on a bad pivot.
-__device__ __forceinline__ bool potrf7_warp(double* col, double* inv, int lane) {
-  double v[7];
-#pragma unroll
-  for (int k = 0; k < 7; ++k) v[k] = (lane < 7) ? col[lane * 7 + k] : 0.0;
-  bool good = true;
-#pragma unroll
-  for (int p = 0; p < 7; ++p) {
-    const double piv = __shfl_sync(0xffffffffu, v[p], p);
-    const bool gd = (piv > 0.0) && (piv < 1.0e300);           // false for NaN, <= 0, inf
-    good = good && gd;
-    const double iv = gd ? fast_rsqrt(piv) : 1.0;
-    v[p] *= iv;
-#pragma unroll
-    for (int t = p + 1; t < 7; ++t) {
-      const double lt = __shfl_sync(0xffffffffu, v[p], t);
-      v[t] = fma(-v[p], lt, v[t]);
-    }
-    if (lane == 0) inv[p] = iv;
-  }
-  if (lane < 7) {
-#pragma unroll
-    for (int k = 0; k < 7; ++k) col[lane * 7 + k] = (k <= lane) ? v[k] : 0.0;
-  }
-  return good;
-}
-
 // Right-looking block Cholesky of segment s with one column of look-ahead: while warps 1..7 apply the trailing update of
 // column l and write it back, warp 0 finishes the diagonal block of column l + 1 and factorises it, so the serial chain
 // per column is  TRSM(l) -> max(update(l), POTRF(l + 1)).
@@ -169,7 +141,7 @@ __device__ void bb_segment(const BBArgs& a, double* win, double* brhs, SegSmem& 
   for (int l = 0; l < kWin - 1; ++l) { load_col(l); cp_commit(); }
   cp_wait<kWin - 2>();                                        // column 0 has landed
   __syncthreads();
-  if (warp == 0 && !potrf7_warp(slot(0), ss.inv[0], lane) && lane == 0) ss.fail = 1;
+  if (warp == 0 && !potrf_warp<7>(slot(0), 7, ss.inv[0], lane) && lane == 0) ss.fail = 1;
   __syncthreads();
   for (int l = 0; l < len; ++l) {
     if (ss.fail) break;                                       // uniform: the attempt has failed
@@ -225,7 +197,7 @@ __device__ void bb_segment(const BBArgs& a, double* win, double* brhs, SegSmem& 
           tc[e] -= acc;
         }
         __syncwarp();
-        if (!potrf7_warp(tc, ss.inv[(l + 1) & 1], lane) && lane == 0) ss.fail = 1;
+        if (!potrf_warp<7>(tc, 7, ss.inv[(l + 1) & 1], lane) && lane == 0) ss.fail = 1;
       }
     } else {
       const int wt = tid - 32;                                // 0 .. 223

@@ -79,6 +79,36 @@ __device__ __forceinline__ double fast_rsqrt(double p) {
   return y;
 }
 
+// Cholesky of an N x N block (N <= 8, row stride ld) by one warp: lane r holds row r, pivots and columns travel by
+// shuffles, the column updates of a pivot run in parallel over the lanes.  Leaves L in the lower triangle (the strict upper
+// triangle is zeroed) and the reciprocal pivots in inv[]; returns false on a pivot that is <= 0 or not finite.
+template <int N>
+__device__ __forceinline__ bool potrf_warp(double* blk, int ld, double* inv, int lane) {
+  double v[N];
+#pragma unroll
+  for (int k = 0; k < N; ++k) v[k] = (lane < N) ? blk[lane * ld + k] : 0.0;
+  bool good = true;
+#pragma unroll
+  for (int p = 0; p < N; ++p) {
+    const double piv = __shfl_sync(0xffffffffu, v[p], p);
+    const bool gd = (piv > 0.0) && (piv < 1.0e300);           // false for NaN, <= 0, inf
+    good = good && gd;
+    const double iv = gd ? fast_rsqrt(piv) : 1.0;
+    v[p] *= iv;
+#pragma unroll
+    for (int t = p + 1; t < N; ++t) {
+      const double lt = __shfl_sync(0xffffffffu, v[p], t);
+      v[t] = fma(-v[p], lt, v[t]);
+    }
+    if (lane == 0) inv[p] = iv;
+  }
+  if (lane < N) {
+#pragma unroll
+    for (int k = 0; k < N; ++k) blk[lane * ld + k] = (k <= lane) ? v[k] : 0.0;
+  }
+  return good;
+}
+
 // ---- rank-8 update on the FP64 tensor pipe ----------------------------------------------------------
 // C[rb + i][cb + j] -= sum_{s<8} X[rb + i][c0 + s] * D[cb + j][c0 + s], i, j < 8: one warp, two DMMA.8x8x4.
 // X (stride ldx) holds the rows being updated, D (stride LDD) the factorised panel; C lives in X.
@@ -97,8 +127,8 @@ __device__ __forceinline__ void rank8_dmma(double* X, int ldx, const double* D, 
 // ---- Cholesky of the 64x64 tile in sm.D (lower triangle; the upper triangle is scratch) ---------
 // Returns false (uniformly) on a pivot that is <= 0 or not finite.  Only the first npan 8-column micro-panels are
 // factorised: the rows behind them are identity padding (pivot 1, nothing to eliminate).  Per micro-panel: the 8x8
-// diagonal block by ONE thread in registers (no shuffles on the 8-pivot chain), the rows below it by one thread each
-// against that block, the trailing matrix by rank-8 DMMA updates (lower block pairs spread over the warps).
+// diagonal block by one warp (lane = row, fp32-seeded Newton rsqrt), the rows below it by one thread each against that
+// block, the trailing matrix by rank-8 DMMA updates (lower block pairs spread over the warps).
 __device__ bool potrf64(Smem& sm, int tid, int npan) {
   const int lane = tid & 31, warp = tid >> 5;
   if (tid == 0) sm.flag = 0;
@@ -106,33 +136,7 @@ __device__ bool potrf64(Smem& sm, int tid, int npan) {
   __syncthreads();
   for (int pb = 0; pb < npan; ++pb) {
     const int c0 = 8 * pb;
-    if (tid == 0) {
-      double a[8][8];
-#pragma unroll
-      for (int r = 0; r < 8; ++r)
-#pragma unroll
-        for (int c = 0; c <= r; ++c) a[r][c] = sm.D[(c0 + r) * LDD + c0 + c];
-      bool good = true;
-#pragma unroll
-      for (int p = 0; p < 8; ++p) {
-        const double piv = a[p][p];
-        const bool g = (piv > 0.0) && (piv < 1.0e300);   // false for NaN, <= 0, inf
-        good = good && g;
-        const double inv = g ? fast_rsqrt(piv) : 1.0;
-        sm.dinv[c0 + p] = inv;
-#pragma unroll
-        for (int r = p; r < 8; ++r) a[r][p] *= inv;
-#pragma unroll
-        for (int c = p + 1; c < 8; ++c)
-#pragma unroll
-          for (int r = c; r < 8; ++r) a[r][c] = fma(-a[r][p], a[c][p], a[r][c]);
-      }
-#pragma unroll
-      for (int r = 0; r < 8; ++r)
-#pragma unroll
-        for (int c = 0; c <= r; ++c) sm.D[(c0 + r) * LDD + c0 + c] = a[r][c];
-      if (!good) sm.flag = 1;
-    }
+    if (warp == 0 && !potrf_warp<8>(sm.D + c0 * LDD + c0, LDD, sm.dinv + c0, lane) && lane == 0) sm.flag = 1;
     __syncthreads();
     const int below = NB - c0 - 8;                       // rows under the diagonal block
     if (tid < below) {                                   // x L11^T = a, one row per thread
