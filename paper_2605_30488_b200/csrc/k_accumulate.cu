@@ -431,10 +431,11 @@ k_edge_prep(const double* __restrict__ poses, const int32_t* __restrict__ edges,
 }
 
 // Kernel 2: per edge, sum the slice records (FP64, fixed order: kFinGroups interleaved running sums, then group
-// 0..5), then the adjoint congruence A_e = Ad^T M Ad, b_e = Ad^T c with Ad = Ad_{T_i^-1}.
-constexpr int kFinGroups = 6;
-constexpr int kFinThreads = 256;
-__global__ void __launch_bounds__(kFinThreads)
+// 0 .. kFinGroups - 1), then the adjoint congruence A_e = Ad^T M Ad, b_e = Ad^T c with Ad = Ad_{T_i^-1}.
+// Two shapes: 6 groups / 256 threads, and 24 groups / 1024 threads for few edges with many records (latency of the serial
+// record loop against the number of resident CTAs); the choice depends on (E, records) only, so results stay reproducible.
+template <int kFinGroups>
+__global__ void __launch_bounds__(kFinGroups * 40 + 16)
 k_finalize(const double* __restrict__ partials, const int32_t* __restrict__ edges, const double* __restrict__ poses,
            double* __restrict__ blocks35, double* __restrict__ edge_cost, int32_t* __restrict__ n_valid,
            unsigned long long* __restrict__ checksum, int records) {
@@ -549,8 +550,13 @@ cudaError_t launch_accumulate(Ctx* c) {
   err = cudaGetLastError();
   if (err != cudaSuccess) return err;
   if (c->profiling) cudaEventRecord(c->ev[1], c->stream);
-  k_finalize<<<c->E, kFinThreads, 0, c->stream>>>(c->partials, c->edges, c->poses, c->blocks35, c->edge_cost, c->n_valid,
-                                                  c->checksum, c->chunks * (kAccThreads / 32));
+  const int records = c->chunks * (kAccThreads / 32);
+  if (records >= 256 && c->E <= 600)
+    k_finalize<24><<<c->E, 24 * 40 + 16, 0, c->stream>>>(c->partials, c->edges, c->poses, c->blocks35, c->edge_cost, c->n_valid,
+                                                         c->checksum, records);
+  else
+    k_finalize<6><<<c->E, 6 * 40 + 16, 0, c->stream>>>(c->partials, c->edges, c->poses, c->blocks35, c->edge_cost, c->n_valid,
+                                                       c->checksum, records);
   c->launches += 3;
   return cudaGetLastError();
 }
