@@ -349,7 +349,10 @@ __device__ void bb_schur_row(const BBArgs& a, double* buf, int b) {
 }
 
 // ---- phase 3, border system of at most one tile (7 n_bord <= 64): unblocked Cholesky and both solves in shared memory
-// by CTA 0 (the tiled path costs two grid barriers and a 64-pivot tile for what is here a 14 x 14 system).
+// by CTA 0 (the tiled path costs two grid barriers and a 64-pivot tile for what is here a 14 x 14 .. 63 x 63 system).
+// One barrier per pivot: the trailing update reads the UNSCALED pivot column from the lower triangle
+// (a_rc -= a_rp a_cp / a_pp) while the scaled column L_rp = a_rp / sqrt(a_pp) is written to the mirror position in the
+// upper triangle, D[p][r]; the two triangular solves read L from there.
 __device__ void bb_small_border(const BBArgs& a, Smem& sm, int n7) {
   const int tid = threadIdx.x;
   const int nB = a.npadB;
@@ -358,39 +361,35 @@ __device__ void bb_small_border(const BBArgs& a, Smem& sm, int n7) {
     if (c <= r) sm.D[r * LDD + c] = __ldcg(a.B.L + (size_t)r * nB + c);
   }
   if (tid < n7) sm.y[tid] = __ldcg(a.B.rhs + tid);
-  if (tid == 0) sm.flag = 0;
   __syncthreads();
+  bool good = true;
+  const int ty = tid >> 4, tx = tid & 15;
   for (int p = 0; p < n7; ++p) {
-    const double piv = sm.D[p * LDD + p];
-    const bool gd = (piv > 0.0) && (piv < 1.0e300);
-    if (!gd) { if (tid == 0) sm.flag = 1; break; }             // uniform: everybody reads the same pivot
-    const double inv = rsqrt(piv);
-    __syncthreads();                                           // the pivot has been read by all
-    for (int r = p + tid; r < n7; r += kSolveThreads) sm.D[r * LDD + p] *= inv;
+    const double piv = sm.D[p * LDD + p];                      // everybody reads the same pivot: uniform control flow
+    if (!((piv > 0.0) && (piv < 1.0e300))) { good = false; break; }
+    const double inv = fast_rsqrt(piv), ipiv = inv * inv;
     if (tid == 0) sm.dinv[p] = inv;
-    __syncthreads();
-    const int m = n7 - p - 1;
-    for (int idx = tid; idx < m * m; idx += kSolveThreads) {
-      const int r = p + 1 + idx / m, c = p + 1 + idx % m;
-      if (c <= r) sm.D[r * LDD + c] = fma(-sm.D[r * LDD + p], sm.D[c * LDD + p], sm.D[r * LDD + c]);
+    for (int r = p + 1 + tid; r < n7; r += kSolveThreads) sm.D[p * LDD + r] = sm.D[r * LDD + p] * inv;   // L_rp, mirrored
+    for (int r = p + 1 + ty; r < n7; r += 16) {
+      const double arp = sm.D[r * LDD + p] * ipiv;
+      for (int c = p + 1 + tx; c <= r; c += 16) sm.D[r * LDD + c] = fma(-arp, sm.D[c * LDD + p], sm.D[r * LDD + c]);
     }
     __syncthreads();
   }
-  __syncthreads();
-  if (sm.flag) { if (tid == 0) a.status[0] = 1; return; }
-  if (tid < 32) {                                              // L y = b, then L^T x = y: lanes own rows tid, tid + 32
+  if (!good) { if (tid == 0) a.status[0] = 1; return; }
+  if (tid < 32) {                                              // L y = b, then L^T x = y: lanes own rows tid, tid + 32; L_rc = D[c][r]
     double b0 = tid < n7 ? sm.y[tid] : 0.0, b1 = tid + 32 < n7 ? sm.y[tid + 32] : 0.0;
     for (int c = 0; c < n7; ++c) {
       const double yc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * sm.dinv[c];
       if (tid == (c & 31)) { if (c < 32) b0 = yc; else b1 = yc; }
-      if (tid > c && tid < n7) b0 -= sm.D[tid * LDD + c] * yc;
-      if (tid + 32 > c && tid + 32 < n7) b1 -= sm.D[(tid + 32) * LDD + c] * yc;
+      if (tid > c && tid < n7) b0 -= sm.D[c * LDD + tid] * yc;
+      if (tid + 32 > c && tid + 32 < n7) b1 -= sm.D[c * LDD + tid + 32] * yc;
     }
     for (int c = n7 - 1; c >= 0; --c) {
       const double xc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * sm.dinv[c];
       if (tid == (c & 31)) { if (c < 32) b0 = xc; else b1 = xc; }
-      if (tid < c) b0 -= sm.D[c * LDD + tid] * xc;
-      if (tid + 32 < c) b1 -= sm.D[c * LDD + tid + 32] * xc;
+      if (tid < c) b0 -= sm.D[tid * LDD + c] * xc;
+      if (tid + 32 < c) b1 -= sm.D[(tid + 32) * LDD + c] * xc;
     }
     if (tid < n7) a.B.tau[tid] = b0;
     if (tid + 32 < n7) a.B.tau[tid + 32] = b1;
