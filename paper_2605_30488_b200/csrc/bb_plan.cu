@@ -19,21 +19,21 @@ namespace sim3ba {
 namespace {
 template <class T>
 cudaError_t up(T** dst, const std::vector<T>& src, cudaStream_t s) {
-  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(dst), std::max<size_t>(src.size(), 1) * sizeof(T));
+  cudaError_t e = dmalloc(reinterpret_cast<void**>(dst), std::max<size_t>(src.size(), 1) * sizeof(T));
   if (e != cudaSuccess || src.empty()) return e;
   return cudaMemcpyAsync(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice, s);
 }
 template <class T>
 cudaError_t dalloc(T** p, size_t count) {
-  return cudaMalloc(reinterpret_cast<void**>(p), std::max<size_t>(count, 1) * sizeof(T));
+  return dmalloc(reinterpret_cast<void**>(p), std::max<size_t>(count, 1) * sizeof(T));
 }
 }  // namespace
 
 void free_bb_plan(BBPlan& p) {
-  cudaFree(p.seg_ptr); cudaFree(p.seg_bptr); cudaFree(p.seg_bord); cudaFree(p.col_kf); cudaFree(p.col_nb); cudaFree(p.col_ofs);
-  cudaFree(p.col_band); cudaFree(p.col_bpair); cudaFree(p.col_bofs); cudaFree(p.bord_kf); cudaFree(p.bord_sptr);
-  cudaFree(p.bord_seg); cudaFree(p.bord_slot); cudaFree(p.bb_pair); cudaFree(p.colbuf); cudaFree(p.seg_rhs);
-  cudaFree(p.LB); cudaFree(p.rhsB); cudaFree(p.ysolB); cudaFree(p.DinvB); cudaFree(p.tauB);
+  dfree(p.seg_ptr); dfree(p.seg_bptr); dfree(p.seg_bord); dfree(p.col_kf); dfree(p.col_nb); dfree(p.col_ofs);
+  dfree(p.col_band); dfree(p.col_bpair); dfree(p.col_bofs); dfree(p.bord_kf); dfree(p.bord_sptr);
+  dfree(p.bord_seg); dfree(p.bord_slot); dfree(p.bb_pair); dfree(p.colbuf); dfree(p.seg_rhs);
+  dfree(p.LB); dfree(p.rhsB); dfree(p.ysolB); dfree(p.DinvB); dfree(p.tauB);
   free_plan(p.dense);
   p = BBPlan();
 }

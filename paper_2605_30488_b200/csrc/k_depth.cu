@@ -194,7 +194,7 @@ __global__ void k_depth_apply(const float* __restrict__ pts, const float* __rest
 
 template <class T>
 cudaError_t up(T** dst, const std::vector<T>& src, cudaStream_t s) {
-  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(dst), std::max<size_t>(src.size(), 1) * sizeof(T));
+  cudaError_t e = dmalloc(reinterpret_cast<void**>(dst), std::max<size_t>(src.size(), 1) * sizeof(T));
   if (e != cudaSuccess || src.empty()) return e;
   return cudaMemcpyAsync(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice, s);
 }
@@ -230,9 +230,9 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
   auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return e == cudaSuccess; };
   ok(up(&d_sp_ptr, sp_ptr, c->stream)); ok(up(&d_sp_other, sp_other, c->stream)); ok(up(&d_sp_delta, sp_delta, c->stream));
   ok(up(&d_pairs, pairs, c->stream)); ok(up(&d_delta, delta, c->stream)); ok(up(&d_anchor, anchor, c->stream));
-  ok(cudaMalloc(reinterpret_cast<void**>(&d_partial), std::max<size_t>((size_t)c->E * tiles * rec, 1) * sizeof(double)));
-  ok(cudaMalloc(reinterpret_cast<void**>(&d_eta2), std::max<size_t>(n_total, 1) * sizeof(double)));
-  ok(cudaMalloc(reinterpret_cast<void**>(&d_cost), std::max(n_iters, 1) * sizeof(double)));
+  ok(dmalloc(reinterpret_cast<void**>(&d_partial), std::max<size_t>((size_t)c->E * tiles * rec, 1) * sizeof(double)));
+  ok(dmalloc(reinterpret_cast<void**>(&d_eta2), std::max<size_t>(n_total, 1) * sizeof(double)));
+  ok(dmalloc(reinterpret_cast<void**>(&d_cost), std::max(n_iters, 1) * sizeof(double)));
   double *cur = d_eta, *nxt = d_eta2;
   for (int it = 0; it < n_iters && e == cudaSuccess; ++it) {
     if (c->E > 0)
@@ -249,8 +249,8 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
   if (e == cudaSuccess && h_cost && n_iters > 0) ok(cudaMemcpyAsync(h_cost, d_cost, (size_t)n_iters * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   cudaError_t es = cudaStreamSynchronize(c->stream);          // the host vectors and temporaries go out of scope
   if (e == cudaSuccess) e = es;
-  cudaFree(d_sp_ptr); cudaFree(d_sp_other); cudaFree(d_sp_delta); cudaFree(d_pairs); cudaFree(d_delta); cudaFree(d_anchor);
-  cudaFree(d_partial); cudaFree(d_eta2); cudaFree(d_cost);
+  dfree(d_sp_ptr); dfree(d_sp_other); dfree(d_sp_delta); dfree(d_pairs); dfree(d_delta); dfree(d_anchor);
+  dfree(d_partial); dfree(d_eta2); dfree(d_cost);
   return e;
 }
 

@@ -38,7 +38,7 @@ int cuda_fail(Ctx* c, cudaError_t e, const char* what) {
 
 template <class T>
 cudaError_t dev_alloc(T** p, size_t count) {
-  return cudaMalloc(reinterpret_cast<void**>(p), std::max<size_t>(count, 1) * sizeof(T));
+  return dmalloc(reinterpret_cast<void**>(p), std::max<size_t>(count, 1) * sizeof(T));
 }
 
 bool params_ok(const sim3ba_params* p) {
@@ -86,12 +86,12 @@ cudaError_t upload(T** dst, const std::vector<T>& src, cudaStream_t s) {
 }
 
 void free_all(Ctx* c) {
-  cudaFree(c->pm); cudaFree(c->edges); cudaFree(c->grp_kf); cudaFree(c->grp_ptr); cudaFree(c->grp_edge); cudaFree(c->edgeT); cudaFree(c->fixed_mask); cudaFree(c->poses);
-  cudaFree(c->kf_ptr); cudaFree(c->kf_edge); cudaFree(c->pair_kf); cudaFree(c->pair_ptr); cudaFree(c->pair_edge);
-  cudaFree(c->partials); cudaFree(c->blocks35); cudaFree(c->edge_cost); cudaFree(c->n_valid); cudaFree(c->checksum);
-  cudaFree(c->Hd); cudaFree(c->L); cudaFree(c->g); cudaFree(c->rhs); cudaFree(c->ysol); cudaFree(c->Dinv); cudaFree(c->pairhi_ptr);
+  dfree(c->pm); dfree(c->edges); dfree(c->grp_kf); dfree(c->grp_ptr); dfree(c->grp_edge); dfree(c->edgeT); dfree(c->fixed_mask); dfree(c->poses);
+  dfree(c->kf_ptr); dfree(c->kf_edge); dfree(c->pair_kf); dfree(c->pair_ptr); dfree(c->pair_edge);
+  dfree(c->partials); dfree(c->blocks35); dfree(c->edge_cost); dfree(c->n_valid); dfree(c->checksum);
+  dfree(c->Hd); dfree(c->L); dfree(c->g); dfree(c->rhs); dfree(c->ysol); dfree(c->Dinv); dfree(c->pairhi_ptr);
   free_plan(c->plan_sparse); free_plan(c->plan_dense); free_bb_plan(c->plan_bb);
-  cudaFree(c->tau); cudaFree(c->total_cost); cudaFree(c->fail_flag); cudaFree(c->d_eps_used); cudaFree(c->bar);
+  dfree(c->tau); dfree(c->total_cost); dfree(c->fail_flag); dfree(c->d_eps_used); dfree(c->bar);
   if (c->h_flag) cudaFreeHost(c->h_flag);
   if (c->h_scalar) cudaFreeHost(c->h_scalar);
   for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
@@ -162,6 +162,7 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
   cudaError_t de = cudaGetDeviceCount(&ndev);
   if (de != cudaSuccess || ndev == 0) return fail(c, SIM3BA_ERR_CUDA, "no CUDA device (libsim3ba has no CPU fallback)");
 
+  tl_stream = (cudaStream_t)cuda_stream;
   sim3ba_ctx* h = new (std::nothrow) sim3ba_ctx();
   if (!h) return fail(c, SIM3BA_ERR_ALLOC, "host allocation failed");
   c = &h->c;
@@ -274,6 +275,7 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
 
 int sim3ba_destroy(sim3ba_ctx* h) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
+  tl_stream = h->c.stream;
   cudaStreamSynchronize(h->c.stream);
   free_all(&h->c);
   delete h;
@@ -283,6 +285,7 @@ int sim3ba_destroy(sim3ba_ctx* h) {
 int sim3ba_set_params(sim3ba_ctx* h, const sim3ba_params* p) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (!params_ok(p)) return fail(c, SIM3BA_ERR_INVALID_ARG, "invalid params");
   if (p->conf_min != c->prm.conf_min)
     return fail(c, SIM3BA_ERR_INVALID_ARG, "conf_min is fixed at sim3ba_create (the validity mask is baked into the packed pointmap)");
@@ -293,6 +296,7 @@ int sim3ba_set_params(sim3ba_ctx* h, const sim3ba_params* p) {
 int sim3ba_set_poses(sim3ba_ctx* h, const double* d_poses) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (!d_poses) return fail(c, SIM3BA_ERR_INVALID_ARG, "d_poses is NULL");
   CU(cudaMemcpyAsync(c->poses, d_poses, (size_t)8 * c->N * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
   return SIM3BA_OK;
@@ -301,6 +305,7 @@ int sim3ba_set_poses(sim3ba_ctx* h, const double* d_poses) {
 int sim3ba_get_poses(sim3ba_ctx* h, double* d_poses) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (!d_poses) return fail(c, SIM3BA_ERR_INVALID_ARG, "d_poses is NULL");
   CU(cudaMemcpyAsync(d_poses, c->poses, (size_t)8 * c->N * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
   return SIM3BA_OK;
@@ -309,6 +314,7 @@ int sim3ba_get_poses(sim3ba_ctx* h, double* d_poses) {
 int sim3ba_build_system(sim3ba_ctx* h) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   int rc = build_blocks(c);
   if (rc) return rc;
   CU(launch_assemble(c, c->Hd, 0.0, 0.0, false));
@@ -327,6 +333,7 @@ int sim3ba_build_system(sim3ba_ctx* h) {
 int sim3ba_solve(sim3ba_ctx* h) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (!c->built && !c->dense_loaded) return fail(c, SIM3BA_ERR_BAD_STATE, "sim3ba_solve before sim3ba_build_system");
   return solve_impl(c);
 }
@@ -334,6 +341,7 @@ int sim3ba_solve(sim3ba_ctx* h) {
 int sim3ba_retract(sim3ba_ctx* h) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (!c->solved) return fail(c, SIM3BA_ERR_BAD_STATE, "sim3ba_retract before sim3ba_solve");
   CU(launch_retract(c));
   c->built = false; c->solved = false;
@@ -343,6 +351,7 @@ int sim3ba_retract(sim3ba_ctx* h) {
 int sim3ba_step(sim3ba_ctx* h) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   int rc = build_blocks(c);
   if (rc) return rc;
   c->hd_valid = false;
@@ -366,6 +375,7 @@ int sim3ba_step(sim3ba_ctx* h) {
 int sim3ba_step_host(sim3ba_ctx* h, const double* h_in, double* h_out, double* h_cost) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   const size_t bytes = (size_t)8 * c->N * sizeof(double);
   if (h_in) CU(cudaMemcpyAsync(c->poses, h_in, bytes, cudaMemcpyHostToDevice, c->stream));
   int rc = sim3ba_step(h);
@@ -386,6 +396,7 @@ int sim3ba_optimize_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_
   if (!h_points || !h_conf || (n_edges > 0 && (!h_edges || !h_match)) || !h_poses_in || !h_poses_out)
     return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL host pointer");
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  tl_stream = st;
   const size_t NHW = (size_t)n_kf * height * width, EHW = (size_t)n_edges * height * width;
   float *d_points = nullptr, *d_conf = nullptr;
   int32_t *d_edges = nullptr, *d_match = nullptr;
@@ -446,6 +457,7 @@ int sim3ba_gauge_sync(sim3ba_ctx* h, int32_t edge, const int32_t* h_moving_kf, i
                       int32_t n_c_min, double* h_T, int32_t* h_n_c, int32_t* h_fallback) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (edge < 0 || edge >= c->E) return fail(c, SIM3BA_ERR_INVALID_ARG, "edge index out of range");
   if (n_moving < 0 || (n_moving > 0 && !h_moving_kf) || n_c_min < 1) return fail(c, SIM3BA_ERR_INVALID_ARG, "bad moving list or n_c_min");
   for (int k = 0; k < n_moving; ++k)
@@ -462,8 +474,8 @@ int sim3ba_gauge_sync(sim3ba_ctx* h, int32_t edge, const int32_t* h_moving_kf, i
   if (e == cudaSuccess)
     e = cudaMemcpyAsync(res, d_work + (size_t)gauge_sync_work_doubles(grid) - 10, sizeof(res), cudaMemcpyDeviceToHost, c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // also keeps h_moving_kf / the temporaries alive long enough
-  cudaFree(d_work);
-  cudaFree(d_moving);
+  dfree(d_work);
+  dfree(d_moving);
   if (e != cudaSuccess) return cuda_fail(c, e, "sim3ba_gauge_sync");
   if (h_T) memcpy(h_T, res, 8 * sizeof(double));
   if (h_n_c) *h_n_c = (int32_t)res[8];
@@ -483,6 +495,7 @@ int sim3ba_depth_refine(sim3ba_ctx* h, const int32_t* d_labels, int32_t n_seg, c
                         double* d_eta, double* h_cost) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (!d_labels || !d_eta || !p || n_seg < 1 || n_seg > depth_max_segments() || n_iters < 0 || n_pairs < 0 || n_anchor < 0 ||
       (n_pairs > 0 && (!h_pairs || !h_delta)) || (n_anchor > 0 && !h_anchor_kf))
     return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL pointer, or n_seg outside 1..64, or a negative count");
@@ -502,6 +515,7 @@ int sim3ba_apply_depth(sim3ba_ctx* h, const float* d_points, const float* d_conf
                        const double* d_eta) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (!d_points || !d_conf || !d_labels || !d_eta || n_seg < 1) return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL pointer or n_seg < 1");
   CU(launch_depth_apply(c, d_points, d_conf, d_labels, n_seg, d_eta));
   c->built = false; c->solved = false;   // the pointmaps changed
@@ -511,6 +525,7 @@ int sim3ba_apply_depth(sim3ba_ctx* h, const float* d_points, const float* d_conf
 int sim3ba_get_edge_stats(sim3ba_ctx* h, const int32_t** nv, const uint64_t** chk, const double** cost) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (nv) *nv = c->n_valid;
   if (chk) *chk = reinterpret_cast<const uint64_t*>(c->checksum);
   if (cost) *cost = c->edge_cost;
@@ -526,6 +541,7 @@ int sim3ba_get_edge_blocks(sim3ba_ctx* h, const double** b) {
 int sim3ba_get_system(sim3ba_ctx* h, const double** H, int32_t* ld, const double** g) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (!c->hd_valid) return fail(c, SIM3BA_ERR_BAD_STATE, "no dense system: call sim3ba_build_system first");
   if (H) *H = c->Hd;
   if (ld) *ld = c->npad;
@@ -536,6 +552,7 @@ int sim3ba_get_system(sim3ba_ctx* h, const double** H, int32_t* ld, const double
 int sim3ba_get_update(sim3ba_ctx* h, const double** tau, int32_t* attempts, double* eps_used, double* cost) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (tau) *tau = c->tau;
   if (attempts || eps_used) {
     int rc = fetch_status(c);
@@ -555,6 +572,7 @@ int sim3ba_get_bookkeeping(sim3ba_ctx* h, const int32_t** kf_ptr, const int32_t*
                            const int32_t** pair_kf, const int32_t** pair_ptr, const int32_t** pair_edge) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (kf_ptr) *kf_ptr = c->h_kf_ptr.data();
   if (kf_edge) *kf_edge = c->h_kf_edge.data();
   if (n_pairs) *n_pairs = c->n_pairs;
@@ -567,6 +585,7 @@ int sim3ba_get_bookkeeping(sim3ba_ctx* h, const int32_t** kf_ptr, const int32_t*
 int sim3ba_load_system(sim3ba_ctx* h, const double* d_H, const double* d_g) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (!d_H || !d_g) return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL system pointer");
   CU(cudaMemcpyAsync(c->Hd, d_H, (size_t)c->n * c->n * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
   CU(launch_load_gradient(c, d_g));
@@ -577,6 +596,7 @@ int sim3ba_load_system(sim3ba_ctx* h, const double* d_H, const double* d_g) {
 int sim3ba_set_solver_mode(sim3ba_ctx* h, int32_t mode) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (mode < 0 || mode > 2) return fail(c, SIM3BA_ERR_INVALID_ARG, "solver mode must be 0 (tile-sparse), 1 (dense) or 2 (band + border)");
   c->solver_mode = mode;
   return SIM3BA_OK;
@@ -585,6 +605,7 @@ int sim3ba_set_solver_mode(sim3ba_ctx* h, int32_t mode) {
 int sim3ba_get_solver_info(sim3ba_ctx* h, int32_t* n_tiles, int32_t* n_tiles_dense, double* flops, int32_t* grid) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   const bool dense = c->solver_mode == 1;
   SolvePlan& plan = dense ? c->plan_dense : c->plan_sparse;
   if (!plan.ready) {
@@ -627,6 +648,7 @@ int sim3ba_get_phase_ms(sim3ba_ctx* h, float ms[8]) {
 int sim3ba_copy_d2d(sim3ba_ctx* h, void* dst, const void* src, uint64_t bytes) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
+  tl_stream = c->stream;
   if (bytes == 0) return SIM3BA_OK;
   if (!dst || !src) return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL pointer in sim3ba_copy_d2d");
   CU(cudaMemcpyAsync(dst, src, (size_t)bytes, cudaMemcpyDeviceToDevice, c->stream));

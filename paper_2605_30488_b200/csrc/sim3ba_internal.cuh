@@ -11,6 +11,13 @@
 
 namespace sim3ba {
 
+// Device memory of the library comes from the device's stream-ordered pool on the stream of the running API call
+// (set on entry of every entry point that may allocate or free): no device-wide synchronisation per allocation, and
+// a caller that keeps the pool warm (sim3ba_optimize_host does) pays no map / unmap per context.
+inline thread_local cudaStream_t tl_stream = nullptr;
+inline cudaError_t dmalloc(void** p, size_t bytes) { return cudaMallocAsync(p, bytes < 16 ? 16 : bytes, tl_stream); }
+inline void dfree(void* p) { if (p) cudaFreeAsync(p, tl_stream); }
+
 constexpr int kAccThreads = 32;      // accumulate CTA: ONE warp -- warps are independent workers, so the finest CTA gives the block
                                      // scheduler the finest grain (a two-warp CTA holds its slot until the slower warp is done)
 constexpr int kTilePx = 16 * kAccThreads;   // pixels of a keyframe handled by one accumulate CTA (512 contiguous per warp)

@@ -13,14 +13,14 @@ namespace sim3ba {
 namespace {
 template <class T>
 cudaError_t up(T** dst, const std::vector<T>& src, cudaStream_t s) {
-  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(dst), std::max<size_t>(src.size(), 1) * sizeof(T));
+  cudaError_t e = dmalloc(reinterpret_cast<void**>(dst), std::max<size_t>(src.size(), 1) * sizeof(T));
   if (e != cudaSuccess || src.empty()) return e;
   return cudaMemcpyAsync(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice, s);
 }
 }  // namespace
 
 void free_plan(SolvePlan& p) {
-  cudaFree(p.col_ptr); cudaFree(p.col_rows); cudaFree(p.row_ptr); cudaFree(p.row_cols); cudaFree(p.tiles);
+  dfree(p.col_ptr); dfree(p.col_rows); dfree(p.row_ptr); dfree(p.row_cols); dfree(p.tiles);
   p = SolvePlan();
 }
 
