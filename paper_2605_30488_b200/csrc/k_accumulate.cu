@@ -8,12 +8,12 @@
 //   PAPER.md:118           J_j = J_xi Ad_{T_i^-1}, J_i = -J_j  ->  the adjoint is applied once per
 //                          edge:  A_e = Ad^T (sum J_xi^T Omega J_xi) Ad,  b_e = Ad^T (sum J_xi^T Omega e)
 //
-// Work decomposition: one CTA per (keyframe i, tile of 3072 pixels of i), 192 threads,
-// two CTAs per SM.  The tile of X_i is staged in shared memory ONCE by a TMA bulk copy (cp.async.bulk +
-// mbarrier) and reused by every edge (i, j) that leaves i; per edge the match indices are streamed
-// (coalesced, evict-first) and X_j is gathered (128-bit loads), software-pipelined one pair ahead.
-// Every thread evaluates TWO matches at a time in the two lanes of packed fp32x2 instructions
-// (FFMA2 / FMUL2 / FADD2: one issue slot per two lanes), accumulators included.
+// Work decomposition: one warp = one CTA = one (keyframe i, slice of 512 pixels of i), 14-15 CTAs per
+// SM.  The slice of X_i is staged in shared memory ONCE by a TMA bulk copy (cp.async.bulk + mbarrier) and reused by every
+// edge (i, j) that leaves i; per edge the match indices arrive by a TMA bulk copy one edge ahead, X_j is gathered by
+// per-lane cp.async into a two-slot ring one pair ahead of the arithmetic.  Every thread evaluates TWO matches at a time
+// in the two lanes of packed fp32x2 instructions (FFMA2 / FMUL2 / FADD2: one issue slot per two lanes), accumulators
+// included.
 //
 // Precision plan: delta = T_ij X_j - X_i in FP64 (the one cancellation of the residual); everything
 // after it, the per-thread partial sums (<= 8 terms per lane, 16 per thread) and the first two levels of
