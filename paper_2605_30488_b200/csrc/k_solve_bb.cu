@@ -348,51 +348,98 @@ __device__ void bb_schur_row(const BBArgs& a, double* buf, int b) {
   }
 }
 
-// ---- phase 3, border system of at most one tile (7 n_bord <= 64): unblocked Cholesky and both solves in shared memory
+// ---- phase 3, border system of at most one tile (7 n_bord <= 64): unblocked LDL^T and both solves in shared memory
 // by CTA 0 (the tiled path costs two grid barriers and a 64-pivot tile for what is here a 14 x 14 .. 63 x 63 system).
-// One barrier per pivot: the trailing update reads the UNSCALED pivot column from the lower triangle
-// (a_rc -= a_rp a_cp / a_pp) while the scaled column L_rp = a_rp / sqrt(a_pp) is written to the mirror position in the
-// upper triangle, D[p][r]; the two triangular solves read L from there.
+// S = L~ D L~^T with l_rc = a_rc / d_c: column c of the lower triangle keeps the UNSCALED a_rc (nothing touches it after
+// pivot c), so there is no square root and no scaling pass.  One barrier per pivot, and the pivot chain is taken off
+// the update: thread 0 alone produces d_{p+1} and 1 / d_{p+1} (its Newton chain) while warps 2..7 apply pivot p to the
+// rest of the trailing matrix and warp 1 takes column p of the forward solve.  1 / d = 0 marks a pivot that is <= 0 or not finite.
+__device__ __forceinline__ double fast_rcp(double p) {
+  const float pf = (float)p;
+  if (!(pf > 1e-30f && pf < 1e30f)) return 1.0 / p;
+  float rf;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rf) : "f"(pf));
+  double y = (double)rf;
+  double e = fma(-p, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-p, y, 1.0);
+  y = fma(y, e, y);
+  return y;
+}
+
 __device__ void bb_small_border(const BBArgs& a, Smem& sm, int n7) {
   const int tid = threadIdx.x;
   const int nB = a.npadB;
+  double* ipv = sm.red;                                        // [n7] 1 / d_p
   for (int idx = tid; idx < n7 * n7; idx += kSolveThreads) {
     const int r = idx / n7, c = idx - r * n7;
     if (c <= r) sm.D[r * LDD + c] = __ldcg(a.B.L + (size_t)r * nB + c);
   }
   if (tid < n7) sm.y[tid] = __ldcg(a.B.rhs + tid);
   __syncthreads();
+  if (tid == 0) {
+    const double d0 = sm.D[0];
+    ipv[0] = ((d0 > 0.0) && (d0 < 1.0e300)) ? fast_rcp(d0) : 0.0;
+  }
+  __syncthreads();
   bool good = true;
-  const int ty = tid >> 4, tx = tid & 15;
+  constexpr int kRows = (kSolveThreads - 64) / 16;             // update threads: warps 2.., kRows x 16
+  constexpr int kRowIt = (NB + kRows - 1) / kRows, kColIt = NB / 16;
+  const int ty = (tid - 64) >> 4, tx = tid & 15;
+  const int lane = tid & 31;
+  // warp 1 carries the forward solve L~ y = b one column per pivot, as z_c = y_c / d_c (b_r -= a_rc z_c): lanes own rows
+  // lane, lane + 32
+  double b0 = 0.0, b1 = 0.0;
+  if (tid >= 32 && tid < 64) { b0 = lane < n7 ? sm.y[lane] : 0.0; b1 = lane + 32 < n7 ? sm.y[lane + 32] : 0.0; }
   for (int p = 0; p < n7; ++p) {
-    const double piv = sm.D[p * LDD + p];                      // everybody reads the same pivot: uniform control flow
-    if (!((piv > 0.0) && (piv < 1.0e300))) { good = false; break; }
-    const double inv = fast_rsqrt(piv), ipiv = inv * inv;
-    if (tid == 0) sm.dinv[p] = inv;
-    for (int r = p + 1 + tid; r < n7; r += kSolveThreads) sm.D[p * LDD + r] = sm.D[r * LDD + p] * inv;   // L_rp, mirrored
-    for (int r = p + 1 + ty; r < n7; r += 16) {
-      const double arp = sm.D[r * LDD + p] * ipiv;
-      for (int c = p + 1 + tx; c <= r; c += 16) sm.D[r * LDD + c] = fma(-arp, sm.D[c * LDD + p], sm.D[r * LDD + c]);
+    const double ipiv = ipv[p];                                // everybody reads the same value: uniform control flow
+    if (ipiv == 0.0) { good = false; break; }
+    if (tid == 0) {
+      if (p + 1 < n7) {                                        // the next pivot, one step ahead of its row
+        const double ap = sm.D[(p + 1) * LDD + p];
+        const double d = fma(-(ap * ipiv), ap, sm.D[(p + 1) * LDD + p + 1]);
+        sm.D[(p + 1) * LDD + p + 1] = d;
+        ipv[p + 1] = ((d > 0.0) && (d < 1.0e300)) ? fast_rcp(d) : 0.0;
+      }
+    } else if (tid >= 64) {                                    // all loads of a thread are independent: fully unrolled
+      double lc[kColIt];
+#pragma unroll
+      for (int j = 0; j < kColIt; ++j) {
+        const int c = p + 1 + tx + 16 * j;
+        lc[j] = c < n7 ? sm.D[c * LDD + p] : 0.0;
+      }
+#pragma unroll
+      for (int i = 0; i < kRowIt; ++i) {
+        const int r = p + 1 + ty + kRows * i;
+        if (r > p + 1 && r < n7) {                             // row p + 1 is its diagonal only: thread 0's
+          const double arp = sm.D[r * LDD + p] * ipiv;
+#pragma unroll
+          for (int j = 0; j < kColIt; ++j) {
+            const int c = p + 1 + tx + 16 * j;
+            if (c <= r) sm.D[r * LDD + c] = fma(-arp, lc[j], sm.D[r * LDD + c]);
+          }
+        }
+      }
+    } else if (tid >= 32) {
+      const double zc = __shfl_sync(0xffffffffu, p < 32 ? b0 * ipiv : b1 * ipiv, p & 31);
+      if (lane == (p & 31)) { if (p < 32) b0 = zc; else b1 = zc; }
+      if (lane > p && lane < n7) b0 = fma(-sm.D[lane * LDD + p], zc, b0);
+      if (lane + 32 > p && lane + 32 < n7) b1 = fma(-sm.D[(lane + 32) * LDD + p], zc, b1);
     }
     __syncthreads();
   }
   if (!good) { if (tid == 0) a.status[0] = 1; return; }
-  if (tid < 32) {                                              // L y = b, then L^T x = y: lanes own rows tid, tid + 32; L_rc = D[c][r]
-    double b0 = tid < n7 ? sm.y[tid] : 0.0, b1 = tid + 32 < n7 ? sm.y[tid + 32] : 0.0;
-    for (int c = 0; c < n7; ++c) {
-      const double yc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * sm.dinv[c];
-      if (tid == (c & 31)) { if (c < 32) b0 = yc; else b1 = yc; }
-      if (tid > c && tid < n7) b0 -= sm.D[c * LDD + tid] * yc;
-      if (tid + 32 > c && tid + 32 < n7) b1 -= sm.D[c * LDD + tid + 32] * yc;
-    }
+  if (tid >= 32 && tid < 64) {
+    const double i0 = lane < n7 ? ipv[lane] : 0.0, i1 = lane + 32 < n7 ? ipv[lane + 32] : 0.0;
+    double s0 = 0.0, s1 = 0.0;                                 // L~^T x = z: x_c = z_c - (1 / d_c) sum_{r > c} a_rc x_r
     for (int c = n7 - 1; c >= 0; --c) {
-      const double xc = __shfl_sync(0xffffffffu, c < 32 ? b0 : b1, c & 31) * sm.dinv[c];
-      if (tid == (c & 31)) { if (c < 32) b0 = xc; else b1 = xc; }
-      if (tid < c) b0 -= sm.D[tid * LDD + c] * xc;
-      if (tid + 32 < c) b1 -= sm.D[(tid + 32) * LDD + c] * xc;
+      const double xc = __shfl_sync(0xffffffffu, c < 32 ? fma(-i0, s0, b0) : fma(-i1, s1, b1), c & 31);
+      if (lane == (c & 31)) { if (c < 32) b0 = xc; else b1 = xc; }
+      if (lane < c) s0 = fma(sm.D[c * LDD + lane], xc, s0);
+      if (lane + 32 < c) s1 = fma(sm.D[c * LDD + lane + 32], xc, s1);
     }
-    if (tid < n7) a.B.tau[tid] = b0;
-    if (tid + 32 < n7) a.B.tau[tid + 32] = b1;
+    if (lane < n7) a.B.tau[lane] = b0;
+    if (lane + 32 < n7) a.B.tau[lane + 32] = b1;
   }
   __syncthreads();
 }
@@ -520,7 +567,7 @@ k_solve_bb(BBArgs a) {
       grid_barrier(a.bar, G, gen);   // everybody has seen the flag before it is cleared again
       continue;
     }
-    grid_barrier(a.bar, G, gen);     // tau_B is final
+    if (nbB != 1) grid_barrier(a.bar, G, gen);     // tau_B is final (the one-tile path has just passed a barrier)
     BB_STAMP(5);
     {
       double* ring = win;
