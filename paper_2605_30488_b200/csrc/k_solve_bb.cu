@@ -615,9 +615,10 @@ cudaError_t launch_solve_bb(Ctx* c) {
     smem_set = smem;
   }
   const SolvePlan& D = P.dense;
-  // enough CTAs for the widest phase: a few block columns each in the assembly, one per segment / border keyframe / tile task
+  // enough CTAs for the widest phase: one block column each in the assembly (its loads are a chain of L2 round trips),
+  // one per segment / border keyframe / tile task
   long long want = std::max<long long>({(long long)P.n_seg, (long long)P.n_bord, (long long)D.max_upd, (long long)D.max_col,
-                                        (long long)(P.n_int + 3) / 4, 1LL});
+                                        (long long)P.n_int, 1LL});
   const int G = (int)std::min<long long>(want, (long long)num_sms * std::min(max_blocks_per_sm, 1));
   BBArgs a{};
   a.blocks35 = c->blocks35; a.g = c->g; a.kf_ptr = c->kf_ptr; a.kf_edge = c->kf_edge; a.pair_ptr = c->pair_ptr; a.pair_edge = c->pair_edge;
