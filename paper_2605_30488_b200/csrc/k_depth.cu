@@ -27,6 +27,10 @@ namespace {
 constexpr int kDpThreads = 256;
 constexpr int kDpWarps = kDpThreads / 32;
 constexpr int kDpMaxSeg = 64;
+#ifndef SIM3BA_DP_TILE_PX
+#define SIM3BA_DP_TILE_PX 8192
+#endif
+constexpr int kDpTilePx = SIM3BA_DP_TILE_PX;
 
 struct DepthDev {
   double inv_sigma, huber_k, lambda_smooth, lambda_prior, lambda_lm, eta_max;
@@ -51,14 +55,16 @@ __device__ __forceinline__ void bin_by_label(double* bins, bool valid, int label
   }
 }
 
-__global__ void __launch_bounds__(kDpThreads)
+__global__ void __launch_bounds__(kDpThreads, 3)
 k_depth_edge(const float4* __restrict__ pm, const int32_t* __restrict__ match, const int32_t* __restrict__ edges,
-             const int32_t* __restrict__ labels, const double* __restrict__ eta, const double* __restrict__ poses, int HW,
+             const int32_t* __restrict__ grp_edge, int E, const int32_t* __restrict__ labels, const double* __restrict__ eta, const double* __restrict__ poses, int HW,
              int n_seg, int tiles, DepthDev prm, double* __restrict__ partial) {
   __shared__ double s_bins[kDpWarps][2][kDpMaxSeg][2];
   __shared__ double s_exp[2][kDpMaxSeg];
   __shared__ double s_cost[kDpWarps];
-  const int e = blockIdx.x / tiles, tile = blockIdx.x - e * tiles;
+  // tile-major launch order over the edges sorted by (i, j): the CTAs in flight work on the same pixel range of
+  // neighbouring keyframes, so the tiles of X_i, X_j and of the labels are fetched from HBM once and shared through L2
+  const int tile = blockIdx.x / E, e = grp_edge[blockIdx.x - tile * E];
   const int i = edges[2 * e], j = edges[2 * e + 1];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   for (int q = tid; q < kDpWarps * 2 * kDpMaxSeg * 2; q += kDpThreads) (&s_bins[0][0][0][0])[q] = 0.0;
@@ -112,7 +118,7 @@ k_depth_edge(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
   cost = warp_sum(cost);
   if (lane == 0) s_cost[warp] = cost;
   __syncthreads();
-  double* out = partial + (size_t)blockIdx.x * (4 * n_seg + 1);
+  double* out = partial + ((size_t)e * tiles + tile) * (4 * n_seg + 1);
   for (int q = tid; q < 4 * n_seg; q += kDpThreads) {          // q = (side, label, {g, H})
     const int side = q / (2 * n_seg), rest = q - side * 2 * n_seg;
     double v = 0.0;
@@ -205,7 +211,9 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
                              const int32_t* h_anchor, int n_anchor, const sim3ba_depth_params& p, int n_iters, double* d_eta,
                              double* h_cost) {
   const int n_total = c->N * n_seg;
-  const int tiles = std::max(1, std::min(16, (592 + std::max(c->E, 1) - 1) / std::max(c->E, 1)));
+  // tiles of ~kDpTilePx pixels (the per-CTA setup is ~2000 shared-memory words), at least ~4 CTAs per SM in the grid
+  const int E1 = std::max(c->E, 1);
+  const int tiles = std::max(1, std::min(std::max((c->HW + kDpTilePx - 1) / kDpTilePx, (592 + E1 - 1) / E1), std::max(c->HW / 256, 1)));
   const int rec = 4 * n_seg + 1;
   DepthDev dev{1.0 / (double)p.sigma_point, (double)p.huber_k, p.lambda_smooth, p.lambda_prior, p.lambda_lm, p.eta_max};
   // segment -> boundary pairs CSR (host), the sign of Delta folded in: d = eta_s - eta_other + delta'
@@ -236,7 +244,7 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
   double *cur = d_eta, *nxt = d_eta2;
   for (int it = 0; it < n_iters && e == cudaSuccess; ++it) {
     if (c->E > 0)
-      k_depth_edge<<<c->E * tiles, kDpThreads, 0, c->stream>>>(c->pm, c->match, c->edges, d_labels, cur, c->poses, c->HW, n_seg, tiles, dev,
+      k_depth_edge<<<c->E * tiles, kDpThreads, 0, c->stream>>>(c->pm, c->match, c->edges, c->grp_edge, c->E, d_labels, cur, c->poses, c->HW, n_seg, tiles, dev,
                                                               d_partial);
     k_depth_cost<<<1, 256, 0, c->stream>>>(d_partial, c->E * tiles, rec, cur, n_total, d_pairs, d_delta, n_pairs, dev, d_cost + it);
     k_depth_update<<<(n_total + 127) / 128, 128, 0, c->stream>>>(d_partial, cur, nxt, c->edges, c->kf_ptr, c->kf_edge, d_sp_ptr, d_sp_other,
