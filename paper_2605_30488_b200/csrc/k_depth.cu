@@ -42,9 +42,15 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// add (a, b) of the lanes with `valid` into bins[label][0..1], label by label (deterministic: butterfly sums)
+// add (a, b) of the lanes with `valid` into bins[label][0..1] (deterministic).  A lane whose label no other valid lane
+// of the warp carries (an outlier match landing in some far segment) adds straight to the bin -- distinct labels, so these
+// adds do not meet; the labels shared by several lanes go label by label: butterfly sum of the lanes carrying it, lane 0
+// adds.  The usual warp (one segment, a few stray matches) takes one butterfly round instead of one per stray lane.
 __device__ __forceinline__ void bin_by_label(double* bins, bool valid, int label, double a, double b, int lane) {
-  unsigned active = __ballot_sync(0xffffffffu, valid);
+  const unsigned peers = __match_any_sync(0xffffffffu, valid ? label : -1 - lane);   // invalid lanes: unique keys
+  const bool single = valid && peers == (1u << lane);
+  if (single) { bins[2 * label] += a; bins[2 * label + 1] += b; }
+  unsigned active = __ballot_sync(0xffffffffu, valid && !single);
   while (active) {
     const int leader = __ffs(active) - 1;
     const int L = __shfl_sync(0xffffffffu, label, leader);
@@ -53,6 +59,7 @@ __device__ __forceinline__ void bin_by_label(double* bins, bool valid, int label
     if (lane == 0) { bins[2 * L] += sa; bins[2 * L + 1] += sb; }
     active &= ~__ballot_sync(0xffffffffu, mine);
   }
+  __syncwarp();                                                // the next call's adds may come from other lanes
 }
 
 __global__ void __launch_bounds__(kDpThreads, 3)
