@@ -44,8 +44,8 @@ __device__ __forceinline__ double warp_sum(double v) {
 
 // add (a, b) of the lanes with `valid` into bins[label][0..1] (deterministic).  A lane whose label no other valid lane
 // of the warp carries (an outlier match landing in some far segment) adds straight to the bin -- distinct labels, so these
-// adds do not meet; the labels shared by several lanes go label by label: butterfly sum of the lanes carrying it, lane 0
-// adds.  The usual warp (one segment, a few stray matches) takes one butterfly round instead of one per stray lane.
+// adds do not meet; the labels shared by several lanes go label by label: butterfly sum of the lanes carrying it,
+// lanes 0 and 1 add.  The usual warp (one segment, a few stray matches) takes one butterfly round instead of one per stray lane.
 __device__ __forceinline__ void bin_by_label(double* bins, bool valid, int label, double a, double b, int lane) {
   const unsigned peers = __match_any_sync(0xffffffffu, valid ? label : -1 - lane);   // invalid lanes: unique keys
   const bool single = valid && peers == (1u << lane);
@@ -55,8 +55,13 @@ __device__ __forceinline__ void bin_by_label(double* bins, bool valid, int label
     const int leader = __ffs(active) - 1;
     const int L = __shfl_sync(0xffffffffu, label, leader);
     const bool mine = valid && label == L;
-    const double sa = warp_sum(mine ? a : 0.0), sb = warp_sum(mine ? b : 0.0);
-    if (lane == 0) { bins[2 * L] += sa; bins[2 * L + 1] += sb; }
+    // both sums in one butterfly: after the first exchange even lanes carry pair sums of a, odd lanes of b
+    const double va = mine ? a : 0.0, vb = mine ? b : 0.0;
+    double x = (lane & 1) ? vb : va;
+    x += __shfl_xor_sync(0xffffffffu, (lane & 1) ? va : vb, 1);
+#pragma unroll
+    for (int o = 2; o < 32; o <<= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    if (lane < 2) bins[2 * L + lane] += x;                     // lane 0: sum of a, lane 1: sum of b
     active &= ~__ballot_sync(0xffffffffu, mine);
   }
   __syncwarp();                                                // the next call's adds may come from other lanes
