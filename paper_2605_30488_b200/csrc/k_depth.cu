@@ -27,6 +27,9 @@ namespace {
 constexpr int kDpThreads = 256;
 constexpr int kDpWarps = kDpThreads / 32;
 constexpr int kDpMaxSeg = 64;
+#ifndef SIM3BA_DP_CTAS
+#define SIM3BA_DP_CTAS 2
+#endif
 #ifndef SIM3BA_DP_TILE_PX
 #define SIM3BA_DP_TILE_PX 8192
 #endif
@@ -67,7 +70,7 @@ __device__ __forceinline__ void bin_by_label(double* bins, bool valid, int label
   __syncwarp();                                                // the next call's adds may come from other lanes
 }
 
-__global__ void __launch_bounds__(kDpThreads, 3)
+__global__ void __launch_bounds__(kDpThreads, SIM3BA_DP_CTAS)
 k_depth_edge(const float4* __restrict__ pm, const int32_t* __restrict__ match, const int32_t* __restrict__ edges,
              const int32_t* __restrict__ grp_edge, int E, const int32_t* __restrict__ labels, const double* __restrict__ eta, const double* __restrict__ poses, int HW,
              int n_seg, int tiles, DepthDev prm, double* __restrict__ partial) {
@@ -91,39 +94,53 @@ k_depth_edge(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
   const int per = (HW + tiles - 1) / tiles;
   const int m0 = tile * per, m1 = min(HW, m0 + per);
   double cost = 0.0;
-  for (int base = m0; base < m1; base += kDpThreads) {        // warp-uniform trip count: the binning uses full-warp shuffles
-    const int m = base + tid;
+  // Software pipeline over the CTA's iterations (warp-uniform trip count: the binning uses full-warp shuffles): the
+  // streamed loads (match index, X_i, label of m) run two iterations ahead, the gathers they address (X_j, label of n) one.
+  const int niter = (m1 - m0 + kDpThreads - 1) / kDpThreads;
+  auto load_stream = [&](int it, int& n, float4& a, int& lg) {
+    const int m = m0 + it * kDpThreads + tid;
+    n = -1;
+    if (it < niter && m < m1) { n = __ldcs(mt + m); a = Pi[m]; lg = li[m]; }
+  };
+  auto load_gather = [&](int n, float4& b, int& lh) {
+    if ((unsigned)n < (unsigned)HW) { b = Pj[n]; lh = lj[n]; }
+  };
+  int n0, n1, n2, lg0 = 0, lg1 = 0, lg2 = 0, lh0 = 0, lh1 = 0;
+  float4 a0 = make_float4(0.f, 0.f, 0.f, -1.f), a1 = a0, a2 = a0, b0 = a0, b1 = a0;
+  load_stream(0, n0, a0, lg0);
+  load_stream(1, n1, a1, lg1);
+  load_gather(n0, b0, lh0);
+  for (int it = 0; it < niter; ++it) {
+    load_stream(it + 2, n2, a2, lg2);
+    load_gather(n1, b1, lh1);
     bool valid = false;
-    int lg = 0, lh = 0;
+    const int lg = lg0, lh = lh0;
     double vg = 0.0, Hg = 0.0, vh = 0.0, Hh = 0.0;
-    if (m < m1) {
-      const int n = mt[m];
-      if ((unsigned)n < (unsigned)HW) {
-        const float4 a = Pi[m], b = Pj[n];
-        lg = li[m];
-        lh = lj[n];
-        if (a.w >= 0.f && b.w >= 0.f && lg >= 0 && lh >= 0 && lg < n_seg && lh < n_seg) {
-          valid = true;
-          const double eg = s_exp[0][lg], eh = s_exp[1][lh];
-          const double Xi[3] = {eg * (double)a.x, eg * (double)a.y, eg * (double)a.z};
-          const double Xj[3] = {eh * (double)b.x, eh * (double)b.y, eh * (double)b.z};
-          const double sq = (double)a.w * (double)b.w, q = sq * sq;     // w = c^(1/4): sqrt(q) = w_i w_j, q = sqrt(c_i c_j)
+    if ((unsigned)n0 < (unsigned)HW) {
+      const float4 a = a0, b = b0;
+      if (a.w >= 0.f && b.w >= 0.f && lg >= 0 && lh >= 0 && lg < n_seg && lh < n_seg) {
+        valid = true;
+        const double eg = s_exp[0][lg], eh = s_exp[1][lh];
+        const double Xi[3] = {eg * (double)a.x, eg * (double)a.y, eg * (double)a.z};
+        const double Xj[3] = {eh * (double)b.x, eh * (double)b.y, eh * (double)b.z};
+        const double sq = (double)a.w * (double)b.w, q = sq * sq;     // w = c^(1/4): sqrt(q) = w_i w_j, q = sqrt(c_i c_j)
 #pragma unroll
-          for (int c = 0; c < 3; ++c) {
-            const double Jh = T.s * (T.R[3 * c] * Xj[0] + T.R[3 * c + 1] * Xj[1] + T.R[3 * c + 2] * Xj[2]);
-            const double res = Jh + T.t[c] - Xi[c];
-            const double r = sq * res * prm.inv_sigma, ar = fabs(r);
-            const double w = ar <= prm.huber_k ? 1.0 : prm.huber_k / ar;
-            const double om = q * w * prm.inv_sigma * prm.inv_sigma;
-            cost += ar <= prm.huber_k ? 0.5 * r * r : prm.huber_k * (ar - 0.5 * prm.huber_k);
-            vg -= om * Xi[c] * res;                                        // J_g = -X_i(eta)
-            Hg += om * Xi[c] * Xi[c];
-            vh += om * Jh * res;                                           // J_h = s_ij R_ij X_j(eta)
-            Hh += om * Jh * Jh;
-          }
+        for (int c = 0; c < 3; ++c) {
+          const double Jh = T.s * (T.R[3 * c] * Xj[0] + T.R[3 * c + 1] * Xj[1] + T.R[3 * c + 2] * Xj[2]);
+          const double res = Jh + T.t[c] - Xi[c];
+          const double r = sq * res * prm.inv_sigma, ar = fabs(r);
+          const double w = ar <= prm.huber_k ? 1.0 : prm.huber_k / ar;
+          const double om = q * w * prm.inv_sigma * prm.inv_sigma;
+          cost += ar <= prm.huber_k ? 0.5 * r * r : prm.huber_k * (ar - 0.5 * prm.huber_k);
+          vg -= om * Xi[c] * res;                                        // J_g = -X_i(eta)
+          Hg += om * Xi[c] * Xi[c];
+          vh += om * Jh * res;                                           // J_h = s_ij R_ij X_j(eta)
+          Hh += om * Jh * Jh;
         }
       }
     }
+    n0 = n1; a0 = a1; lg0 = lg1; b0 = b1; lh0 = lh1;
+    n1 = n2; a1 = a2; lg1 = lg2;
     bin_by_label(&s_bins[warp][0][0][0], valid, lg, vg, Hg, lane);
     bin_by_label(&s_bins[warp][1][0][0], valid, lh, vh, Hh, lane);
   }
