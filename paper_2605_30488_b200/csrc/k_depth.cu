@@ -31,7 +31,7 @@ constexpr int kDpMaxSeg = 64;
 #define SIM3BA_DP_CTAS 2
 #endif
 #ifndef SIM3BA_DP_TILE_PX
-#define SIM3BA_DP_TILE_PX 8192
+#define SIM3BA_DP_TILE_PX 16384
 #endif
 constexpr int kDpTilePx = SIM3BA_DP_TILE_PX;
 
