@@ -92,9 +92,9 @@ k_depth_edge(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
   __shared__ double s_bins[kDpWarps][2][kDpMaxSeg][2];
   __shared__ double s_exp[2][kDpMaxSeg];
   __shared__ double s_cost[kDpWarps];
-  // tile-major launch order over the edges sorted by (i, j): the CTAs in flight work on the same pixel range of
-  // neighbouring keyframes, so the tiles of X_i, X_j and of the labels are fetched from HBM once and shared through L2
-  const int tile = blockIdx.x / E, e = grp_edge[blockIdx.x - tile * E];
+  // launch order = kernel 1's: the edges sorted by (i, j), all tiles of an edge together, so the CTAs in flight cover a
+  // few neighbouring keyframes completely and X_i, X_j and the labels are fetched from HBM once and shared through L2
+  const int k = blockIdx.x / tiles, tile = blockIdx.x - k * tiles, e = grp_edge[k];
   const int i = edges[2 * e], j = edges[2 * e + 1];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   for (int q = tid; q < kDpWarps * 2 * kDpMaxSeg * 2; q += kDpThreads) (&s_bins[0][0][0][0])[q] = 0.0;
