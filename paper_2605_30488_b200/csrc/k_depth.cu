@@ -7,10 +7,12 @@
 //                   Delta eta_g = -g_g / ((1 + lambda_lm) H_gg), clipped to eta_max, anchor keyframes fixed
 // Conventions D1-D5 of DESIGN.md section 10 (objective = sum rho + lambda_s/2 E_bnd + lambda_p/2 E_prior).
 //
-// Kernel A (k_depth_edge): one CTA per (edge, tile of the pixels of i).  Per match everything is FP64 (the residual is a
-// difference of two ~10 m points).  The per-segment sums are binned without atomics: a warp serialises over the distinct
-// labels of its 32 matches (butterfly sum of the lanes carrying the label, one lane adds to the warp's own shared-memory
-// bin), the eight warps' bins are added in a fixed order -> one record [2 sides][n_seg][g, H] + cost per (edge, tile).
+// Kernel A (k_depth_edge): one CTA per (edge, tile of the pixels of i), in kernel 1's order (edges sorted by keyframe,
+// the tiles of an edge together: X_j and the labels are shared through L2).  Per match everything is FP64 (the residual
+// is a difference of two ~10 m points); the loads run in a software pipeline (streams two iterations ahead, gathers
+// one).  The per-segment sums are binned without atomics: a lane whose label is alone in its warp adds straight to the
+// warp's own shared-memory bin, a label shared by several lanes takes one butterfly carrying both sums; the eight warps'
+// bins are added in a fixed order -> one record [2 sides][n_seg][g, H] + cost per (edge, tile).
 // Kernel B (k_depth_update): one thread per segment gathers its records through the keyframe -> edge CSR, adds boundary
 // and prior terms, takes the damped clipped step into a second eta buffer.  Kernel C sums the objective.
 #include <math.h>
@@ -87,8 +89,8 @@ __device__ __forceinline__ void bin_by_label(double* bins, bool valid, int label
 
 __global__ void __launch_bounds__(kDpThreads, SIM3BA_DP_CTAS)
 k_depth_edge(const float4* __restrict__ pm, const int32_t* __restrict__ match, const int32_t* __restrict__ edges,
-             const int32_t* __restrict__ grp_edge, int E, const int32_t* __restrict__ labels, const double* __restrict__ eta, const double* __restrict__ poses, int HW,
-             int n_seg, int tiles, DepthDev prm, double* __restrict__ partial) {
+             const int32_t* __restrict__ grp_edge, const int32_t* __restrict__ labels, const double* __restrict__ eta,
+             const double* __restrict__ poses, int HW, int n_seg, int tiles, DepthDev prm, double* __restrict__ partial) {
   __shared__ double s_bins[kDpWarps][2][kDpMaxSeg][2];
   __shared__ double s_exp[2][kDpMaxSeg];
   __shared__ double s_cost[kDpWarps];
@@ -288,7 +290,7 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
   double *cur = d_eta, *nxt = d_eta2;
   for (int it = 0; it < n_iters && e == cudaSuccess; ++it) {
     if (c->E > 0)
-      k_depth_edge<<<c->E * tiles, kDpThreads, 0, c->stream>>>(c->pm, c->match, c->edges, c->grp_edge, c->E, d_labels, cur, c->poses, c->HW, n_seg, tiles, dev,
+      k_depth_edge<<<c->E * tiles, kDpThreads, 0, c->stream>>>(c->pm, c->match, c->edges, c->grp_edge, d_labels, cur, c->poses, c->HW, n_seg, tiles, dev,
                                                               d_partial);
     k_depth_cost<<<1, 256, 0, c->stream>>>(d_partial, c->E * tiles, rec, cur, n_total, d_pairs, d_delta, n_pairs, dev, d_cost + it);
     k_depth_update<<<(n_total + 127) / 128, 128, 0, c->stream>>>(d_partial, cur, nxt, c->edges, c->kf_ptr, c->kf_edge, d_sp_ptr, d_sp_other,
