@@ -92,14 +92,21 @@ int sim3ba_build_system(sim3ba_ctx* ctx);
 
 /* a7 on the last built system: Eq. (7) with the epsilon escalation of PAPER.md:122 by blocked
  * FP64 Cholesky and two triangular solves.  Requires a previous build (else BAD_STATE).
- * "All attempts failed" is not an error: tau = 0, attempts = max_attempts.  Synchronises the
- * stream once per attempt to read the factorisation flag. */
+ * "All attempts failed" is not an error: tau = 0, attempts = max_attempts.  The retry loop runs on the
+ * device inside one persistent kernel: no host synchronisation. */
 int sim3ba_solve(sim3ba_ctx* ctx);
 
 /* One Gauss-Newton iteration: a1-a5, assembly of the damped system, a7, and the retraction
  * T_i <- Exp(tau_i) T_i of every non-fixed keyframe.  (The undamped dense H of
  * sim3ba_get_system is not refreshed by this call; the per-edge blocks and g are.) */
 int sim3ba_step(sim3ba_ctx* ctx);
+
+/* n_steps Gauss-Newton iterations (sim3ba_step each) enqueued as ONE CUDA-graph launch.  The kernel sequence of the
+ * iterations is captured once per (context, n_steps, params, solver mode) and replayed: the same kernels in the same
+ * order, so the poses afterwards equal those of n_steps x sim3ba_step bit for bit.  For small problems -- the tracker's
+ * single relative pose (E = 1, n = 7), config 1 -- an iteration is bound by launch latency and the graph
+ * removes the per-kernel launch cost.  Asynchronous.  Errors: INVALID_ARG (n_steps outside 1..4096), CUDA. */
+int sim3ba_step_graph(sim3ba_ctx* ctx, int32_t n_steps);
 
 /* Same iteration with HOST pose buffers: copies h_poses_in [N][8] to the device (if non-NULL),
  * runs sim3ba_step, copies the new poses to h_poses_out [N][8] and the robust cost at the input
@@ -123,7 +130,8 @@ int sim3ba_optimize_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_
  * Over the valid matches (m, n) of edge `edge` = (i, j) of the graph -- the validity rule of the GN step -- the matched
  * points are lifted into the two world frames with the CURRENT poses, x = T_WCi X_i[m], y = T_WCj X_j[n], and
  * (s*, R*, t*) = argmin sum |x - (s R y + t)|^2 (Eq. (3)) is found in closed form (Eq. (4), Umeyama; FP64).  With fewer
- * than n_c_min correspondences (paper: 64) T* = T_WCi T_WCj^-1 instead.  T* is then left-multiplied onto the poses of
+ * than n_c_min correspondences (paper: 64) T* = T_WCi T_WCj^-1 instead (also when the matched cloud is degenerate --
+ * zero variance or a non-positive / non-finite scale -- where Eq. (4) has no answer).  T* is then left-multiplied onto the poses of
  * the n_moving keyframes h_moving_kf (host array; the component of j).  moving_is_i != 0 swaps the roles: the similarity
  * maps x onto y (fallback T_WCj T_WCi^-1) and is meant for the component of i.  Host outputs, each may be NULL:
  * h_T [8] = T* in the pose layout (t, q_xyzw, s), *h_n_c = number of correspondences, *h_fallback = 1 if the endpoint
@@ -231,6 +239,16 @@ int sim3ba_get_launch_count(sim3ba_ctx* ctx, int64_t* h_count);
  * [5..7] reserved (0).  Synchronises.  Only recorded after sim3ba_set_profiling(ctx, 1). */
 int sim3ba_set_profiling(sim3ba_ctx* ctx, int32_t enable);
 int sim3ba_get_phase_ms(sim3ba_ctx* ctx, float h_ms[8]);
+
+/* With profiling on, the band + border solve kernel (mode 2) stamps its phases with the device's global timer; microseconds
+ * of the last solve: [0] assembly (a6), [1] segment elimination, [2] grid barrier after it, [3] Schur rows, [4] border
+ * system, [5] back-substitution, [6..7] reserved (0).  All zero if the last solve was not profiled.  Synchronises. */
+int sim3ba_get_solve_phase_us(sim3ba_ctx* ctx, float h_us[8]);
+
+/* All device memory of the library comes from a stream-ordered memory pool the library owns (one per device), which keeps
+ * freed blocks for the next context / job.  This call synchronises the current device and returns the pool's unused memory
+ * to the driver. */
+int sim3ba_release_memory(void);
 
 /* Binding convenience: asynchronous device-to-device copy of `bytes` bytes on the context's stream
  * (used to move the read-back buffers above into caller-owned device memory). */

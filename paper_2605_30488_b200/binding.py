@@ -16,11 +16,11 @@ LIB_PATH = os.path.join(_HERE, "libsim3ba.so")
 
 EXPORTS = (
     "sim3ba_default_params", "sim3ba_create", "sim3ba_destroy", "sim3ba_set_params", "sim3ba_set_poses",
-    "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_host", "sim3ba_optimize_host", "sim3ba_gauge_sync", "sim3ba_depth_default_params", "sim3ba_depth_refine", "sim3ba_apply_depth",
+    "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_graph", "sim3ba_step_host", "sim3ba_optimize_host", "sim3ba_gauge_sync", "sim3ba_depth_default_params", "sim3ba_depth_refine", "sim3ba_apply_depth",
     "sim3ba_retract", "sim3ba_get_edge_stats", "sim3ba_get_edge_blocks", "sim3ba_get_system",
     "sim3ba_get_update", "sim3ba_get_bookkeeping", "sim3ba_load_system", "sim3ba_get_launch_count",
     "sim3ba_set_solver_mode", "sim3ba_get_solver_info", "sim3ba_get_bb_info",
-    "sim3ba_set_profiling", "sim3ba_get_phase_ms", "sim3ba_copy_d2d", "sim3ba_last_error", "sim3ba_version",
+    "sim3ba_set_profiling", "sim3ba_get_phase_ms", "sim3ba_get_solve_phase_us", "sim3ba_release_memory", "sim3ba_copy_d2d", "sim3ba_last_error", "sim3ba_version",
 )
 
 
@@ -65,6 +65,7 @@ def load_library() -> C.CDLL:
         "sim3ba_build_system": [vp],
         "sim3ba_solve": [vp],
         "sim3ba_step": [vp],
+        "sim3ba_step_graph": [vp, i32],
         "sim3ba_step_host": [vp, vp, vp, vp],
         "sim3ba_optimize_host": [i32, i32, i32, i32, vp, vp, vp, vp, P(i32), i32, P(Params), vp, i32, vp, vp, vp],
         "sim3ba_gauge_sync": [vp, i32, P(i32), i32, i32, i32, P(C.c_double), P(i32), P(i32)],
@@ -84,6 +85,8 @@ def load_library() -> C.CDLL:
         "sim3ba_get_bb_info": [vp, P(i32)],
         "sim3ba_set_profiling": [vp, i32],
         "sim3ba_get_phase_ms": [vp, P(C.c_float)],
+        "sim3ba_get_solve_phase_us": [vp, P(C.c_float)],
+        "sim3ba_release_memory": [],
         "sim3ba_copy_d2d": [vp, vp, vp, C.c_uint64],
     }
     for name, args in sig.items():
@@ -200,6 +203,10 @@ class Sim3BA:
     def step(self):
         self._check(self.lib.sim3ba_step(self._h))
 
+    def step_graph(self, n_steps: int = 1):
+        """n_steps GN iterations as one CUDA-graph launch (sim3ba_step_graph)."""
+        self._check(self.lib.sim3ba_step_graph(self._h, int(n_steps)))
+
     def gauge_sync(self, edge: int, moving_kf: Sequence[int], moving_is_i: bool = False, n_c_min: int = 64):
         """sim3ba_gauge_sync on the current poses; returns (T* as an 8-vector pose, N_c, fallback used)."""
         mk = (C.c_int32 * max(1, len(moving_kf)))(*[int(k) for k in moving_kf])
@@ -291,7 +298,7 @@ class Sim3BA:
         self._check(self.lib.sim3ba_load_system(self._h, H.data_ptr(), g.data_ptr()))
 
     def set_solver_mode(self, mode: int):
-        """0: tile-sparse plan of the graph (default); 1: dense plan (every lower tile)."""
+        """2: band + border block Cholesky (default); 0: tile-sparse plan of the graph; 1: dense plan (every lower tile)."""
         self._check(self.lib.sim3ba_set_solver_mode(self._h, int(mode)))
 
     def solver_info(self) -> Dict[str, float]:
@@ -316,4 +323,9 @@ class Sim3BA:
     def phase_ms(self) -> Tuple[float, ...]:
         buf = (C.c_float * 8)()
         self._check(self.lib.sim3ba_get_phase_ms(self._h, buf))
+        return tuple(buf)
+
+    def solve_phase_us(self) -> Tuple[float, ...]:
+        buf = (C.c_float * 8)()
+        self._check(self.lib.sim3ba_get_solve_phase_us(self._h, buf))
         return tuple(buf)

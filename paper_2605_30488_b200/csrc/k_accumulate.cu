@@ -526,13 +526,18 @@ cudaError_t launch_pack(Ctx* c, const float* d_points, const float* d_conf) {
   return cudaGetLastError();
 }
 
+cudaError_t prepare_accumulate(Ctx* c) {
+  if (c->acc_ready) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(k_accumulate, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAccSmem);
+  if (e == cudaSuccess) c->acc_ready = true;
+  return e;
+}
+
 cudaError_t launch_accumulate(Ctx* c) {
   if (c->E == 0) return cudaSuccess;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_accumulate, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kAccSmem);
+  {
+    cudaError_t e = prepare_accumulate(c);
     if (e != cudaSuccess) return e;
-    attr_set = true;
   }
   DevParams p;
   p.inv_var_ray = 1.0f / (c->prm.sigma_ray * c->prm.sigma_ray);

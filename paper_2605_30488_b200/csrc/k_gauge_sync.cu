@@ -7,7 +7,8 @@
 //   PAPER.md:102    T* is left-multiplied onto every pose of the moving component
 //
 // Three small FP64 kernels: (1) a fixed-order reduction of the 19 moments (count, sum x, sum y, sum x y^T, sum |x|^2,
-// sum |y|^2) over the pixels of the edge, (2) one warp: centred cross-covariance A, the proper rotation maximising
+// sum |y|^2) over the pixels of the edge, taken about the two camera centres t_i, t_j (pivots: two components with
+// far-apart origins would otherwise lose (|centroid| / spread)^2 ulps to cancellation when the moments are centred), (2) one warp: centred cross-covariance A, the proper rotation maximising
 // tr(R^T A) -- the largest eigenvector of Horn's symmetric 4x4 matrix by cyclic Jacobi sweeps, which IS U S V^T of
 // Eq. (4) (the search is over rotations only, so the reflection case needs no special handling) -- then
 // s* = tr(R*^T A) / var(y) (= tr(S Lambda) / var(y)) and t*; (3) T* applied to the listed keyframes.
@@ -39,8 +40,9 @@ k_gs_moments(const float4* __restrict__ pm, const int32_t* __restrict__ match_e,
     double x[3], y[3];
 #pragma unroll
     for (int r = 0; r < 3; ++r) {
-      x[r] = Ti.s * (Ti.R[3 * r] * (double)a.x + Ti.R[3 * r + 1] * (double)a.y + Ti.R[3 * r + 2] * (double)a.z) + Ti.t[r];
-      y[r] = Tj.s * (Tj.R[3 * r] * (double)b.x + Tj.R[3 * r + 1] * (double)b.y + Tj.R[3 * r + 2] * (double)b.z) + Tj.t[r];
+      // x_l - t_i and y_l - t_j: the moments are accumulated about the camera centres (see k_gs_solve)
+      x[r] = Ti.s * (Ti.R[3 * r] * (double)a.x + Ti.R[3 * r + 1] * (double)a.y + Ti.R[3 * r + 2] * (double)a.z);
+      y[r] = Tj.s * (Tj.R[3 * r] * (double)b.x + Tj.R[3 * r + 1] * (double)b.y + Tj.R[3 * r + 2] * (double)b.z);
     }
     acc[0] += 1.0;
 #pragma unroll
@@ -122,9 +124,13 @@ k_gs_solve(const double* __restrict__ partial, int n_part, const double* __restr
   __syncwarp();
   if (lane != 0) return;
   const double nc = s_m[0];
-  double Tq[4], Tt[3], Ts;
-  if (nc >= (double)n_c_min) {
-    // reference cloud r (target) and moving cloud m: x ~ s R y + t, or with the roles swapped
+  double Tq[4], Tt[3], Ts = 0.0;
+  bool closed_form = nc >= (double)n_c_min;
+  if (closed_form) {
+    // reference cloud r (target) and moving cloud m: x ~ s R y + t, or with the roles swapped; the moments are about the
+    // pivots t_i (x side) and t_j (y side): centroid offsets rb, mb first, the pivots added back for t* only
+    const double* piv_r = poses + 8 * (moving_is_i ? j : i);
+    const double* piv_m = poses + 8 * (moving_is_i ? i : j);
     double rb[3], mb[3], A[3][3], var_m;
     for (int r = 0; r < 3; ++r) { rb[r] = s_m[(moving_is_i ? 4 : 1) + r] / nc; mb[r] = s_m[(moving_is_i ? 1 : 4) + r] / nc; }
     for (int r = 0; r < 3; ++r)
@@ -151,9 +157,13 @@ k_gs_solve(const double* __restrict__ partial, int n_part, const double* __restr
     for (int r = 0; r < 3; ++r)
       for (int c = 0; c < 3; ++c) tr += R[3 * r + c] * A[r][c];
     Ts = tr / var_m;
-    for (int r = 0; r < 3; ++r) Tt[r] = rb[r] - Ts * (R[3 * r] * mb[0] + R[3 * r + 1] * mb[1] + R[3 * r + 2] * mb[2]);
+    const double mc[3] = {mb[0] + piv_m[0], mb[1] + piv_m[1], mb[2] + piv_m[2]};
+    for (int r = 0; r < 3; ++r) Tt[r] = (rb[r] + piv_r[r]) - Ts * (R[3 * r] * mc[0] + R[3 * r + 1] * mc[1] + R[3 * r + 2] * mc[2]);
     out[9] = 0.0;
-  } else {
+    // degenerate clouds (coincident or collinear points: var = 0, tr <= 0) have no similarity: endpoint transform instead
+    if (!(var_m > 0.0) || !(Ts > 0.0) || !isfinite(Ts) || !isfinite(Tt[0] + Tt[1] + Tt[2])) closed_form = false;
+  }
+  if (!closed_form) {
     // endpoint fallback: T* = T_ref T_mov^-1
     const double* pr = poses + 8 * (moving_is_i ? j : i);
     const double* pv = poses + 8 * (moving_is_i ? i : j);

@@ -86,18 +86,16 @@ k_solve(SolveArgs a) {
 
 }  // namespace
 
-cudaError_t launch_solve(Ctx* c) {
-  static int max_blocks_per_sm = -1, num_sms = 0;
+cudaError_t prepare_solve(Ctx* c) {
   const size_t smem = sizeof(Smem);
-  if (max_blocks_per_sm < 0) {
+  if (c->solve_bpsm < 0) {
     cudaError_t e = cudaFuncSetAttribute(k_solve, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&max_blocks_per_sm, k_solve, kSolveThreads, smem);
+    int bpsm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bpsm, k_solve, kSolveThreads, smem);
     if (e != cudaSuccess) return e;
-    if (max_blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
+    if (bpsm < 1) return cudaErrorLaunchOutOfResources;
+    c->solve_bpsm = bpsm;
   }
   const bool dense = c->dense_loaded || c->solver_mode == 1;
   SolvePlan& plan = dense ? c->plan_dense : c->plan_sparse;
@@ -105,6 +103,18 @@ cudaError_t launch_solve(Ctx* c) {
     std::string err;
     if (!build_plan(c, dense, plan, err)) { c->err = err; return cudaErrorUnknown; }
   }
+  return ensure_dense(c, false, true);
+}
+
+cudaError_t launch_solve(Ctx* c) {
+  const size_t smem = sizeof(Smem);
+  {
+    cudaError_t e = prepare_solve(c);
+    if (e != cudaSuccess) return e;
+  }
+  const int num_sms = c->num_sms, max_blocks_per_sm = c->solve_bpsm;
+  const bool dense = c->dense_loaded || c->solver_mode == 1;
+  SolvePlan& plan = dense ? c->plan_dense : c->plan_sparse;
   long long want = std::max<long long>({(long long)plan.max_upd, (long long)plan.max_col, (long long)plan.max_row, 1LL});
   const int G = (int)std::min<long long>(want, (long long)num_sms * std::min(max_blocks_per_sm, 2));
   SolveArgs a;

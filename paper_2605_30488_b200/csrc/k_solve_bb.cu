@@ -30,14 +30,20 @@ constexpr int kWin = 8;            // block columns resident in shared memory pe
 constexpr int kBackRing = 8;       // [D | band] parts in flight during the back-substitution
 static_assert(kBand == 3, "the trailing update of the border blocks is written out for three band blocks");
 
-#ifdef SIM3BA_BB_STAMPS
-__device__ unsigned long long g_bb_stamps[16];
-#define BB_STAMP(i) do { if (blockIdx.x == 0 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_bb_stamps[i] = t_; } } while (0)
-#else
-#define BB_STAMP(i)
-#endif
+// phase time stamps of the persistent kernel (only with sim3ba_set_profiling: a.stamps is NULL otherwise), read back by
+// sim3ba_get_solve_phase_us: [0] start, [1] assembled, [2] segments eliminated, [3] barrier passed, [4] Schur rows done,
+// [5] border system solved, [6] back-substitution done (stamps of the last attempt)
+#define BB_STAMP(i)                                                                  \
+  do {                                                                               \
+    if (a.stamps != nullptr && blockIdx.x == 0 && threadIdx.x == 0) {                \
+      unsigned long long t_;                                                         \
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                         \
+      a.stamps[i] = t_;                                                              \
+    }                                                                                \
+  } while (0)
 
 struct BBArgs {
+  unsigned long long* stamps;
   const double *blocks35, *g;
   const int32_t *kf_ptr, *kf_edge, *pair_ptr, *pair_edge;
   double lambda;
@@ -594,26 +600,38 @@ k_solve_bb(BBArgs a) {
 
 }  // namespace
 
-cudaError_t launch_solve_bb(Ctx* c) {
-  BBPlan& P = c->plan_bb;
-  static int max_blocks_per_sm = -1, num_sms = 0;
-  static size_t smem_set = 0;
+static size_t bb_smem_bytes(const BBPlan& P, int* slot_out) {
   const int slot = ((1 + kBand + P.max_nb) * 49 + 7 + 1) & ~1;
   const size_t smem_seg = ((size_t)kWin * slot + 7 * kMaxSegBorder) * sizeof(double) + sizeof(SegSmem);
   const size_t smem_back = ((size_t)kBackRing * (1 + kBand) * 49 + 7 * (size_t)P.max_len + 7 * kMaxSegBorder) * sizeof(double);
   const size_t smem_schur = (size_t)2 * kSchurCols * kSchurPart * sizeof(double);
-  const size_t smem = std::max({sizeof(Smem), smem_seg, smem_back, smem_schur});
-  if (max_blocks_per_sm < 0 || smem > smem_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_solve_bb, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (slot_out) *slot_out = slot;
+  return std::max({sizeof(Smem), smem_seg, smem_back, smem_schur});
+}
+
+cudaError_t prepare_solve_bb(Ctx* c) {
+  const size_t smem = bb_smem_bytes(c->plan_bb, nullptr);
+  if (c->bb_bpsm >= 0 && smem <= c->bb_smem) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(k_solve_bb, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  int bpsm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bpsm, k_solve_bb, kSolveThreads, smem);
+  if (e != cudaSuccess) return e;
+  if (bpsm < 1) return cudaErrorLaunchOutOfResources;
+  c->bb_bpsm = bpsm;
+  c->bb_smem = smem;
+  return cudaSuccess;
+}
+
+cudaError_t launch_solve_bb(Ctx* c) {
+  BBPlan& P = c->plan_bb;
+  {
+    cudaError_t e = prepare_solve_bb(c);
     if (e != cudaSuccess) return e;
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&max_blocks_per_sm, k_solve_bb, kSolveThreads, smem);
-    if (e != cudaSuccess) return e;
-    if (max_blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
-    smem_set = smem;
   }
+  int slot = 0;
+  const size_t smem = bb_smem_bytes(P, &slot);
+  const int num_sms = c->num_sms, max_blocks_per_sm = c->bb_bpsm;
   const SolvePlan& D = P.dense;
   // enough CTAs for the widest phase: one block column each in the assembly (its loads are a chain of L2 round trips),
   // one per segment / border keyframe / tile task
@@ -621,6 +639,7 @@ cudaError_t launch_solve_bb(Ctx* c) {
                                         (long long)P.n_int, 1LL});
   const int G = (int)std::min<long long>(want, (long long)num_sms * std::min(max_blocks_per_sm, 1));
   BBArgs a{};
+  a.stamps = c->profiling ? c->solve_stamps : nullptr;
   a.blocks35 = c->blocks35; a.g = c->g; a.kf_ptr = c->kf_ptr; a.kf_edge = c->kf_edge; a.pair_ptr = c->pair_ptr; a.pair_edge = c->pair_edge;
   a.lambda = c->prm.lm_lambda;
   a.n_int = P.n_int; a.n_seg = P.n_seg; a.n_bord = P.n_bord; a.npadB = P.npadB; a.slot_doubles = slot; a.max_len = P.max_len;
@@ -642,16 +661,6 @@ cudaError_t launch_solve_bb(Ctx* c) {
   e = cudaLaunchCooperativeKernel((const void*)k_solve_bb, dim3(G), dim3(kSolveThreads), args, smem, c->stream);
   c->launches += 1;
   c->last_solve_grid = G;
-#ifdef SIM3BA_BB_STAMPS
-  {
-    cudaStreamSynchronize(c->stream);
-    unsigned long long st[16];
-    cudaMemcpyFromSymbol(st, g_bb_stamps, sizeof(st));
-    fprintf(stderr, "[bb] G=%d seg=%d bord=%d maxlen=%d | asm %.1f seg %.1f (bar %.1f) schur %.1f border-chol %.1f back %.1f us\n", G, P.n_seg, P.n_bord,
-            P.max_len, (st[1] - st[0]) * 1e-3, (st[2] - st[1]) * 1e-3, (st[3] - st[2]) * 1e-3, (st[4] - st[3]) * 1e-3, (st[5] - st[4]) * 1e-3,
-            (st[6] - st[5]) * 1e-3);
-  }
-#endif
   return e;
 }
 

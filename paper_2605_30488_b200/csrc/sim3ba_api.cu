@@ -5,6 +5,7 @@
 
 #include <algorithm>
 #include <map>
+#include <mutex>
 #include <new>
 #include <numeric>
 #include <utility>
@@ -12,6 +13,53 @@
 #include "sim3ba_internal.cuh"
 
 using namespace sim3ba;
+
+namespace sim3ba {
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_pool_mutex;
+cudaMemPool_t g_pools[kMaxDevices] = {};
+}  // namespace
+
+cudaError_t lib_pool(cudaMemPool_t* pool) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_pool_mutex);
+  if (!g_pools[dev]) {
+    cudaMemPoolProps props = {};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    e = cudaMemPoolCreate(&g_pools[dev], &props);
+    if (e != cudaSuccess) { g_pools[dev] = nullptr; return e; }
+    uint64_t keep = UINT64_MAX;   // freed blocks stay in the library's pool until sim3ba_release_memory
+    cudaMemPoolSetAttribute(g_pools[dev], cudaMemPoolAttrReleaseThreshold, &keep);
+  }
+  *pool = g_pools[dev];
+  return cudaSuccess;
+}
+
+// Hd (undamped dense system: sim3ba_build_system read-back, sim3ba_load_system) and L (work matrix of the tile plans,
+// solver modes 0 / 1) are npad^2 doubles each -- 1.57 GB at N = 2000: allocated when first needed, never by the
+// default path (sim3ba_step with the band + border plan)
+cudaError_t ensure_dense(Ctx* c, bool want_Hd, bool want_L) {
+  const size_t bytes = (size_t)c->npad * c->npad * sizeof(double);
+  if (want_Hd && !c->Hd) {
+    cudaError_t e = dmalloc(reinterpret_cast<void**>(&c->Hd), bytes);
+    if (e != cudaSuccess) return e;
+  }
+  if (want_L && !c->L) {
+    cudaError_t e = dmalloc(reinterpret_cast<void**>(&c->L), bytes);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
+}  // namespace sim3ba
 
 struct sim3ba_ctx {
   Ctx c;
@@ -91,13 +139,20 @@ void free_all(Ctx* c) {
   dfree(c->partials); dfree(c->blocks35); dfree(c->edge_cost); dfree(c->n_valid); dfree(c->checksum);
   dfree(c->Hd); dfree(c->L); dfree(c->g); dfree(c->rhs); dfree(c->ysol); dfree(c->Dinv); dfree(c->pairhi_ptr);
   free_plan(c->plan_sparse); free_plan(c->plan_dense); free_bb_plan(c->plan_bb);
-  dfree(c->tau); dfree(c->total_cost); dfree(c->fail_flag); dfree(c->d_eps_used); dfree(c->bar);
+  dfree(c->tau); dfree(c->total_cost); dfree(c->fail_flag); dfree(c->d_eps_used); dfree(c->bar); dfree(c->solve_stamps);
+  if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
   if (c->h_flag) cudaFreeHost(c->h_flag);
   if (c->h_scalar) cudaFreeHost(c->h_scalar);
   for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
 }
 
 inline void mark(Ctx* c, int i) { if (c->profiling) cudaEventRecord(c->ev[i], c->stream); }
+
+void drop_graph(Ctx* c) {
+  if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+  c->graph_exec = nullptr;
+  c->graph_steps = 0;
+}
 
 // a1-a5 (+ gradient and total cost): the block-sparse system at the current poses
 int build_blocks(Ctx* c) {
@@ -216,7 +271,12 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
   if (n_edges == 0) grp_ptr.assign(1, 0);
   c->n_groups = (int)grp_kf.size();
 
-  const size_t NHW = (size_t)c->N * c->HW, np2 = (size_t)c->npad * c->npad;
+  const size_t NHW = (size_t)c->N * c->HW;
+  {
+    int dev = 0;
+    CUB(cudaGetDevice(&dev));
+    CUB(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
+  }
   CUB(dev_alloc(&c->pm, NHW));
   CUB(upload(&c->edges, c->h_edges, c->stream));
   CUB(upload(&c->grp_kf, grp_kf, c->stream));
@@ -236,8 +296,6 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
   CUB(dev_alloc(&c->edge_cost, (size_t)c->E));
   CUB(dev_alloc(&c->n_valid, (size_t)c->E));
   CUB(dev_alloc(&c->checksum, (size_t)c->E));
-  CUB(dev_alloc(&c->Hd, np2));
-  CUB(dev_alloc(&c->L, np2));
   CUB(dev_alloc(&c->g, (size_t)c->npad));
   CUB(dev_alloc(&c->rhs, (size_t)c->npad));
   CUB(dev_alloc(&c->ysol, (size_t)c->npad));
@@ -247,6 +305,8 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
   CUB(dev_alloc(&c->fail_flag, 4));
   CUB(dev_alloc(&c->d_eps_used, 1));
   CUB(dev_alloc(&c->bar, 1));
+  CUB(dev_alloc(&c->solve_stamps, 16));
+  CUB(cudaMemsetAsync(c->solve_stamps, 0, 16 * sizeof(unsigned long long), c->stream));
   CUB(cudaMallocHost(reinterpret_cast<void**>(&c->h_flag), 4 * sizeof(int32_t)));
   CUB(cudaMallocHost(reinterpret_cast<void**>(&c->h_scalar), 4 * sizeof(double)));
   for (auto& ev : c->ev) CUB(cudaEventCreate(&ev));
@@ -290,6 +350,7 @@ int sim3ba_set_params(sim3ba_ctx* h, const sim3ba_params* p) {
   if (p->conf_min != c->prm.conf_min)
     return fail(c, SIM3BA_ERR_INVALID_ARG, "conf_min is fixed at sim3ba_create (the validity mask is baked into the packed pointmap)");
   c->prm = *p;
+  drop_graph(c);   // the constants are kernel arguments of the captured launches
   return SIM3BA_OK;
 }
 
@@ -317,6 +378,7 @@ int sim3ba_build_system(sim3ba_ctx* h) {
   tl_stream = c->stream;
   int rc = build_blocks(c);
   if (rc) return rc;
+  CU(ensure_dense(c, true, false));
   CU(launch_assemble(c, c->Hd, 0.0, 0.0, false));
   mark(c, 3);
   c->hd_valid = true;
@@ -372,6 +434,78 @@ int sim3ba_step(sim3ba_ctx* h) {
   return SIM3BA_OK;
 }
 
+int sim3ba_step_graph(sim3ba_ctx* h, int32_t n_steps) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  tl_stream = c->stream;
+  if (n_steps < 1 || n_steps > 4096) return fail(c, SIM3BA_ERR_INVALID_ARG, "n_steps must be in 1..4096");
+  if (!c->graph_exec || c->graph_steps != n_steps) {
+    drop_graph(c);
+    // everything that is not a stream operation (function attributes, occupancy, lazily allocated buffers) first
+    c->dense_loaded = false;
+    CU(prepare_accumulate(c));
+    if (c->solver_mode == 2 && c->plan_bb.valid) CU(prepare_solve_bb(c)); else CU(prepare_solve(c));
+    const bool prof = c->profiling;
+    c->profiling = false;                               // no event records inside the capture
+    const int64_t l0 = c->launches;
+    cudaGraph_t graph = nullptr;
+    // captured on a stream of the library's own (the caller's may be the legacy default stream, which cannot be
+    // captured); the launchers enqueue on c->stream, so it is swapped for the duration of the capture
+    cudaStream_t user_stream = c->stream, cap = nullptr;
+    cudaError_t e = cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking);
+    int rc = SIM3BA_OK;
+    if (e == cudaSuccess) e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+      c->stream = cap;
+      for (int it = 0; it < n_steps && rc == SIM3BA_OK; ++it) {
+        rc = build_blocks(c);
+        if (rc == SIM3BA_OK) rc = solve_impl(c);
+        if (rc == SIM3BA_OK && launch_retract(c) != cudaSuccess) rc = fail(c, SIM3BA_ERR_CUDA, "launch_retract during capture");
+      }
+      c->stream = user_stream;
+      cudaError_t e2 = cudaStreamEndCapture(cap, &graph);
+      if (e2 != cudaSuccess && rc == SIM3BA_OK) e = e2;
+    }
+    if (cap) cudaStreamDestroy(cap);
+    c->profiling = prof;
+    c->graph_launches = c->launches - l0;
+    c->launches = l0;
+    if (rc != SIM3BA_OK) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
+    if (e != cudaSuccess || !graph) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return cuda_fail(c, e, "stream capture of the GN step"); }
+    e = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { c->graph_exec = nullptr; return cuda_fail(c, e, "cudaGraphInstantiate"); }
+    c->graph_steps = n_steps;
+  }
+  CU(cudaGraphLaunch(c->graph_exec, c->stream));
+  c->launches += c->graph_launches;
+  c->hd_valid = false; c->built = false; c->solved = false;
+  c->status_stale = true;
+  return SIM3BA_OK;
+}
+
+int sim3ba_get_solve_phase_us(sim3ba_ctx* h, float us[8]) {
+  if (!h || !us) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  tl_stream = c->stream;
+  unsigned long long st[16];
+  CU(cudaMemcpyAsync(st, c->solve_stamps, sizeof(st), cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < 8; ++k) us[k] = 0.f;
+  if (st[6] > st[0] && st[0] != 0ull)
+    for (int k = 0; k < 6; ++k) us[k] = st[k + 1] >= st[k] ? (float)((double)(st[k + 1] - st[k]) * 1e-3) : 0.f;
+  return SIM3BA_OK;
+}
+
+int sim3ba_release_memory(void) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return SIM3BA_ERR_CUDA;
+  cudaMemPool_t pool;
+  if (lib_pool(&pool) != cudaSuccess) return SIM3BA_ERR_CUDA;
+  if (cudaDeviceSynchronize() != cudaSuccess) return SIM3BA_ERR_CUDA;
+  return cudaMemPoolTrimTo(pool, 0) == cudaSuccess ? SIM3BA_OK : SIM3BA_ERR_CUDA;
+}
+
 int sim3ba_step_host(sim3ba_ctx* h, const double* h_in, double* h_out, double* h_cost) {
   if (!h) return SIM3BA_ERR_INVALID_ARG;
   Ctx* c = &h->c;
@@ -402,20 +536,12 @@ int sim3ba_optimize_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_
   int32_t *d_edges = nullptr, *d_match = nullptr;
   sim3ba_ctx* h = nullptr;
   int rc = SIM3BA_OK;
-  // the graph buffers come from the device's stream-ordered pool, kept warm between jobs (no map / unmap per job)
-  {
-    int dev = 0;
-    cudaMemPool_t pool;
-    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-      uint64_t keep = UINT64_MAX;
-      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-    }
-  }
+  // the graph buffers come from the library's own stream-ordered pool, kept warm between jobs (no map / unmap per job)
   auto cleanup = [&]() {
     if (h) sim3ba_destroy(h);                                   // synchronises the stream
     cudaFreeAsync(d_points, st); cudaFreeAsync(d_conf, st); cudaFreeAsync(d_edges, st); cudaFreeAsync(d_match, st);
   };
-  auto pool_alloc = [&](void** ptr, size_t bytes) { return cudaMallocAsync(ptr, std::max<size_t>(bytes, 16), st); };
+  auto pool_alloc = [&](void** ptr, size_t bytes) { return dmalloc(ptr, bytes); };
 #define CUJ(call)                                                       \
   do {                                                                  \
     cudaError_t e_ = (call);                                            \
@@ -587,9 +713,11 @@ int sim3ba_load_system(sim3ba_ctx* h, const double* d_H, const double* d_g) {
   Ctx* c = &h->c;
   tl_stream = c->stream;
   if (!d_H || !d_g) return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL system pointer");
+  CU(ensure_dense(c, true, false));
   CU(cudaMemcpyAsync(c->Hd, d_H, (size_t)c->n * c->n * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
   CU(launch_load_gradient(c, d_g));
   c->dense_loaded = true; c->hd_valid = false; c->built = false; c->solved = false;
+  drop_graph(c);
   return SIM3BA_OK;
 }
 
@@ -599,6 +727,7 @@ int sim3ba_set_solver_mode(sim3ba_ctx* h, int32_t mode) {
   tl_stream = c->stream;
   if (mode < 0 || mode > 2) return fail(c, SIM3BA_ERR_INVALID_ARG, "solver mode must be 0 (tile-sparse), 1 (dense) or 2 (band + border)");
   c->solver_mode = mode;
+  drop_graph(c);
   return SIM3BA_OK;
 }
 

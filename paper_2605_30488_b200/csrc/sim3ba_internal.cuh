@@ -11,11 +11,18 @@
 
 namespace sim3ba {
 
-// Device memory of the library comes from the device's stream-ordered pool on the stream of the running API call
-// (set on entry of every entry point that may allocate or free): no device-wide synchronisation per allocation, and
-// a caller that keeps the pool warm (sim3ba_optimize_host does) pays no map / unmap per context.
+// Device memory of the library comes from a stream-ordered memory pool OWNED BY THE LIBRARY (one per device, created on
+// first use, release threshold = keep everything until sim3ba_release_memory), on the stream of the running API call
+// (set on entry of every entry point that may allocate or free): no device-wide synchronisation per allocation, a warm
+// pool costs no map / unmap per context, and the device's default pool (PyTorch's, the caller's) is left alone.
 inline thread_local cudaStream_t tl_stream = nullptr;
-inline cudaError_t dmalloc(void** p, size_t bytes) { return cudaMallocAsync(p, bytes < 16 ? 16 : bytes, tl_stream); }
+cudaError_t lib_pool(cudaMemPool_t* pool);          // the library's pool on the current device (sim3ba_api.cu)
+inline cudaError_t dmalloc(void** p, size_t bytes) {
+  cudaMemPool_t pool;
+  cudaError_t e = lib_pool(&pool);
+  if (e != cudaSuccess) return e;
+  return cudaMallocFromPoolAsync(p, bytes < 16 ? 16 : bytes, pool, tl_stream);
+}
 inline void dfree(void* p) { if (p) cudaFreeAsync(p, tl_stream); }
 
 constexpr int kAccThreads = 32;      // accumulate CTA: ONE warp -- warps are independent workers, so the finest CTA gives the block
@@ -126,6 +133,7 @@ struct Ctx {
   int32_t* fail_flag = nullptr;    // [4] device: [0] failure flag, [1] attempts used, [2] solved
   double* d_eps_used = nullptr;    // [1] device
   unsigned int* bar = nullptr;     // [1] device: grid-barrier counter of k_solve
+  unsigned long long* solve_stamps = nullptr;   // [16] device: globaltimer stamps of the phases of k_solve_bb (profiling only)
   int32_t* h_flag = nullptr;       // pinned
   double* h_scalar = nullptr;      // pinned [4]
   bool built = false, solved = false, dense_loaded = false, hd_valid = false, status_stale = false;
@@ -133,6 +141,15 @@ struct Ctx {
   double eps_used = 0.0;
   int64_t launches = 0;
   int last_solve_grid = 0;
+  // per-context launch configuration (function attributes and occupancy are per device: nothing process-wide is cached)
+  int num_sms = 0;
+  bool acc_ready = false;
+  int solve_bpsm = -1, bb_bpsm = -1;     // resident CTAs per SM of k_solve / k_solve_bb at their shared-memory size
+  size_t bb_smem = 0;
+  // sim3ba_step_graph: n GN iterations captured once as a CUDA graph
+  cudaGraphExec_t graph_exec = nullptr;
+  int graph_steps = 0;
+  int64_t graph_launches = 0;
   bool profiling = false;
   cudaEvent_t ev[8] = {};
   float phase_ms[8] = {};
@@ -142,6 +159,11 @@ struct Ctx {
 // kernel launchers (each returns the cudaError of the launch)
 cudaError_t launch_pack(Ctx* c, const float* d_points, const float* d_conf);
 cudaError_t launch_accumulate(Ctx* c);                   // kernels 1+2: partials -> blocks35, stats, cost
+// function attributes / occupancy / lazily allocated work buffers of the launchers, done outside a stream capture
+cudaError_t prepare_accumulate(Ctx* c);
+cudaError_t prepare_solve(Ctx* c);
+cudaError_t prepare_solve_bb(Ctx* c);
+cudaError_t ensure_dense(Ctx* c, bool want_Hd, bool want_L);   // Hd (read-back / loaded system) and L (tile plans) exist only when used
 cudaError_t launch_assemble(Ctx* c, double* dst, double lambda, double eps, bool from_dense);  // kernel 3
 cudaError_t launch_gradient(Ctx* c);                     // g from the per-edge b_e
 cudaError_t launch_load_gradient(Ctx* c, const double* d_g);

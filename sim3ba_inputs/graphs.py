@@ -13,6 +13,8 @@ stream and generation is order independent.
 """
 from __future__ import annotations
 
+import os
+from concurrent.futures import ThreadPoolExecutor
 from dataclasses import dataclass, field, replace
 from typing import Dict, List, Optional, Tuple
 
@@ -83,6 +85,14 @@ def _haar_quat(rng: np.random.Generator) -> np.ndarray:
     return q / np.linalg.norm(q)
 
 
+def _n_threads() -> int:
+    try:
+        n = len(os.sched_getaffinity(0))
+    except AttributeError:  # pragma: no cover
+        n = os.cpu_count() or 1
+    return max(1, min(32, n))
+
+
 # ----------------------------------------------------------------------------------------------
 @dataclass(frozen=True)
 class GraphSpec:
@@ -147,8 +157,8 @@ class Graph:
     agent: np.ndarray         # [N] int32, a(i)
     fixed_kf: np.ndarray      # int32 list of gauge keyframes
     poses_gt: np.ndarray      # [N, 8] float64
-    poses_init: np.ndarray    # [N, 8] float64 (config 3: gauge-synchronised)
-    poses_init_raw: Optional[np.ndarray] = None   # config 3 only: independent gauges
+    poses_init: np.ndarray    # [N, 8] float64 (config 3: the raw start below; synchronise with meta['gauge_sync_plan'])
+    poses_init_raw: Optional[np.ndarray] = None   # config 3 only: independent per-agent gauges
     segments: Optional[np.ndarray] = None         # [HW] int32 segment label grid (config 5)
     meta: Dict[str, object] = field(default_factory=dict)
 
@@ -288,38 +298,6 @@ def _perturb(pose: np.ndarray, rng: np.random.Generator) -> np.ndarray:
     return _compose(d, pose)
 
 
-def _umeyama(x: np.ndarray, y: np.ndarray) -> np.ndarray:
-    """Closed-form similarity mapping y onto x (input preparation for config 3's synced start)."""
-    mx, my = x.mean(0), y.mean(0)
-    xc, yc = x - mx, y - my
-    A = xc.T @ yc / x.shape[0]
-    U, lam, Vt = np.linalg.svd(A)
-    Sg = np.diag([1.0, 1.0, np.sign(np.linalg.det(U @ Vt))])
-    R = U @ Sg @ Vt
-    s = np.trace(Sg @ np.diag(lam)) / (yc ** 2).sum(1).mean()
-    t = mx - s * R @ my
-    # rotation matrix -> quaternion (xyzw)
-    w = np.sqrt(max(0.0, 1.0 + R[0, 0] + R[1, 1] + R[2, 2])) / 2.0
-    if w > 1e-6:
-        q = np.array([(R[2, 1] - R[1, 2]) / (4 * w), (R[0, 2] - R[2, 0]) / (4 * w),
-                      (R[1, 0] - R[0, 1]) / (4 * w), w])
-    else:
-        i = int(np.argmax(np.diag(R)))
-        j, k = (i + 1) % 3, (i + 2) % 3
-        r = np.sqrt(max(0.0, 1.0 + R[i, i] - R[j, j] - R[k, k]))
-        q = np.zeros(4)
-        q[i] = r / 2.0
-        q[j] = (R[j, i] + R[i, j]) / (2 * r)
-        q[k] = (R[k, i] + R[i, k]) / (2 * r)
-        q[3] = (R[k, j] - R[j, k]) / (2 * r)
-    q /= np.linalg.norm(q)
-    return np.concatenate([t, q, [s]])
-
-
-def _apply(pose: np.ndarray, X: np.ndarray) -> np.ndarray:
-    return pose[7] * X @ _quat_to_mat(pose[3:7]).T + pose[0:3]
-
-
 def make_graph(spec: GraphSpec) -> Graph:
     scene = _make_scene(spec)
     poses_gt = _make_gt_poses(spec)
@@ -327,19 +305,28 @@ def make_graph(spec: GraphSpec) -> Graph:
     N, HW = spec.n_kf, spec.hw
     points = np.empty((N, HW, 3), dtype=np.float32)
     conf = np.empty((N, HW), dtype=np.float32)
-    for k in range(N):
-        points[k], conf[k] = _make_keyframe(spec, k, scene, poses_gt[k], int(o[k]))
     edges, kind, frac = _make_edges(spec)
     E = edges.shape[0]
     match = np.empty((E, HW), dtype=np.int32)
-    for e in range(E):
+
+    def fill_keyframe(k: int) -> None:
+        points[k], conf[k] = _make_keyframe(spec, k, scene, poses_gt[k], int(o[k]))
+
+    def fill_match(e: int) -> None:
         match[e] = _make_match(spec, e, int(o[edges[e, 0]]), int(o[edges[e, 1]]), float(frac[e]))
+
+    # every keyframe / edge draws from its own stream, so the order (and the thread) does not matter; NumPy's
+    # generators and gathers release the GIL
+    with ThreadPoolExecutor(max_workers=_n_threads()) as pool:
+        list(pool.map(fill_keyframe, range(N)))
+        list(pool.map(fill_match, range(E)))
     agent = np.repeat(np.arange(spec.n_agents, dtype=np.int32), spec.kf_per_agent)
 
     poses_init = poses_gt.copy()
     for k in range(1, N):
         poses_init[k] = _perturb(poses_gt[k], _rng(spec.seed, _K_INIT, k))
     poses_raw = None
+    sync_plan: List[Tuple[int, List[int], bool]] = []    # (linking edge, moving keyframes, moving component is i's)
     if spec.agent_gauge and spec.n_agents > 1:
         poses_raw = poses_init.copy()
         for a in range(1, spec.n_agents):
@@ -348,22 +335,16 @@ def make_graph(spec: GraphSpec) -> Graph:
                                 [np.exp(rng.uniform(np.log(0.3), np.log(3.0)))]])
             for k in range(a * spec.kf_per_agent, (a + 1) * spec.kf_per_agent):
                 poses_raw[k] = _compose(G, poses_init[k])
-        # gauge synchronisation on the first inter-agent edge of each moving agent
-        poses_init = poses_raw.copy()
+        # The start handed out is the RAW one: the components are brought into one gauge by the method itself
+        # (sim3ba_gauge_sync on the device, oracle/gauge_sync_oracle.py in the tests), on the first
+        # inter-agent edge of each moving agent, in this order.  The plan below is bookkeeping only.
+        poses_init = poses_raw
         for a in range(1, spec.n_agents):
             es = [e for e in range(E) if kind[e] == 2 and
                   {int(agent[edges[e, 0]]), int(agent[edges[e, 1]])} == {a - 1, a}]
             e = es[0]
-            i, j = int(edges[e, 0]), int(edges[e, 1])
-            mm = np.flatnonzero(match[e] >= 0)
-            xi = _apply(poses_init[i], points[i, mm].astype(np.float64))
-            yj = _apply(poses_init[j], points[j, match[e, mm]].astype(np.float64))
-            if agent[i] == a:                    # i is on the moving component
-                Tst = _umeyama(yj, xi)
-            else:
-                Tst = _umeyama(xi, yj)
-            for k in range(a * spec.kf_per_agent, (a + 1) * spec.kf_per_agent):
-                poses_init[k] = _compose(Tst, poses_init[k])
+            moving = list(range(a * spec.kf_per_agent, (a + 1) * spec.kf_per_agent))
+            sync_plan.append((int(e), moving, bool(agent[edges[e, 0]] == a)))
 
     segments = None
     if spec.n_segments[0] > 0:
@@ -375,7 +356,7 @@ def make_graph(spec: GraphSpec) -> Graph:
     return Graph(spec=spec, points=points, conf=conf, edges=edges, match=match, edge_kind=kind,
                  agent=agent, fixed_kf=np.array([0], dtype=np.int32), poses_gt=poses_gt,
                  poses_init=poses_init, poses_init_raw=poses_raw, segments=segments,
-                 meta=dict(valid_frac_target=frac))
+                 meta=dict(valid_frac_target=frac, gauge_sync_plan=sync_plan))
 
 
 def make_config(k: int, **scaled) -> Graph:

@@ -1,7 +1,11 @@
 """Shared helpers of the GPU parity tests: move a seeded graph to the device, wrap oracle outputs
 in the layouts of the C ABI, relative-error norms.  No arithmetic of the method lives here."""
+import json
+import os
+
 import numpy as np
 
+from oracle import gauge_sync_oracle as gs
 from oracle import sim3_gn_oracle as orc
 from sim3ba_inputs import PRESETS
 
@@ -51,3 +55,23 @@ def rel(a: np.ndarray, b: np.ndarray, floor: float = 0.0) -> float:
 
 def free_idx(g, fixed=None):
     return orc.free_index(g.n_kf, g.fixed_kf if fixed is None else fixed)
+
+
+def start_poses(g, prm: orc.Params) -> np.ndarray:
+    """The seeded start of a graph.  Config 3 hands out independent per-agent gauges plus the plan to synchronise them
+    (PAPER.md:92-104); here the ORACLE's gauge synchronisation executes the plan, so no oracle input ever comes from the
+    CUDA path (sim3ba_gauge_sync itself is compared with it in tests/test_gpu_gauge_sync.py)."""
+    poses = g.poses_init.copy()
+    for e, moving, moving_is_i in g.meta.get("gauge_sync_plan", []):
+        poses, _, _ = gs.gauge_sync(poses, g.points, g.conf, g.edges[e], g.match[e], moving, prm.conf_min, moving_is_i)
+    return poses
+
+
+def parity_log(**rec):
+    """Appends one record of measured parity errors to $SIM3BA_PARITY_LOG (JSON lines) -- the table of DESIGN.md
+    "Parity protocol" is made from these; without the variable nothing is written."""
+    path = os.environ.get("SIM3BA_PARITY_LOG")
+    if not path:
+        return
+    with open(path, "a") as f:
+        f.write(json.dumps({k: (float(v) if isinstance(v, (np.floating, float)) else v) for k, v in rec.items()}) + "\n")

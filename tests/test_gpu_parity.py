@@ -3,26 +3,27 @@
 Bars (BASELINE.json north_star): bit-exact on edge/index bookkeeping and the gathered match set
 (per-edge n_valid and checksum); <= 1e-4 relative Frobenius on per-edge blocks, H and g;
 <= 1e-3 relative on the pose update tau.  Floors for converged iterations follow DESIGN.md
-"Parity protocol": gradients (per edge and assembled) against max(||g||, FLOOR_G ||g_abs||) with
-g_abs = sum |J^T| Omega |e| from the oracle and FLOOR_G = 2^-23 / 1e-4 (every term J^T Omega e is
-evaluated in fp32, i.e. to ~2^-23 relative; worst case without any averaging), tau against
-max(||tau||, 1e-6 sqrt(n)).
+"Parity protocol": gradients (per edge and assembled) against
+max(||g||, FLOOR_G ||g_abs||) with g_abs = sum |J^T| Omega |e| from the oracle and FLOOR_G = 1e-6, tau against
+max(||tau||, 1e-6 sqrt(n)).  Every check_system call appends its measured errors, ||g|| / ||g_abs|| and whether a floor
+was the active bound to $SIM3BA_PARITY_LOG (the table in DESIGN.md).
 """
 import numpy as np
 import pytest
 
 from oracle import sim3_gn_oracle as orc
+from oracle.edge_pool import build_system_parallel
 from sim3ba_inputs import CONFIGS, make_config, make_graph
 from tests.gpu_common import (TOL_BLOCK, TOL_TAU, blocks35_from_oracle, free_idx, make_solver, oracle_params,
-                              rel, set_poses, sym_from_lower)
+                              parity_log, rel, set_poses, start_poses, sym_from_lower)
 
 pytestmark = pytest.mark.gpu
 
-FLOOR_G = 2.0 ** -23 / TOL_BLOCK
+FLOOR_G = 1e-6
 
 
 def reduced(k):
-    """Reduced variants: several 4096-pixel tiles per edge plus a ragged tail."""
+    """Reduced variants: several 512-pixel slices per edge plus a ragged tail."""
     if k == 2:
         return CONFIGS[2].scaled(kf_per_agent=8, height=100, width=130, n_scene=20_000)
     if k == 3:
@@ -34,31 +35,51 @@ def reduced(k):
     raise KeyError(k)
 
 
-def check_system(ba, g, poses, prm, tag=""):
-    """One lock-step comparison at the given poses; returns (oracle system, oracle solution)."""
+def check_system(ba, g, poses, prm, tag="", pool=False):  # noqa: C901
+    """One lock-step comparison at the given poses; returns (oracle system, oracle solution).  ``pool``: the unchanged
+    oracle runs edge-parallel on every host core (oracle/edge_pool.py) -- the full-size configs."""
     set_poses(ba, poses)
     ba.build_system()
     ba.solve()
-    sysm = orc.build_system(poses, g.points, g.conf, g.edges, g.match, prm)
+    if pool:
+        sysm = build_system_parallel(poses, g.points, g.conf, g.edges, g.match, prm)
+    else:
+        sysm = orc.build_system(poses, g.points, g.conf, g.edges, g.match, prm)
     sol = orc.solve(sysm.H, sysm.g, g.fixed_kf, prm)
     nv, chk, cost_e = (t.cpu().numpy() for t in ba.edge_stats())
     assert np.array_equal(nv.astype(np.int64), sysm.n_valid), tag
     assert np.array_equal(chk.view(np.uint64), sysm.checksum), tag
     blk = ba.edge_blocks().cpu().numpy()
     ref = blocks35_from_oracle(sysm)
+    err_A, err_b = 0.0, 0.0
     for e in range(g.n_edges):
         if sysm.n_valid[e] == 0:
             assert np.all(blk[e] == 0.0)
             continue
+        err_A = max(err_A, rel(blk[e, :28], ref[e, :28]))
+        err_b = max(err_b, rel(blk[e, 28:], ref[e, 28:], FLOOR_G * np.linalg.norm(sysm.edge_b_abs[e])))
         assert rel(blk[e, :28], ref[e, :28]) <= TOL_BLOCK, (tag, e)
         assert rel(blk[e, 28:], ref[e, 28:], FLOOR_G * np.linalg.norm(sysm.edge_b_abs[e])) <= TOL_BLOCK, (tag, e)
     assert rel(cost_e, sysm.edge_cost) <= TOL_BLOCK, tag
     Hl, gg = (t.cpu().numpy() for t in ba.system())
     fr = free_idx(g)
     Hs = sym_from_lower(Hl)
-    assert rel(Hs[np.ix_(fr, fr)], sysm.H[np.ix_(fr, fr)]) <= TOL_BLOCK, tag
-    g_floor = FLOOR_G * np.linalg.norm(sysm.g_abs[fr])
-    assert rel(gg[fr], sysm.g[fr], g_floor) <= TOL_BLOCK, tag
+    del Hl
+    err_H = rel(Hs[np.ix_(fr, fr)], sysm.H[np.ix_(fr, fr)])
+    g_norm, g_abs_norm = np.linalg.norm(sysm.g[fr]), np.linalg.norm(sysm.g_abs[fr])
+    g_floor = FLOOR_G * g_abs_norm
+    err_g = rel(gg[fr], sysm.g[fr], g_floor)
+    tau, attempts, eps, cost = ba.update()
+    tau = tau.cpu().numpy()
+    tau_floor = 1e-6 * np.sqrt(tau.size)
+    err_tau = rel(tau, sol.tau, tau_floor)
+    parity_log(tag=tag, n_kf=g.n_kf, n_edges=g.n_edges, hw=g.hw, n_valid=int(sysm.n_valid.sum()), err_edge_A_max=err_A,
+               err_edge_b_max=err_b, err_H=err_H, err_g=err_g, err_tau=err_tau, g_over_g_abs=g_norm / max(g_abs_norm, 1e-300),
+               g_err_over_g_abs=float(np.linalg.norm(gg[fr] - sysm.g[fr]) / max(g_abs_norm, 1e-300)),
+               g_floor_active=bool(g_norm < g_floor), tau_norm=float(np.linalg.norm(sol.tau)),
+               tau_floor_active=bool(np.linalg.norm(sol.tau) < tau_floor), attempts=int(attempts))
+    assert err_H <= TOL_BLOCK, tag
+    assert err_g <= TOL_BLOCK, tag
     # gauge rows/cols: identity block, zero gradient
     for k in g.fixed_kf:
         s = slice(7 * k, 7 * k + 7)
@@ -66,11 +87,8 @@ def check_system(ba, g, poses, prm, tag=""):
         Hs_off = Hs[s, :].copy()
         Hs_off[:, s] = 0.0
         assert np.all(Hs_off == 0.0)
-    tau, attempts, eps, cost = ba.update()
-    tau = tau.cpu().numpy()
     assert attempts == sol.attempts and (eps == sol.eps_used), tag
-    tau_floor = 1e-6 * np.sqrt(tau.size)
-    assert rel(tau, sol.tau, tau_floor) <= TOL_TAU, tag
+    assert err_tau <= TOL_TAU, tag
     assert rel(np.array([cost]), np.array([sysm.cost])) <= TOL_BLOCK
     for k in g.fixed_kf:
         assert np.all(tau[7 * k:7 * k + 7] == 0.0)
@@ -100,7 +118,7 @@ def test_reduced_configs_lockstep(k, preset):
     bk, ref = ba.bookkeeping(), orc.bookkeeping(g.n_kf, g.edges)
     for key in ref:
         assert np.array_equal(bk[key], ref[key]), key
-    poses = g.poses_init.copy()
+    poses = start_poses(g, prm)
     for it in range(4):
         sysm, sol = check_system(ba, g, poses, prm, f"C{k}r/{preset}/it{it}")
         poses = orc.retract(poses, sol.tau)
@@ -114,18 +132,19 @@ def test_free_running_matches_oracle(k):
     g = make_config(1) if k == 1 else make_graph(reduced(k))
     prm = oracle_params("config")
     ba = make_solver(g, prm)
-    set_poses(ba, g.poses_init)
-    poses = g.poses_init.copy()
+    p0 = start_poses(g, prm)
+    set_poses(ba, p0)
+    poses = p0.copy()
     n_it = max(1, min(g.spec.n_iters, 5))
     for _ in range(n_it):
         ba.step()
         poses, _, _ = orc.gn_step(poses, g.points, g.conf, g.edges, g.match, g.fixed_kf, prm)
     out = ba.get_poses().cpu().numpy()
-    d_gpu = np.concatenate([orc.pose_delta_log(out[i], g.poses_init[i]) for i in range(g.n_kf)])
-    d_orc = np.concatenate([orc.pose_delta_log(poses[i], g.poses_init[i]) for i in range(g.n_kf)])
+    d_gpu = np.concatenate([orc.pose_delta_log(out[i], p0[i]) for i in range(g.n_kf)])
+    d_orc = np.concatenate([orc.pose_delta_log(poses[i], p0[i]) for i in range(g.n_kf)])
     assert rel(d_gpu, d_orc) <= TOL_TAU
     assert np.allclose(np.linalg.norm(out[:, 3:7], axis=1), 1.0, atol=1e-14)
-    assert np.array_equal(out[0], g.poses_init[0])
+    assert np.array_equal(out[0], p0[0])
     ba.close()
 
 
@@ -239,7 +258,8 @@ def test_solver_modes_agree(k, monkeypatch):
     systems) and each within the north_star 1e-3 of the oracle.  Mode 2 also with short segments (separators)."""
     g = make_config(1) if k == 1 else make_graph(reduced(k))
     prm = oracle_params("config")
-    sysm = orc.build_system(g.poses_init, g.points, g.conf, g.edges, g.match, prm)
+    p0 = start_poses(g, prm)
+    sysm = orc.build_system(p0, g.points, g.conf, g.edges, g.match, prm)
     sol = orc.solve(sysm.H, sysm.g, g.fixed_kf, prm)
     tau_floor = 1e-6 * np.sqrt(sol.tau.size)
     taus = {}
@@ -254,7 +274,7 @@ def test_solver_modes_agree(k, monkeypatch):
         if lmax is not None:
             assert info["max_segment"] <= 5
         ba.set_solver_mode(mode)
-        set_poses(ba, g.poses_init)
+        set_poses(ba, p0)
         ba.build_system()
         ba.solve()
         tau, attempts, eps, _ = ba.update()
@@ -333,72 +353,41 @@ def test_create_rejects_bad_arguments():
     ba.close()
 
 
-def test_config2_full_size_sampled_edges():
-    """BASELINE configs[1] at full size (the bench workload): every edge's match set bit-exact,
-    a sample of per-edge blocks against the oracle, and H, g, tau from the oracle run on all edges."""
+def test_config2_full_size_all_edges():
+    """BASELINE configs[1] at full size: every edge's match set bit-exact, every per-edge block, H, g and tau against the
+    oracle run on all edges."""
     g = make_config(2)
     prm = oracle_params("config")
     ba = make_solver(g, prm)
-    check_system(ba, g, g.poses_init, prm, "C2-full")
+    check_system(ba, g, g.poses_init, prm, "C2-full/config/it0", pool=True)
     ba.close()
 
 
-def test_config4_full_size_sampled_edges_and_solver_property():
-    """BASELINE configs[3] at full size (1000 keyframes, 3036 edges, 7000 x 7000 system, the launch configuration bench.py
-    times): the match set of EVERY edge bit-exact against the validity rule written out in NumPy, the 7x7 blocks of a sample of
-    edges (first, last, every inter-agent tenth, a stride through the chains) against the oracle, and the update tau against
-    SciPy's dense Cholesky of the system assembled in NumPy from the GPU's own per-edge blocks (decomposition: a1-a5 vs the
-    oracle on samples, a6-a7 vs a library solve on the whole system)."""
-    import scipy.linalg
-    g = make_config(4)
-    prm = oracle_params("config")
+@pytest.mark.parametrize("k,preset", [(3, "config"), (3, "paper"), (4, "config"), (4, "paper"), (5, "config")])
+def test_full_size_vs_oracle(k, preset):
+    """BASELINE configs[2..4] at FULL size, in the launch configuration bench.py times (C3: 200 keyframes 512x384, 608
+    edges; C4: 1000 keyframes 256x192, 3036 edges, n = 7000; C5: 2000 keyframes 512x384, 6003 edges, 1.18e9 candidate
+    matches, n = 14000), iteration 0 from the seeded start: every edge's n_valid / checksum bit-exact, ALL per-edge blocks,
+    the assembled H and g on the free blocks (<= 1e-4) and tau against orc.solve of the ORACLE's own H, g (<= 1e-3; this
+    is where cond(H) ~ 1e8-1e10 amplifies the fp32 per-match arithmetic).  The unchanged NumPy
+    oracle runs edge-parallel on the host cores (oracle/edge_pool.py).  C3 starts from the independent per-agent gauges
+    brought together by the oracle's gauge synchronisation; the device's own sim3ba_gauge_sync on the same
+    raw start must land on the same poses."""
+    g = make_config(k)
+    prm = oracle_params(preset)
     ba = make_solver(g, prm)
-    set_poses(ba, g.poses_init)
-    ba.build_system()
-    ba.solve()
-    nv, chk, _ = (t.cpu().numpy() for t in ba.edge_stats())
-    blk = ba.edge_blocks().cpu().numpy()
-    tau, attempts, eps, _ = ba.update()
-    tau = tau.cpu().numpy()
-    HW = g.hw
-    for e in range(g.n_edges):                                 # R12, typed out: 0 <= n < HW, c_i[m] > c_min, c_j[n] > c_min
-        i, j = g.edges[e]
-        n = g.match[e].astype(np.int64)
-        m = np.flatnonzero((n >= 0) & (n < HW))
-        m = m[(g.conf[i, m] > prm.conf_min) & (g.conf[j, n[m]] > prm.conf_min)]
-        assert nv[e] == m.size, e
-        with np.errstate(over="ignore"):
-            ref = np.sum(m.astype(np.uint64) * np.uint64(HW) + n[m].astype(np.uint64), dtype=np.uint64)
-        assert chk.view(np.uint64)[e] == ref, e
-    inter = np.flatnonzero(g.edge_kind == 2)
-    sample = sorted(set([0, g.n_edges - 1] + list(inter[::10]) + list(range(5, g.n_edges, 211))))
-    sysm = orc.build_system(g.poses_init, g.points, g.conf, g.edges, g.match, prm, edge_subset=sample)
-    ref = blocks35_from_oracle(sysm)
-    for e in sample:
-        assert rel(blk[e, :28], ref[e, :28]) <= TOL_BLOCK, e
-        assert rel(blk[e, 28:], ref[e, 28:], FLOOR_G * np.linalg.norm(sysm.edge_b_abs[e])) <= TOL_BLOCK, e
-    # a6 + a7 on the whole system: assemble H, g from the GPU's blocks (two diagonal, one off-diagonal block per edge,
-    # PAPER.md:118), delete the gauge rows (PAPER.md:108), eps_0 on the diagonal (Eq. (7)), library Cholesky
-    n = 7 * g.n_kf
-    H, gg = np.zeros((n, n)), np.zeros(n)
-    iu = np.triu_indices(7)
-    for e in range(g.n_edges):
-        i, j = (int(v) for v in g.edges[e])
-        A = np.zeros((7, 7))
-        A[iu] = blk[e, :28]
-        A = A + A.T - np.diag(np.diag(A))
-        si, sj = slice(7 * i, 7 * i + 7), slice(7 * j, 7 * j + 7)
-        H[si, si] += A
-        H[sj, sj] += A
-        H[si, sj] -= A
-        H[sj, si] -= A
-        gg[sj] += blk[e, 28:]
-        gg[si] -= blk[e, 28:]
-    fr = free_idx(g)
-    Hf = H[np.ix_(fr, fr)] + prm.eps0 * np.eye(fr.size)
-    ref_tau = np.zeros(n)
-    ref_tau[fr] = -scipy.linalg.cho_solve(scipy.linalg.cho_factor(Hf, lower=True), gg[fr])
-    assert attempts == 1 and eps == prm.eps0
-    assert rel(tau, ref_tau) <= 1e-6
+    bk, ref = ba.bookkeeping(), orc.bookkeeping(g.n_kf, g.edges)
+    for key in ref:
+        assert np.array_equal(bk[key], ref[key]), key
+    p0 = start_poses(g, prm)
+    if g.meta.get("gauge_sync_plan"):
+        set_poses(ba, g.poses_init)
+        for e, moving, moving_is_i in g.meta["gauge_sync_plan"]:
+            ba.gauge_sync(e, moving, moving_is_i)
+        dev = ba.get_poses().cpu().numpy()
+        sgn = np.sign(np.sum(dev[:, 3:7] * p0[:, 3:7], axis=1, keepdims=True))
+        assert np.allclose(dev[:, :3], p0[:, :3], rtol=0, atol=1e-9 * max(1.0, np.abs(p0[:, :3]).max()))
+        assert np.allclose(dev[:, 3:7], sgn * p0[:, 3:7], rtol=0, atol=1e-9) and np.allclose(dev[:, 7], p0[:, 7], rtol=1e-9)
+    check_system(ba, g, p0, prm, f"C{k}-full/{preset}/it0", pool=True)
     assert ba.bb_info()["valid"] == 1
     ba.close()

@@ -35,7 +35,9 @@ def test_config1_is_deterministic_and_has_stated_fractions():
 def test_reduced_config3_has_two_gauges():
     g = make_graph(CONFIGS[3].scaled(kf_per_agent=6, height=12, width=16, n_inter=2))
     assert g.poses_init_raw is not None and g.n_kf == 12
-    assert not np.allclose(g.poses_init_raw[6:], g.poses_init[6:])
-    assert np.array_equal(g.poses_init_raw[:6], g.poses_init[:6])
+    assert np.array_equal(g.poses_init_raw, g.poses_init)        # the start handed out is the raw one ...
+    (e, moving, moving_is_i), = g.meta["gauge_sync_plan"]            # ... with the plan to synchronise it by the method
+    assert g.edge_kind[e] == 2 and moving == list(range(6, 12))
+    assert g.agent[g.edges[e, 0 if moving_is_i else 1]] == 1
     s_ratio = g.poses_init_raw[6:, 7] / g.poses_gt[6:, 7]
     assert 0.25 < s_ratio.mean() < 3.5

@@ -259,3 +259,23 @@ def test_bookkeeping_bruteforce():
     assert bk["pair_kf"].tolist() == [[1, 0], [2, 0], [2, 1], [3, 1]]
     assert bk["pair_ptr"].tolist() == [0, 2, 3, 5, 6]
     assert bk["pair_edge"].tolist() == [0, 4, 3, 1, 2, 5]
+
+
+def test_edge_pool_is_bit_identical_to_the_serial_oracle():
+    """oracle/edge_pool.py runs the unchanged oracle one edge per call in worker processes and adds the 14 x 14 corners in
+    edge order: every output equals the serial build_system bit for bit (duplicate and reversed edges included)."""
+    from oracle.edge_pool import build_system_parallel
+    g = make_graph(CONFIGS[3].scaled(kf_per_agent=5, height=20, width=30, n_scene=2_000, n_inter=3))
+    edges = np.concatenate([g.edges, g.edges[:2, ::-1], g.edges[3:4]]).astype(np.int32)      # (j, i) and a duplicate
+    match = np.concatenate([g.match, g.match[:2], g.match[3:4]])
+    prm = orc.Params(sigma_ray=1.0, sigma_dist=1.0, huber_k=0.05, conf_min=0.2)
+    ref = orc.build_system(g.poses_init, g.points, g.conf, edges, match, prm)
+    for nw in (1, 3):
+        par = build_system_parallel(g.poses_init, g.points, g.conf, edges, match, prm, n_workers=nw)
+        for name in ("H", "g", "g_abs", "n_valid", "checksum", "edge_A", "edge_b", "edge_cost", "edge_b_abs"):
+            assert np.array_equal(getattr(par, name), getattr(ref, name)), (nw, name)
+        assert par.cost == ref.cost
+    sub = [1, 4, 7]
+    par = build_system_parallel(g.poses_init, g.points, g.conf, edges, match, prm, edge_subset=sub, n_workers=2, dense=False)
+    ref = orc.build_system(g.poses_init, g.points, g.conf, edges, match, prm, edge_subset=sub)
+    assert par.H is None and np.array_equal(par.g, ref.g) and np.array_equal(par.edge_A, ref.edge_A)
