@@ -155,8 +155,9 @@ typedef struct {
   double eta_max;          /* paper 0.5 */
 } sim3ba_depth_params;
 int sim3ba_depth_default_params(sim3ba_depth_params* p);
-/* n_iters iterations at the context's CURRENT poses on its packed pointmaps.  d_labels [N][HW] int32 DEVICE: label of a
- * pixel inside its keyframe, 0 <= label < n_seg <= 64, < 0 = excluded pixel; segment id = keyframe * n_seg + label.
+/* n_iters iterations at the context's CURRENT poses on the PRISTINE pointmaps given at sim3ba_create (eta is the absolute
+ * log-scale of Eq. (8) whatever sim3ba_apply_depth has done to the pointmaps the pose passes see).  d_labels [N][HW] int32 DEVICE: label of a
+ * pixel inside its keyframe, 0 <= label < n_seg <= 512, < 0 = excluded pixel; segment id = keyframe * n_seg + label.
  * h_pairs [n_pairs][2] HOST segment ids (g, h) of the 4-adjacent pairs, h_delta [n_pairs] HOST Delta_gh,
  * h_anchor_kf HOST list of keyframes whose segments stay fixed.  d_eta [N * n_seg] double DEVICE, in/out (caller
  * owned; start from zeros for eta = 0).  h_cost HOST [n_iters] or NULL: the objective at the start of each iteration.
@@ -164,9 +165,10 @@ int sim3ba_depth_default_params(sim3ba_depth_params* p);
 int sim3ba_depth_refine(sim3ba_ctx* ctx, const int32_t* d_labels, int32_t n_seg, const int32_t* h_pairs, const double* h_delta,
                         int32_t n_pairs, const int32_t* h_anchor_kf, int32_t n_anchor, const sim3ba_depth_params* p,
                         int32_t n_iters, double* d_eta, double* h_cost);
-/* The other half of the alternation: re-packs the context's pointmaps from the caller's pristine d_points [N][HW][3],
- * d_conf [N][HW] (as in sim3ba_create) with every labelled pixel scaled by exp(eta) of its segment, so that the next
- * sim3ba_step sees the refined structure.  Asynchronous on the context's stream. */
+/* The other half of the alternation: re-packs the pointmaps the pose passes read from the caller's pristine d_points
+ * [N][HW][3], d_conf [N][HW] (as in sim3ba_create) with every labelled pixel scaled by exp(eta) of its segment, so that
+ * the next sim3ba_step sees the refined structure.  The first call keeps a pristine packed copy inside the context
+ * (16 bytes per pixel) for the structure passes that follow.  Asynchronous on the context's stream. */
 int sim3ba_apply_depth(sim3ba_ctx* ctx, const float* d_points, const float* d_conf, const int32_t* d_labels, int32_t n_seg,
                        const double* d_eta);
 

@@ -19,6 +19,7 @@
 // after it, the per-thread partial sums (<= 8 terms per lane, 16 per thread) and the first two levels of
 // the warp tree (<= 64 terms) in fp32; every sum from there upwards (warp, edge, adjoint congruence) in FP64.  No floating-point
 // atomics: the reduction order is fixed, results are run-to-run identical.
+#include "f32x2.cuh"
 #include "sim3ba_internal.cuh"
 #include "sim3_math.cuh"
 
@@ -83,29 +84,6 @@ __device__ __forceinline__ void cp_async16(void* dst, const void* src) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-// MUFU.RSQ / MUFU.RCP without the denormal pre/post-scaling of rsqrtf() / 1/x: arguments are clamped or
-// may legitimately give +inf (handled by the min() that follows)
-__device__ __forceinline__ float rsq(float v) {
-  float r;
-  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
-  return r;
-}
-__device__ __forceinline__ float rcp(float v) {
-  float r;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
-  return r;
-}
-
-// ---- packed fp32x2 arithmetic (sm_100: FFMA2 / FMUL2 / FADD2, one issue slot for two lanes) -------
-// The two lanes of every float2 below are TWO DIFFERENT MATCHES (A, B) of the same thread: the whole
-// per-match algebra is evaluated 2-wide, accumulators included; lanes are summed once per (edge, tile).
-using f2 = float2;
-__device__ __forceinline__ f2 operator*(f2 a, f2 b) { return __fmul2_rn(a, b); }
-__device__ __forceinline__ f2 operator+(f2 a, f2 b) { return __fadd2_rn(a, b); }
-__device__ __forceinline__ f2 operator-(f2 a) { return make_float2(-a.x, -a.y); }
-__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
-__device__ __forceinline__ f2 bc(float s) { return make_float2(s, s); }
 
 // Two valid-or-masked matches: accumulate J_xi^T Omega J_xi (25 structurally non-zero upper-triangular
 // entries), J_xi^T Omega e (7) and the two robust-cost sums into acc[] (slot layout: sim3ba_internal.cuh).

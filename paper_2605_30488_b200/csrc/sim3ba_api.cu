@@ -134,7 +134,7 @@ cudaError_t upload(T** dst, const std::vector<T>& src, cudaStream_t s) {
 }
 
 void free_all(Ctx* c) {
-  dfree(c->pm); dfree(c->edges); dfree(c->grp_kf); dfree(c->grp_ptr); dfree(c->grp_edge); dfree(c->edgeT); dfree(c->fixed_mask); dfree(c->poses);
+  dfree(c->pm); dfree(c->pm0); dfree(c->edges); dfree(c->grp_kf); dfree(c->grp_ptr); dfree(c->grp_edge); dfree(c->edgeT); dfree(c->fixed_mask); dfree(c->poses);
   dfree(c->kf_ptr); dfree(c->kf_edge); dfree(c->pair_kf); dfree(c->pair_ptr); dfree(c->pair_edge);
   dfree(c->partials); dfree(c->blocks35); dfree(c->edge_cost); dfree(c->n_valid); dfree(c->checksum);
   dfree(c->Hd); dfree(c->L); dfree(c->g); dfree(c->rhs); dfree(c->ysol); dfree(c->Dinv); dfree(c->pairhi_ptr);
@@ -624,7 +624,7 @@ int sim3ba_depth_refine(sim3ba_ctx* h, const int32_t* d_labels, int32_t n_seg, c
   tl_stream = c->stream;
   if (!d_labels || !d_eta || !p || n_seg < 1 || n_seg > depth_max_segments() || n_iters < 0 || n_pairs < 0 || n_anchor < 0 ||
       (n_pairs > 0 && (!h_pairs || !h_delta)) || (n_anchor > 0 && !h_anchor_kf))
-    return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL pointer, or n_seg outside 1..64, or a negative count");
+    return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL pointer, or n_seg outside 1..512, or a negative count");
   if (!(p->sigma_point > 0.f) || !(p->huber_k > 0.f) || p->lambda_smooth < 0.0 || !(p->lambda_prior > 0.0) || p->lambda_lm < 0.0 ||
       !(p->eta_max > 0.0))
     return fail(c, SIM3BA_ERR_INVALID_ARG, "invalid depth params (sigma, kappa, lambda_prior, eta_max > 0; lambda_smooth, lambda_lm >= 0)");

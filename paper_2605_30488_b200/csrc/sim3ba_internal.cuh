@@ -99,6 +99,8 @@ struct Ctx {
   sim3ba_params prm{};
   // inputs
   float4* pm = nullptr;            // [N][HW] packed (x, y, z, w): w = c^(1/4) if c > conf_min else -1
+  float4* pm0 = nullptr;           // pristine copy of pm, taken by the first sim3ba_apply_depth (NULL until then: pm is pristine)
+  size_t depth_smem = 0;           // dynamic shared memory k_depth_edge has been opted in for
   const int32_t* match = nullptr;  // borrowed [E][HW]
   int32_t* edges = nullptr;        // [E][2]
   // kernel-1 schedule: keyframes with outgoing edges (ascending) and their edges (ascending j, then e)

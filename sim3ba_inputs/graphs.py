@@ -377,40 +377,77 @@ class DepthInputs:
     anchor_kf: np.ndarray     # keyframes whose segments stay fixed
 
 
-def make_depth_inputs(g: Graph, grid=None, drop_frac: float = 0.02) -> DepthInputs:
-    """Stands in for the SLIC segmentation of PAPER.md:126: a rows x cols grid of rectangular segments per keyframe (config
-    5: 4 x 8 = 32), a seeded fraction of pixels excluded (label -1, "low confidence"), the 4-adjacent pairs of the grid and
-    Delta_gh = mean over the pixel pairs straddling the shared boundary of log|X_p| - log|X_p'| (p in g, p' in h)."""
-    r, c = grid if grid is not None else (g.spec.n_segments if g.spec.n_segments[0] > 0 else (4, 8))
+def _jittered_labels(H: int, W: int, rows: int, cols: int, rng: np.random.Generator) -> np.ndarray:
+    """An irregular segmentation standing in for SLIC superpixels: rows x cols centres on a lattice, each jittered by up to
+    +-40 % of a cell, every pixel labelled by the nearest of the 3 x 3 centres around its own cell."""
+    ch, cw = H / rows, W / cols
+    cy = (np.arange(rows)[:, None] + 0.5 + rng.uniform(-0.4, 0.4, (rows, cols))) * ch
+    cx = (np.arange(cols)[None, :] + 0.5 + rng.uniform(-0.4, 0.4, (rows, cols))) * cw
+    yy, xx = np.meshgrid(np.arange(H) + 0.5, np.arange(W) + 0.5, indexing="ij")
+    r0 = np.minimum((yy / ch).astype(np.int64), rows - 1)
+    c0 = np.minimum((xx / cw).astype(np.int64), cols - 1)
+    best = np.full((H, W), np.inf)
+    lab = np.zeros((H, W), dtype=np.int32)
+    for dr in (-1, 0, 1):
+        for dc in (-1, 0, 1):
+            r, c = np.clip(r0 + dr, 0, rows - 1), np.clip(c0 + dc, 0, cols - 1)
+            d = (yy - cy[r, c]) ** 2 + (xx - cx[r, c]) ** 2
+            take = d < best
+            best[take] = d[take]
+            lab[take] = (r * cols + c)[take].astype(np.int32)
+    return lab
+
+
+def _boundary_pairs(lab: np.ndarray, logd: np.ndarray, base: int):
+    """4-adjacent segment pairs (g < h, as segment ids base + label) of one keyframe and Delta_gh = mean over the pixel
+    pairs straddling the shared boundary of log|X_p| - log|X_p'| (p in g, p' in h); excluded pixels (label < 0) never count."""
+    keys, vals = [], []
+    for a, b, da, db in ((lab[:, :-1], lab[:, 1:], logd[:, :-1], logd[:, 1:]), (lab[:-1, :], lab[1:, :], logd[:-1, :], logd[1:, :])):
+        sel = (a != b) & (a >= 0) & (b >= 0)
+        la, lb, d = a[sel].astype(np.int64), b[sel].astype(np.int64), (da - db)[sel]
+        swap = la > lb
+        lo, hi = np.where(swap, lb, la), np.where(swap, la, lb)
+        keys.append(lo * (1 << 20) + hi)
+        vals.append(np.where(swap, -d, d))
+    keys, vals = np.concatenate(keys), np.concatenate(vals)
+    uniq, inv = np.unique(keys, return_inverse=True)
+    mean = np.bincount(inv, weights=vals) / np.maximum(np.bincount(inv), 1)
+    pairs = np.stack([base + uniq // (1 << 20), base + uniq % (1 << 20)], axis=1).astype(np.int32)
+    return pairs, mean
+
+
+def make_depth_inputs(g: Graph, grid=None, drop_frac: float = 0.02, irregular: int = 0) -> DepthInputs:
+    """Stands in for the SLIC segmentation of PAPER.md:126.  Default: a rows x cols grid of rectangular segments per
+    keyframe (config 5: 4 x 8 = 32).  ``irregular = M`` (the paper: M_k ~ 200): about M jittered-lattice superpixels per
+    keyframe, eight seeded layouts dealt round-robin over the keyframes.  A seeded fraction of pixels is excluded (label
+    -1, "low confidence"); the pairs are the 4-adjacent segment pairs found in the label image and Delta_gh the mean over
+    the pixel pairs straddling the shared boundary of log|X_p| - log|X_p'| (p in g, p' in h)."""
     H, W = g.spec.height, g.spec.width
-    rr = (np.arange(H) * r // H)[:, None]
-    cc = (np.arange(W) * c // W)[None, :]
-    lab2 = (rr * c + cc).astype(np.int32)                                # [H, W]
-    labels = np.repeat(lab2.reshape(1, -1), g.n_kf, axis=0).copy()
-    for k in range(g.n_kf):
-        rng = _rng(g.spec.seed, 9, k)
-        labels[k, rng.random(H * W) < drop_frac] = -1
-    logd = np.log(np.maximum(np.linalg.norm(g.points.astype(np.float64), axis=2), 1e-12)).reshape(g.n_kf, H, W)
-    pairs, delta = [], []
-    for k in range(g.n_kf):
-        for a in range(r * c):
-            ar, ac = divmod(a, c)
-            for b in ((ar, ac + 1), (ar + 1, ac)):
-                if b[0] >= r or b[1] >= c:
-                    continue
-                bl = b[0] * c + b[1]
-                if b[1] == ac + 1:      # vertical boundary: pixel columns x, x + 1 with labels a, bl
-                    rows = np.flatnonzero(rr[:, 0] == ar)
-                    x = int(np.flatnonzero(cc[0, :] == ac)[-1])
-                    d = logd[k, rows, x] - logd[k, rows, x + 1]
-                else:                   # horizontal boundary: pixel rows y, y + 1
-                    y = int(np.flatnonzero(rr[:, 0] == ar)[-1])
-                    cols = np.flatnonzero(cc[0, :] == ac)
-                    d = logd[k, y, cols] - logd[k, y + 1, cols]
-                pairs.append((k * r * c + a, k * r * c + bl))
-                delta.append(float(np.mean(d)))
-    return DepthInputs(labels=labels, n_seg=r * c, pairs=np.asarray(pairs, dtype=np.int32).reshape(-1, 2),
-                       delta=np.asarray(delta, dtype=np.float64), anchor_kf=g.fixed_kf.copy())
+    if irregular > 0:
+        r = max(1, int(round(np.sqrt(irregular * H / W))))
+        c = max(1, -(-irregular // r))
+        layouts = [_jittered_labels(H, W, r, c, _rng(g.spec.seed, 10, q)) for q in range(min(8, g.n_kf))]
+    else:
+        r, c = grid if grid is not None else (g.spec.n_segments if g.spec.n_segments[0] > 0 else (4, 8))
+        rr = (np.arange(H) * r // H)[:, None]
+        cc = (np.arange(W) * c // W)[None, :]
+        layouts = [(rr * c + cc).astype(np.int32)]
+    n_seg = r * c
+    labels = np.empty((g.n_kf, H * W), dtype=np.int32)
+    pairs: List[Optional[np.ndarray]] = [None] * g.n_kf
+    delta: List[Optional[np.ndarray]] = [None] * g.n_kf
+
+    def one_keyframe(k: int) -> None:
+        lab = layouts[k % len(layouts)].copy()
+        lab.reshape(-1)[_rng(g.spec.seed, 9, k).random(H * W) < drop_frac] = -1
+        labels[k] = lab.reshape(-1)
+        logd = np.log(np.maximum(np.linalg.norm(g.points[k].astype(np.float64), axis=1), 1e-12)).reshape(H, W)
+        pairs[k], delta[k] = _boundary_pairs(lab, logd, k * n_seg)
+
+    with ThreadPoolExecutor(max_workers=_n_threads()) as pool:
+        list(pool.map(one_keyframe, range(g.n_kf)))
+    return DepthInputs(labels=labels, n_seg=n_seg, pairs=np.concatenate(pairs).astype(np.int32).reshape(-1, 2),
+                       delta=np.concatenate(delta).astype(np.float64), anchor_kf=g.fixed_kf.copy())
 
 
 def clean_variant(spec: GraphSpec) -> GraphSpec:
