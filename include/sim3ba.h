@@ -172,6 +172,25 @@ int sim3ba_depth_refine(sim3ba_ctx* ctx, const int32_t* d_labels, int32_t n_seg,
 int sim3ba_apply_depth(sim3ba_ctx* ctx, const float* d_points, const float* d_conf, const int32_t* d_labels, int32_t n_seg,
                        const double* d_eta);
 
+/* The terminal pose-depth alternation as ONE job with HOST buffers (PAPER.md:143 last sentence: "the segment-level
+ * structure refinement alternates with pose refinement"; "at most 100 pose-depth rounds with up to ten depth
+ * iterations and 50 pose iterations per round"; BASELINE config 5).  Uploads the graph (as sim3ba_optimize_host) plus
+ * h_labels [N][HW] int32 and h_eta [N * n_seg] double, creates a context, then runs n_rounds rounds of
+ * { sim3ba_depth_refine with n_depth_iters iterations at the current poses (anchor keyframes = the fixed keyframes);
+ *   sim3ba_apply_depth; n_pose_iters x sim3ba_step on the rescaled pointmaps },
+ * eta carried across the rounds as the absolute log-scale of Eq. (8).  Fixed counts (reading R14): the paper's numbers
+ * are caps and it states no stopping rule.  Host outputs: h_poses_out [N][8], h_eta (in/out), and, if non-NULL,
+ * h_pose_cost [n_rounds * n_pose_iters] (robust cost at the start of each pose iteration) and h_depth_cost
+ * [n_rounds * n_depth_iters] (structure objective at the start of each depth iteration).  h_pairs / h_delta / depth
+ * params as in sim3ba_depth_refine.  Frees everything and synchronises the stream.  Errors as sim3ba_create /
+ * sim3ba_depth_refine / sim3ba_step; the message is read with sim3ba_last_error(NULL). */
+int sim3ba_refine_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_edges, const float* h_points, const float* h_conf,
+                       const int32_t* h_edges, const int32_t* h_match, const int32_t* h_fixed_kf, int32_t n_fixed,
+                       const sim3ba_params* params, const int32_t* h_labels, int32_t n_seg, const int32_t* h_pairs, const double* h_delta,
+                       int32_t n_pairs, const sim3ba_depth_params* depth_params, int32_t n_rounds, int32_t n_depth_iters,
+                       int32_t n_pose_iters, const double* h_poses_in, double* h_poses_out, double* h_eta, double* h_pose_cost,
+                       double* h_depth_cost, void* cuda_stream);
+
 /* a8 only: T_i <- Exp(tau_i) T_i with the tau of the last solve. */
 int sim3ba_retract(sim3ba_ctx* ctx);
 
@@ -225,9 +244,10 @@ int sim3ba_set_solver_mode(sim3ba_ctx* ctx, int32_t mode);
 /* Band + border plan of the graph (host output): h_info[0] = 1 if mode 2 applies to this graph, [1] interior
  * keyframes, [2] segments, [3] border keyframes, [4] longest segment, [5] most border keyframes touched by a segment. */
 int sim3ba_get_bb_info(sim3ba_ctx* ctx, int32_t h_info[6]);
-/* Host outputs (each may be NULL): non-zero tiles of the active plan, lower tiles of the dense plan,
- * flop count of the active plan (factor + both triangular solves, at tile granularity), CTAs of
- * the last persistent solve launch. */
+/* Host outputs (each may be NULL): non-zero tiles of the tile-sparse plan (of the dense plan in mode 1), lower tiles of
+ * the dense plan, flop count of the ACTIVE plan (factor + both triangular solves, FMA = 2: at 7x7 granularity with a dense
+ * border system for the band + border plan of mode 2, at 64x64 tile granularity for modes 0 / 1), CTAs of the last
+ * persistent solve launch. */
 int sim3ba_get_solver_info(sim3ba_ctx* ctx, int32_t* h_n_tiles, int32_t* h_n_tiles_dense, double* h_flops,
                            int32_t* h_grid);
 
@@ -246,6 +266,11 @@ int sim3ba_get_phase_ms(sim3ba_ctx* ctx, float h_ms[8]);
  * of the last solve: [0] assembly (a6), [1] segment elimination, [2] grid barrier after it, [3] Schur rows, [4] border
  * system, [5] back-substitution, [6..7] reserved (0).  All zero if the last solve was not profiled.  Synchronises. */
 int sim3ba_get_solve_phase_us(sim3ba_ctx* ctx, float h_us[8]);
+
+/* Measures the FP64 peak of the current device, the denominator of the solve's roofline (MEASURED_PEAKS.json has none):
+ * TFLOP/s (FMA = 2) of register-resident DFMA chains and of mma.sync.m8n8k4.f64 (DMMA) chains on every SM, best of five
+ * launches, CUDA events on the given stream.  Host outputs.  Takes a few milliseconds; synchronises. */
+int sim3ba_probe_fp64(double* h_dfma_tflops, double* h_dmma_tflops, void* cuda_stream);
 
 /* All device memory of the library comes from a stream-ordered memory pool the library owns (one per device), which keeps
  * freed blocks for the next context / job.  This call synchronises the current device and returns the pool's unused memory

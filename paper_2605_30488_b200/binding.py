@@ -16,11 +16,11 @@ LIB_PATH = os.path.join(_HERE, "libsim3ba.so")
 
 EXPORTS = (
     "sim3ba_default_params", "sim3ba_create", "sim3ba_destroy", "sim3ba_set_params", "sim3ba_set_poses",
-    "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_graph", "sim3ba_step_host", "sim3ba_optimize_host", "sim3ba_gauge_sync", "sim3ba_depth_default_params", "sim3ba_depth_refine", "sim3ba_apply_depth",
+    "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_graph", "sim3ba_step_host", "sim3ba_optimize_host", "sim3ba_refine_host", "sim3ba_gauge_sync", "sim3ba_depth_default_params", "sim3ba_depth_refine", "sim3ba_apply_depth",
     "sim3ba_retract", "sim3ba_get_edge_stats", "sim3ba_get_edge_blocks", "sim3ba_get_system",
     "sim3ba_get_update", "sim3ba_get_bookkeeping", "sim3ba_load_system", "sim3ba_get_launch_count",
     "sim3ba_set_solver_mode", "sim3ba_get_solver_info", "sim3ba_get_bb_info",
-    "sim3ba_set_profiling", "sim3ba_get_phase_ms", "sim3ba_get_solve_phase_us", "sim3ba_release_memory", "sim3ba_copy_d2d", "sim3ba_last_error", "sim3ba_version",
+    "sim3ba_set_profiling", "sim3ba_get_phase_ms", "sim3ba_get_solve_phase_us", "sim3ba_release_memory", "sim3ba_probe_fp64", "sim3ba_copy_d2d", "sim3ba_last_error", "sim3ba_version",
 )
 
 
@@ -68,6 +68,8 @@ def load_library() -> C.CDLL:
         "sim3ba_step_graph": [vp, i32],
         "sim3ba_step_host": [vp, vp, vp, vp],
         "sim3ba_optimize_host": [i32, i32, i32, i32, vp, vp, vp, vp, P(i32), i32, P(Params), vp, i32, vp, vp, vp],
+        "sim3ba_refine_host": [i32, i32, i32, i32, vp, vp, vp, vp, P(i32), i32, P(Params), vp, i32, P(i32), P(C.c_double), i32, P(DepthParams),
+                               i32, i32, i32, vp, vp, vp, vp, vp, vp],
         "sim3ba_gauge_sync": [vp, i32, P(i32), i32, i32, i32, P(C.c_double), P(i32), P(i32)],
         "sim3ba_depth_default_params": [P(DepthParams)],
         "sim3ba_depth_refine": [vp, vp, i32, P(i32), P(C.c_double), i32, P(i32), i32, P(DepthParams), i32, vp, P(C.c_double)],
@@ -87,6 +89,7 @@ def load_library() -> C.CDLL:
         "sim3ba_get_phase_ms": [vp, P(C.c_float)],
         "sim3ba_get_solve_phase_us": [vp, P(C.c_float)],
         "sim3ba_release_memory": [],
+        "sim3ba_probe_fp64": [P(C.c_double), P(C.c_double), vp],
         "sim3ba_copy_d2d": [vp, vp, vp, C.c_uint64],
     }
     for name, args in sig.items():
@@ -121,6 +124,49 @@ def optimize_host(points, conf, edges, match, fixed_kf: Sequence[int], params: O
                                   stream)
     if rc:
         raise Sim3BAError(rc, (lib.sim3ba_last_error(None) or b"").decode())
+
+
+def refine_host(points, conf, edges, match, fixed_kf: Sequence[int], params: Optional[Params], height: int, width: int, labels, n_seg: int,
+                pairs: np.ndarray, delta: np.ndarray, depth_params: Optional[DepthParams], n_rounds: int, n_depth_iters: int, n_pose_iters: int,
+                poses_in, poses_out, eta, pose_cost=None, depth_cost=None, stream: int = 0):
+    """sim3ba_refine_host: the pose-depth alternation as one job with HOST (CPU, pinned recommended) torch tensors; eta
+    [N * n_seg] float64 is updated in place.  Argument marshalling only."""
+    lib = load_library()
+    for t in (points, conf, edges, match, labels, poses_in, poses_out, eta):
+        assert t.device.type == "cpu" and t.is_contiguous()
+    fk = (C.c_int32 * max(1, len(fixed_kf)))(*fixed_kf)
+    prm = params if params is not None else make_params()
+    dprm = depth_params
+    if dprm is None:
+        dprm = DepthParams()
+        lib.sim3ba_depth_default_params(C.byref(dprm))
+    pr = np.ascontiguousarray(pairs, dtype=np.int32).reshape(-1, 2)
+    dl = np.ascontiguousarray(delta, dtype=np.float64).reshape(-1)
+    rc = lib.sim3ba_refine_host(points.shape[0], height, width, edges.shape[0], points.data_ptr(), conf.data_ptr(), edges.data_ptr(),
+                                match.data_ptr(), fk, len(fixed_kf), C.byref(prm), labels.data_ptr(), int(n_seg),
+                                pr.ctypes.data_as(C.POINTER(C.c_int32)), dl.ctypes.data_as(C.POINTER(C.c_double)), pr.shape[0], C.byref(dprm),
+                                int(n_rounds), int(n_depth_iters), int(n_pose_iters), poses_in.data_ptr(), poses_out.data_ptr(), eta.data_ptr(),
+                                pose_cost.data_ptr() if pose_cost is not None else None,
+                                depth_cost.data_ptr() if depth_cost is not None else None, stream)
+    if rc:
+        raise Sim3BAError(rc, (lib.sim3ba_last_error(None) or b"").decode())
+
+
+def probe_fp64(stream: int = 0):
+    """sim3ba_probe_fp64: measured (DFMA, DMMA) TFLOP/s of the current device."""
+    lib = load_library()
+    a, b = C.c_double(), C.c_double()
+    rc = lib.sim3ba_probe_fp64(C.byref(a), C.byref(b), stream)
+    if rc:
+        raise Sim3BAError(rc, (lib.sim3ba_last_error(None) or b"").decode())
+    return a.value, b.value
+
+
+def release_memory():
+    """sim3ba_release_memory: give the library pool's unused device memory back to the driver."""
+    rc = load_library().sim3ba_release_memory()
+    if rc:
+        raise Sim3BAError(rc, "sim3ba_release_memory")
 
 
 class Sim3BA:

@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsim3ba.so")
-SOURCES = ["sim3ba_api.cu", "k_accumulate.cu", "k_assemble.cu", "k_solve.cu", "k_solve_bb.cu", "k_retract.cu", "k_gauge_sync.cu", "k_depth.cu", "solve_plan.cu", "bb_plan.cu"]
+SOURCES = ["sim3ba_api.cu", "k_accumulate.cu", "k_assemble.cu", "k_solve.cu", "k_solve_bb.cu", "k_retract.cu", "k_gauge_sync.cu", "k_depth.cu", "solve_plan.cu", "bb_plan.cu", "probe_fp64.cu"]
 HEADERS = ["f32x2.cuh", "sim3ba_internal.cuh", "sim3_math.cuh", "assemble_tile.cuh", "solve_tile.cuh", os.path.join("..", "..", "include", "sim3ba.h")]
 NVCC_FLAGS = os.environ.get("SIM3BA_NVCC_EXTRA", "").split() + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]

@@ -162,6 +162,23 @@ bool build_bb_plan(Ctx* c, std::string& err) {
         if (role[a.first] == BORDER && a.first < bord_kf[b]) bb_pair[(size_t)b * n_bord + bidx[a.first]] = a.second;
   }
 
+  // flop count of the plan itself (FMA = 2), at 7x7 granularity: per interior column with B = band + border blocks below
+  // the diagonal -- POTRF 7^3/3, TRSM of 7 B + 1 rows (49 each), trailing update B (B + 1) / 2 block products (2 * 7^3) plus
+  // the right-hand side (B * 2 * 49; the border x border part of it is the Schur complement), back-substitution
+  // (B + 1) * 2 * 49 -- and the dense Cholesky + two triangular solves of the border system
+  double flops = 0.0;
+  for (int s = 0; s < n_seg; ++s) {
+    const int nb = seg_bptr[s + 1] - seg_bptr[s], len = seg_ptr[s + 1] - seg_ptr[s];
+    for (int q = 0; q < len; ++q) {
+      const double B = (double)std::min(kBand, len - 1 - q) + nb;
+      flops += 343.0 / 3.0 + (7.0 * B + 1.0) * 49.0 + B * (B + 1.0) / 2.0 * 686.0 + B * 98.0 + (B + 1.0) * 98.0;
+    }
+  }
+  {
+    const double nB = 7.0 * n_bord;
+    flops += nB * nB * nB / 3.0 + 2.0 * nB * nB;
+  }
+  P.flops = flops;
   P.n_int = n_int; P.n_seg = n_seg; P.n_bord = n_bord; P.max_nb = max_nb; P.max_len = max_len;
   P.npadB = (7 * n_bord + kNB - 1) / kNB * kNB;
   P.col_doubles = ofs;

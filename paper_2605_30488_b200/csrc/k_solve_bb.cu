@@ -656,7 +656,10 @@ cudaError_t launch_solve_bb(Ctx* c) {
   a.eps0 = c->prm.eps0; a.max_attempts = c->prm.max_attempts; a.status = c->fail_flag; a.eps_used = c->d_eps_used; a.bar = c->bar;
   cudaError_t e = cudaMemsetAsync(c->bar, 0, sizeof(unsigned int), c->stream);
   if (e != cudaSuccess) return e;
-  if (c->profiling) cudaEventRecord(c->ev[4], c->stream);
+  if (c->profiling) {
+    cudaMemsetAsync(c->solve_stamps, 0, 16 * sizeof(unsigned long long), c->stream);
+    cudaEventRecord(c->ev[4], c->stream);
+  }
   void* args[] = {&a};
   e = cudaLaunchCooperativeKernel((const void*)k_solve_bb, dim3(G), dim3(kSolveThreads), args, smem, c->stream);
   c->launches += 1;

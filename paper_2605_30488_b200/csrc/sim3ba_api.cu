@@ -492,9 +492,20 @@ int sim3ba_get_solve_phase_us(sim3ba_ctx* h, float us[8]) {
   CU(cudaMemcpyAsync(st, c->solve_stamps, sizeof(st), cudaMemcpyDeviceToHost, c->stream));
   CU(cudaStreamSynchronize(c->stream));
   for (int k = 0; k < 8; ++k) us[k] = 0.f;
-  if (st[6] > st[0] && st[0] != 0ull)
-    for (int k = 0; k < 6; ++k) us[k] = st[k + 1] >= st[k] ? (float)((double)(st[k + 1] - st[k]) * 1e-3) : 0.f;
+  // a phase the plan does not have (no border keyframes: no Schur rows, no border system) leaves its stamp at zero
+  unsigned long long prev = st[0];
+  for (int k = 0; k < 6 && st[0] != 0ull; ++k) {
+    if (st[k + 1] == 0ull) continue;
+    us[k] = st[k + 1] >= prev ? (float)((double)(st[k + 1] - prev) * 1e-3) : 0.f;
+    prev = st[k + 1];
+  }
   return SIM3BA_OK;
+}
+
+int sim3ba_probe_fp64(double* h_dfma_tflops, double* h_dmma_tflops, void* cuda_stream) {
+  if (!h_dfma_tflops || !h_dmma_tflops) return SIM3BA_ERR_INVALID_ARG;
+  cudaError_t e = run_probe_fp64((cudaStream_t)cuda_stream, h_dfma_tflops, h_dmma_tflops);
+  return e == cudaSuccess ? SIM3BA_OK : cuda_fail(nullptr, e, "sim3ba_probe_fp64");
 }
 
 int sim3ba_release_memory(void) {
@@ -520,62 +531,115 @@ int sim3ba_step_host(sim3ba_ctx* h, const double* h_in, double* h_out, double* h
   return SIM3BA_OK;
 }
 
+namespace {
+
+// Device copies of a host graph + a context on them: the common front part of the *_host jobs.  Everything comes from the
+// library's stream-ordered pool, kept warm between jobs (no map / unmap per job).
+struct HostJob {
+  float *d_points = nullptr, *d_conf = nullptr;
+  int32_t *d_edges = nullptr, *d_match = nullptr, *d_labels = nullptr;
+  double* d_eta = nullptr;
+  sim3ba_ctx* h = nullptr;
+  cudaStream_t st = nullptr;
+  ~HostJob() {
+    if (h) sim3ba_destroy(h);                                   // synchronises the stream
+    tl_stream = st;
+    dfree(d_points); dfree(d_conf); dfree(d_edges); dfree(d_match); dfree(d_labels); dfree(d_eta);
+  }
+  // returns SIM3BA_OK or a negative status with the message in the thread-local create error
+  int open(int32_t n_kf, int32_t height, int32_t width, int32_t n_edges, const float* h_points, const float* h_conf,
+           const int32_t* h_edges, const int32_t* h_match, const int32_t* h_fixed_kf, int32_t n_fixed, const sim3ba_params* params,
+           const double* h_poses_in, void* cuda_stream) {
+    st = (cudaStream_t)cuda_stream;
+    tl_stream = st;
+    const size_t NHW = (size_t)n_kf * height * width, EHW = (size_t)n_edges * height * width;
+    cudaError_t e = cudaSuccess;
+    auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return e == cudaSuccess; };
+    ok(dmalloc(reinterpret_cast<void**>(&d_points), 3 * NHW * sizeof(float)));
+    ok(dmalloc(reinterpret_cast<void**>(&d_conf), NHW * sizeof(float)));
+    ok(dmalloc(reinterpret_cast<void**>(&d_edges), 2 * (size_t)n_edges * sizeof(int32_t)));
+    ok(dmalloc(reinterpret_cast<void**>(&d_match), EHW * sizeof(int32_t)));
+    if (e == cudaSuccess) ok(cudaMemcpyAsync(d_points, h_points, 3 * NHW * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (e == cudaSuccess) ok(cudaMemcpyAsync(d_conf, h_conf, NHW * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (e == cudaSuccess && n_edges > 0) {
+      ok(cudaMemcpyAsync(d_edges, h_edges, 2 * (size_t)n_edges * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+      ok(cudaMemcpyAsync(d_match, h_match, EHW * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    }
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "host job: graph upload");
+    int rc = sim3ba_create(&h, n_kf, height, width, n_edges, d_points, d_conf, d_edges, d_match, h_fixed_kf, n_fixed, params, cuda_stream);
+    if (rc) { h = nullptr; return rc; }
+    e = cudaMemcpyAsync(h->c.poses, h_poses_in, (size_t)8 * n_kf * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "host job: pose upload");
+    return SIM3BA_OK;
+  }
+};
+
+bool host_graph_args_ok(int32_t n_kf, int32_t height, int32_t width, int32_t n_edges, const float* h_points, const float* h_conf,
+                        const int32_t* h_edges, const int32_t* h_match, const double* h_poses_in, const double* h_poses_out) {
+  if (n_kf <= 0 || height <= 0 || width <= 0 || n_edges < 0 || (int64_t)height * width > (1 << 28)) return false;
+  return h_points && h_conf && (n_edges == 0 || (h_edges && h_match)) && h_poses_in && h_poses_out;
+}
+
+}  // namespace
+
 int sim3ba_optimize_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_edges, const float* h_points,
                          const float* h_conf, const int32_t* h_edges, const int32_t* h_match, const int32_t* h_fixed_kf,
                          int32_t n_fixed, const sim3ba_params* params, const double* h_poses_in, int32_t n_iters,
                          double* h_poses_out, double* h_cost, void* cuda_stream) {
-  Ctx* c = nullptr;   // errors before / outside a context go to the thread-local create error
-  if (n_kf <= 0 || height <= 0 || width <= 0 || n_edges < 0 || n_iters < 0 || (int64_t)height * width > (1 << 28))
-    return fail(c, SIM3BA_ERR_INVALID_ARG, "non-positive or oversized dimensions");
-  if (!h_points || !h_conf || (n_edges > 0 && (!h_edges || !h_match)) || !h_poses_in || !h_poses_out)
-    return fail(c, SIM3BA_ERR_INVALID_ARG, "NULL host pointer");
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  tl_stream = st;
-  const size_t NHW = (size_t)n_kf * height * width, EHW = (size_t)n_edges * height * width;
-  float *d_points = nullptr, *d_conf = nullptr;
-  int32_t *d_edges = nullptr, *d_match = nullptr;
-  sim3ba_ctx* h = nullptr;
-  int rc = SIM3BA_OK;
-  // the graph buffers come from the library's own stream-ordered pool, kept warm between jobs (no map / unmap per job)
-  auto cleanup = [&]() {
-    if (h) sim3ba_destroy(h);                                   // synchronises the stream
-    cudaFreeAsync(d_points, st); cudaFreeAsync(d_conf, st); cudaFreeAsync(d_edges, st); cudaFreeAsync(d_match, st);
-  };
-  auto pool_alloc = [&](void** ptr, size_t bytes) { return dmalloc(ptr, bytes); };
-#define CUJ(call)                                                       \
-  do {                                                                  \
-    cudaError_t e_ = (call);                                            \
-    if (e_ != cudaSuccess) {                                            \
-      cleanup();                                                        \
-      return cuda_fail(nullptr, e_, #call);                             \
-    }                                                                   \
-  } while (0)
-  CUJ(pool_alloc(reinterpret_cast<void**>(&d_points), 3 * NHW * sizeof(float)));
-  CUJ(pool_alloc(reinterpret_cast<void**>(&d_conf), NHW * sizeof(float)));
-  CUJ(pool_alloc(reinterpret_cast<void**>(&d_edges), 2 * (size_t)n_edges * sizeof(int32_t)));
-  CUJ(pool_alloc(reinterpret_cast<void**>(&d_match), EHW * sizeof(int32_t)));
-  CUJ(cudaMemcpyAsync(d_points, h_points, 3 * NHW * sizeof(float), cudaMemcpyHostToDevice, st));
-  CUJ(cudaMemcpyAsync(d_conf, h_conf, NHW * sizeof(float), cudaMemcpyHostToDevice, st));
-  if (n_edges > 0) {
-    CUJ(cudaMemcpyAsync(d_edges, h_edges, 2 * (size_t)n_edges * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-    CUJ(cudaMemcpyAsync(d_match, h_match, EHW * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-  }
-  rc = sim3ba_create(&h, n_kf, height, width, n_edges, d_points, d_conf, d_edges, d_match, h_fixed_kf, n_fixed, params, cuda_stream);
-  if (rc) { h = nullptr; cleanup(); return rc; }
-  c = &h->c;
-  const size_t pose_bytes = (size_t)8 * n_kf * sizeof(double);
-  cudaError_t ce = cudaMemcpyAsync(c->poses, h_poses_in, pose_bytes, cudaMemcpyHostToDevice, st);
+  if (n_iters < 0 || !host_graph_args_ok(n_kf, height, width, n_edges, h_points, h_conf, h_edges, h_match, h_poses_in, h_poses_out))
+    return fail(nullptr, SIM3BA_ERR_INVALID_ARG, "NULL host pointer, or non-positive / oversized dimensions");
+  HostJob job;
+  int rc = job.open(n_kf, height, width, n_edges, h_points, h_conf, h_edges, h_match, h_fixed_kf, n_fixed, params, h_poses_in, cuda_stream);
+  if (rc) return rc;
+  Ctx* c = &job.h->c;
+  cudaStream_t st = job.st;
+  cudaError_t ce = cudaSuccess;
   for (int it = 0; it < n_iters && ce == cudaSuccess && rc == SIM3BA_OK; ++it) {
-    rc = sim3ba_step(h);
+    rc = sim3ba_step(job.h);
     if (rc == SIM3BA_OK && h_cost) ce = cudaMemcpyAsync(h_cost + it, c->total_cost, sizeof(double), cudaMemcpyDeviceToHost, st);
   }
-  if (ce == cudaSuccess && rc == SIM3BA_OK) ce = cudaMemcpyAsync(h_poses_out, c->poses, pose_bytes, cudaMemcpyDeviceToHost, st);
+  if (ce == cudaSuccess && rc == SIM3BA_OK) ce = cudaMemcpyAsync(h_poses_out, c->poses, (size_t)8 * n_kf * sizeof(double), cudaMemcpyDeviceToHost, st);
   if (ce == cudaSuccess && rc == SIM3BA_OK) ce = cudaStreamSynchronize(st);
-  if (rc != SIM3BA_OK) g_create_error = c->err;
-  cleanup();
-  if (rc != SIM3BA_OK) return rc;
+  if (rc != SIM3BA_OK) { g_create_error = c->err; return rc; }
   if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "sim3ba_optimize_host");
-#undef CUJ
+  return SIM3BA_OK;
+}
+
+int sim3ba_refine_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_edges, const float* h_points, const float* h_conf,
+                       const int32_t* h_edges, const int32_t* h_match, const int32_t* h_fixed_kf, int32_t n_fixed,
+                       const sim3ba_params* params, const int32_t* h_labels, int32_t n_seg, const int32_t* h_pairs, const double* h_delta,
+                       int32_t n_pairs, const sim3ba_depth_params* depth_params, int32_t n_rounds, int32_t n_depth_iters,
+                       int32_t n_pose_iters, const double* h_poses_in, double* h_poses_out, double* h_eta, double* h_pose_cost,
+                       double* h_depth_cost, void* cuda_stream) {
+  if (n_rounds < 0 || n_depth_iters < 0 || n_pose_iters < 0 || !h_labels || !h_eta || !depth_params || n_seg < 1 ||
+      !host_graph_args_ok(n_kf, height, width, n_edges, h_points, h_conf, h_edges, h_match, h_poses_in, h_poses_out))
+    return fail(nullptr, SIM3BA_ERR_INVALID_ARG, "NULL host pointer, negative count, or non-positive / oversized dimensions");
+  HostJob job;
+  int rc = job.open(n_kf, height, width, n_edges, h_points, h_conf, h_edges, h_match, h_fixed_kf, n_fixed, params, h_poses_in, cuda_stream);
+  if (rc) return rc;
+  Ctx* c = &job.h->c;
+  cudaStream_t st = job.st;
+  const size_t NHW = (size_t)n_kf * height * width, M = (size_t)n_kf * n_seg;
+  cudaError_t ce = dmalloc(reinterpret_cast<void**>(&job.d_labels), NHW * sizeof(int32_t));
+  if (ce == cudaSuccess) ce = dmalloc(reinterpret_cast<void**>(&job.d_eta), M * sizeof(double));
+  if (ce == cudaSuccess) ce = cudaMemcpyAsync(job.d_labels, h_labels, NHW * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+  if (ce == cudaSuccess) ce = cudaMemcpyAsync(job.d_eta, h_eta, M * sizeof(double), cudaMemcpyHostToDevice, st);
+  for (int r = 0; r < n_rounds && ce == cudaSuccess && rc == SIM3BA_OK; ++r) {
+    // structure pass with the poses fixed (anchor = gauge keyframes), then the pose passes on X(eta)
+    rc = sim3ba_depth_refine(job.h, job.d_labels, n_seg, h_pairs, h_delta, n_pairs, h_fixed_kf, n_fixed, depth_params, n_depth_iters, job.d_eta,
+                             h_depth_cost ? h_depth_cost + (size_t)r * n_depth_iters : nullptr);
+    if (rc == SIM3BA_OK) rc = sim3ba_apply_depth(job.h, job.d_points, job.d_conf, job.d_labels, n_seg, job.d_eta);
+    for (int it = 0; it < n_pose_iters && ce == cudaSuccess && rc == SIM3BA_OK; ++it) {
+      rc = sim3ba_step(job.h);
+      if (rc == SIM3BA_OK && h_pose_cost)
+        ce = cudaMemcpyAsync(h_pose_cost + (size_t)r * n_pose_iters + it, c->total_cost, sizeof(double), cudaMemcpyDeviceToHost, st);
+    }
+  }
+  if (ce == cudaSuccess && rc == SIM3BA_OK) ce = cudaMemcpyAsync(h_poses_out, c->poses, (size_t)8 * n_kf * sizeof(double), cudaMemcpyDeviceToHost, st);
+  if (ce == cudaSuccess && rc == SIM3BA_OK) ce = cudaMemcpyAsync(h_eta, job.d_eta, M * sizeof(double), cudaMemcpyDeviceToHost, st);
+  if (ce == cudaSuccess && rc == SIM3BA_OK) ce = cudaStreamSynchronize(st);
+  if (rc != SIM3BA_OK) { g_create_error = c->err; return rc; }
+  if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "sim3ba_refine_host");
   return SIM3BA_OK;
 }
 
@@ -736,6 +800,7 @@ int sim3ba_get_solver_info(sim3ba_ctx* h, int32_t* n_tiles, int32_t* n_tiles_den
   Ctx* c = &h->c;
   tl_stream = c->stream;
   const bool dense = c->solver_mode == 1;
+  const bool bb = c->solver_mode == 2 && c->plan_bb.valid;
   SolvePlan& plan = dense ? c->plan_dense : c->plan_sparse;
   if (!plan.ready) {
     std::string err;
@@ -744,7 +809,7 @@ int sim3ba_get_solver_info(sim3ba_ctx* h, int32_t* n_tiles, int32_t* n_tiles_den
   const int nb = c->npad / kNB;
   if (n_tiles) *n_tiles = plan.n_tiles;
   if (n_tiles_dense) *n_tiles_dense = nb * (nb + 1) / 2;
-  if (flops) *flops = plan.flops;
+  if (flops) *flops = bb ? c->plan_bb.flops : plan.flops;
   if (grid) *grid = c->last_solve_grid;
   return SIM3BA_OK;
 }

@@ -70,6 +70,7 @@ struct BBPlan {
   int n_int = 0, n_seg = 0, n_bord = 0, max_nb = 0, max_len = 0;
   int npadB = 0;                  // padded size of the border system (multiple of kNB), 0 if no border
   size_t col_doubles = 0;         // doubles of all interior block columns
+  double flops = 0.0;             // flop count of the plan (factor + solves, 7x7 granularity; border system dense)
   // device arrays
   int32_t *seg_ptr = nullptr;     // [n_seg+1] interior columns of a segment (indices into col_*)
   int32_t *seg_bptr = nullptr;    // [n_seg+1] into seg_bord
@@ -186,5 +187,6 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
                              const int32_t* h_anchor, int n_anchor, const sim3ba_depth_params& p, int n_iters, double* d_eta, double* h_cost);
 cudaError_t launch_depth_apply(Ctx* c, const float* d_points, const float* d_conf, const int32_t* d_labels, int n_seg, const double* d_eta);
 int depth_max_segments();
+cudaError_t run_probe_fp64(cudaStream_t st, double* dfma_tflops, double* dmma_tflops);   // FP64 peak probe (probe_fp64.cu)
 
 }  // namespace sim3ba

@@ -119,6 +119,54 @@ def test_two_alternation_rounds_lockstep_and_free_running(irregular):
     ba.close()
 
 
+def test_refine_host_one_call_equals_the_manual_rounds_and_the_chained_oracles():
+    """sim3ba_refine_host (host buffers in, poses and eta out) runs the very same kernels as the manual sequence
+    depth_refine -> apply_depth -> n x step per round: bit-identical poses, eta and cost traces; and it agrees with the two
+    oracles chained on their own numbers to 1e-3 (free-running)."""
+    import torch
+    from paper_2605_30488_b200 import refine_host
+    from tests.gpu_common import gpu_params
+    g, d = graph(irregular=200)
+    prm = oracle_params("config")
+    dprm = dp.DepthParams()
+    n_rounds, n_dit, n_pit = 2, 3, 2
+    M = g.n_kf * d.n_seg
+    labels = torch.from_numpy(d.labels).cuda()
+    pts, cf = torch.from_numpy(g.points).cuda(), torch.from_numpy(g.conf).cuda()
+    ba = make_solver(g, prm)
+    set_poses(ba, g.poses_init)
+    eta_dev = torch.zeros(M, dtype=torch.float64, device="cuda")
+    pose_cost, depth_cost = [], []
+    for _ in range(n_rounds):
+        depth_cost += list(ba.depth_refine(labels, d.n_seg, d.pairs, d.delta, d.anchor_kf, eta_dev, n_dit))
+        ba.apply_depth(pts, cf, labels, d.n_seg, eta_dev)
+        for _ in range(n_pit):
+            ba.step()
+            pose_cost.append(ba.update()[3])
+    ref_poses, ref_eta = ba.get_poses().cpu().numpy(), eta_dev.cpu().numpy()
+    ba.close()
+    h_out = torch.empty((g.n_kf, 8), dtype=torch.float64).pin_memory()
+    h_eta = torch.zeros(M, dtype=torch.float64).pin_memory()
+    h_pc = torch.empty(n_rounds * n_pit, dtype=torch.float64).pin_memory()
+    h_dc = torch.empty(n_rounds * n_dit, dtype=torch.float64).pin_memory()
+    refine_host(torch.from_numpy(g.points).pin_memory(), torch.from_numpy(g.conf).pin_memory(), torch.from_numpy(g.edges).contiguous(),
+                torch.from_numpy(g.match).pin_memory(), g.fixed_kf, gpu_params(prm), g.spec.height, g.spec.width,
+                torch.from_numpy(d.labels).pin_memory(), d.n_seg, d.pairs, d.delta, None, n_rounds, n_dit, n_pit,
+                torch.from_numpy(g.poses_init.copy()), h_out, h_eta, h_pc, h_dc, torch.cuda.current_stream().cuda_stream)
+    assert np.array_equal(h_out.numpy(), ref_poses) and np.array_equal(h_eta.numpy(), ref_eta)
+    assert np.array_equal(h_pc.numpy(), np.asarray(pose_cost)) and np.array_equal(h_dc.numpy(), np.asarray(depth_cost))
+    poses, eta = g.poses_init.copy(), np.zeros(M)
+    for _ in range(n_rounds):
+        eta, _ = dp.depth_refine(poses, g.points, g.conf, g.edges, g.match, d.labels, d.n_seg, eta, d.pairs, d.delta, d.anchor_kf, dprm, n_dit)
+        pts_ref = scaled_points(g, d, eta)
+        for _ in range(n_pit):
+            poses, _, _ = orc.gn_step(poses, pts_ref, g.conf, g.edges, g.match, g.fixed_kf, prm)
+    assert rel(h_eta.numpy(), eta) <= 1e-3
+    d_gpu = np.concatenate([orc.pose_delta_log(h_out.numpy()[i], g.poses_init[i]) for i in range(g.n_kf)])
+    d_orc = np.concatenate([orc.pose_delta_log(poses[i], g.poses_init[i]) for i in range(g.n_kf)])
+    assert rel(d_gpu, d_orc) <= 1e-3
+
+
 def test_argument_checks():
     import torch
     from paper_2605_30488_b200 import Sim3BAError
