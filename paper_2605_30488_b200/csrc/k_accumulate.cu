@@ -35,6 +35,7 @@ constexpr int kStages = 2;                     // ring of gathered X_j pairs per
                                                // no stored 1/|X_i| (14.1 KB + 1 KB reserved per one-warp CTA) let 14 warps share the 228 KB
                                                // of an SM.  Measured on C2: 12 warps / 3 stages 177.6 us, 13 / 2 171.3, 14 / 2 165.8; 16 warps
                                                // with the index buffer refilled in halves 167.8 (not kept)
+constexpr float kCancel = 1.0f / 1024.0f;      // |x|^2 < kCancel |X_i|^2: x = X_i + del has lost 5 bits or more, take the FP64 x instead
 constexpr int kSlots = kPartialStride;         // 40 reduction slots (layout: sim3ba_internal.cuh)
 constexpr int kAccSlots = 37;                  // slots that carry floating-point sums
 
@@ -87,25 +88,32 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 
 // Two valid-or-masked matches: accumulate J_xi^T Omega J_xi (25 structurally non-zero upper-triangular
 // entries), J_xi^T Omega e (7) and the two robust-cost sums into acc[] (slot layout: sim3ba_internal.cuh).
-//   del = T_ij X_j - X_i (fp32 rounding of the FP64 value), Xi, rdi = 1/|X_i|,
+//   del = T_ij X_j - X_i (fp32 rounding of the FP64 value), x = T_ij X_j and d2 = |x|^2 (from the caller: X_i + del, or
+//   the FP64 value rounded where that sum cancels), Xi, rdi = 1/|X_i|,
 //   sq = sqrt(q) = (c_i c_j)^(1/4), 0 for a masked lane (all its weights vanish).
 __device__ __forceinline__ void accumulate_pair(f2 (&acc)[kAccSlots], const f2 del0, const f2 del1, const f2 del2,
+                                                const f2 x0, const f2 x1, const f2 x2, f2 d2,
                                                 const f2 Xi0, const f2 Xi1, const f2 Xi2, const f2 rdi,
-                                                const f2 sq, const DevParams& prm) {
+                                                const f2 sq, const DevParams& prm, const bool any_direct, const bool dirA, const bool dirB) {
   const f2 di = fma2(Xi0, Xi0, fma2(Xi1, Xi1, Xi2 * Xi2)) * rdi;   // |X_i| (rdi is clamped: 0 for X_i = 0)
-  const f2 x0 = Xi0 + del0, x1 = Xi1 + del1, x2 = Xi2 + del2;   // x = T_ij X_j
-  f2 d2 = fma2(x0, x0, fma2(x1, x1, x2 * x2));
   d2.x = fmaxf(d2.x, 1e-20f); d2.y = fmaxf(d2.y, 1e-20f);
   const f2 rd = make_float2(rsq(d2.x), rsq(d2.y));
   const f2 d = d2 * rd;
   const f2 u0 = x0 * rd, u1 = x1 * rd, u2 = x2 * rd;
   // e3 = |x| - |X_i| = delta . (x + X_i) / (|x| + |X_i|);  e_r = x/|x| - X_i/|X_i| = delta/|x| - X_i e3 / (|x| |X_i|)
   const f2 den = d + di;
-  const f2 e3 = fma2(del0, x0 + Xi0, fma2(del1, x1 + Xi1, del2 * (x2 + Xi2))) * make_float2(rcp(den.x), rcp(den.y));
-  const f2 gsc = (e3 * rd) * rdi;
-  const f2 e0 = fma2(del0, rd, -(Xi0 * gsc));
-  const f2 e1 = fma2(del1, rd, -(Xi1 * gsc));
-  const f2 e2 = fma2(del2, rd, -(Xi2 * gsc));
+  const f2 e3d = fma2(del0, x0 + Xi0, fma2(del1, x1 + Xi1, del2 * (x2 + Xi2))) * make_float2(rcp(den.x), rcp(den.y));
+  const f2 gsc = (e3d * rd) * rdi;
+  f2 e0 = fma2(del0, rd, -(Xi0 * gsc));
+  f2 e1 = fma2(del1, rd, -(Xi1 * gsc));
+  f2 e2 = fma2(del2, rd, -(Xi2 * gsc));
+  f2 e3 = e3d;
+  if (any_direct) {   // warp-uniform and rare: lanes whose x came from the FP64 path (|x| << |X_i|, so |del| ~ |X_i|: nothing cancels
+                      // in the plain differences, whereas del / |x| would carry 2^-24 |del| / |x|) take e = [u - u_i; |x| - |X_i|] as written
+    const f2 t0 = fma2(-Xi0, rdi, u0), t1 = fma2(-Xi1, rdi, u1), t2 = fma2(-Xi2, rdi, u2), t3 = d + (-di);
+    if (dirA) { e0.x = t0.x; e1.x = t1.x; e2.x = t2.x; e3.x = t3.x; }
+    if (dirB) { e0.y = t0.y; e1.y = t1.y; e2.y = t2.y; e3.y = t3.y; }
+  }
   // q = sqrt(c_i c_j); s_c = q / sigma_c^2; omega_c = q w_c / sigma_c^2 = min(s_c, kappa sqrt(q) / (sigma_c |e_c|));
   // rho_c = omega_c e_c^2 - min(s_c e_c^2, kappa^2) / 2
   const f2 q = sq * sq;
@@ -355,20 +363,41 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
       const bool vA = (XA0.w >= 0.f) && (P1.z >= 0.f), vB = (XA1.w >= 0.f) && (P1.w >= 0.f);
       if (__any_sync(0xffffffffu, vA || vB)) {               // whole invalid bands are skipped warp-uniformly
         const float4 P0 = s_Xi[pa];                          // (xA, xB, yA, yB)
-        f2 rdi;                                              // 1 / |X_i|, recomputed per edge: a stored copy would cost the 14th warp
-        {
-          const f2 d2i = fma2(make_float2(P0.x, P0.y), make_float2(P0.x, P0.y), fma2(make_float2(P0.z, P0.w), make_float2(P0.z, P0.w),
-                              make_float2(P1.x, P1.y) * make_float2(P1.x, P1.y)));
-          rdi = make_float2(rsq(fmaxf(d2i.x, 1e-20f)), rsq(fmaxf(d2i.y, 1e-20f)));
-        }
+        const f2 Xi0 = make_float2(P0.x, P0.y), Xi1 = make_float2(P0.z, P0.w), Xi2 = make_float2(P1.x, P1.y);
+        const f2 d2i = fma2(Xi0, Xi0, fma2(Xi1, Xi1, Xi2 * Xi2));
+        // 1 / |X_i|, recomputed per edge: a stored copy would cost the 14th warp
+        const f2 rdi = make_float2(rsq(fmaxf(d2i.x, 1e-20f)), rsq(fmaxf(d2i.y, 1e-20f)));
         f2 del0, del1, del2;
         delta(XA0, P0.x, P0.z, P1.x, del0.x, del1.x, del2.x);
         delta(XA1, P0.y, P0.w, P1.y, del0.y, del1.y, del2.y);
+        f2 x0 = Xi0 + del0, x1 = Xi1 + del1, x2 = Xi2 + del2;   // x = T_ij X_j
+        f2 d2 = fma2(x0, x0, fma2(x1, x1, x2 * x2));
+        // X_i + del carries 2^-24 |del|: where the sum cancels (a stray match mapped to within |X_i| / 32 of the camera
+        // centre; the 1 / |x|^2 terms of the Jacobian then dominate its edge's block) x is the FP64 value rounded.  Rare: one
+        // warp-uniform test per pair.
+        const bool tA = vA && d2.x < d2i.x * kCancel, tB = vB && d2.y < d2i.y * kCancel;
+        const bool any_t = __any_sync(0xffffffffu, tA || tB);
+        {
+          if (any_t) {
+            if (tA) {
+              const double a = (double)XA0.x, b = (double)XA0.y, c = (double)XA0.z;
+              x0.x = (float)fma(Td[0], a, fma(Td[1], b, fma(Td[2], c, Td[9])));
+              x1.x = (float)fma(Td[3], a, fma(Td[4], b, fma(Td[5], c, Td[10])));
+              x2.x = (float)fma(Td[6], a, fma(Td[7], b, fma(Td[8], c, Td[11])));
+            }
+            if (tB) {
+              const double a = (double)XA1.x, b = (double)XA1.y, c = (double)XA1.z;
+              x0.y = (float)fma(Td[0], a, fma(Td[1], b, fma(Td[2], c, Td[9])));
+              x1.y = (float)fma(Td[3], a, fma(Td[4], b, fma(Td[5], c, Td[10])));
+              x2.y = (float)fma(Td[6], a, fma(Td[7], b, fma(Td[8], c, Td[11])));
+            }
+            d2 = fma2(x0, x0, fma2(x1, x1, x2 * x2));
+          }
+        }
         f2 sq = make_float2(P1.z, P1.w) * make_float2(XA0.w, XA1.w);
         sq.x = vA ? sq.x : 0.f;
         sq.y = vB ? sq.y : 0.f;
-        accumulate_pair(acc, del0, del1, del2, make_float2(P0.x, P0.y), make_float2(P0.z, P0.w), make_float2(P1.x, P1.y),
-                        rdi, sq, prm);
+        accumulate_pair(acc, del0, del1, del2, x0, x1, x2, d2, Xi0, Xi1, Xi2, rdi, sq, prm, any_t, tA, tB);
         const unsigned mA = vA ? 0xffffffffu : 0u, mB = vB ? 0xffffffffu : 0u;
         cnt += (mA & 1u) + (mB & 1u);
         sum_m += ((unsigned)pa & mA) + ((unsigned)pb & mB);

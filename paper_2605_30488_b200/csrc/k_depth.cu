@@ -7,16 +7,30 @@
 //                   Delta eta_g = -g_g / ((1 + lambda_lm) H_gg), clipped to eta_max, anchor keyframes fixed
 // Conventions D1-D5 of DESIGN.md section 10 (objective = sum rho + lambda_s/2 E_bnd + lambda_p/2 E_prior).
 //
-// Kernel A (k_depth_edge): one CTA per (edge, tile of the pixels of i), in kernel 1's order (edges sorted by keyframe,
-// the tiles of an edge together: X_j and the labels are shared through L2).  Every thread evaluates TWO adjacent
-// pixels at a time in the two lanes of packed fp32x2 instructions.  Precision plan (the one of kernel 1): the one
-// cancellation -- res = T_ij X_j(eta) - X_i(eta), a difference of two ~10 m points -- is evaluated in FP64 and rounded
-// once; everything after it per match is fp32; fp32 partial sums hold at most 64 terms (the two matches of a lane and
-// one 32-lane butterfly), every sum from there upwards is FP64.  The loads run in a software pipeline (streams two
-// iterations ahead, gathers one).  The per-segment sums are binned WITHOUT atomics in per-warp FP64 shared-memory bins
-// (dynamic shared memory: 32 n_seg bytes per warp): a lane whose label is alone in its warp adds straight to the bin,
-// a label shared by several lanes takes one fp32 butterfly over the peers found by match.any; the eight warps' bins are
-// added in a fixed order -> one record [2 sides][n_seg][g, H] + cost per (edge, tile).  Bit-reproducible run to run.
+// The poses are fixed during a structure pass, so the one expensive, cancellation-prone part of the residual does not
+// change between its iterations.  With y = T_ij X_j - X_i (both at eta = 0) and E_g = exp(eta_g),
+//     res = T_ij X_j(eta_h) - X_i(eta_g) = E_h y + (E_h - E_g) X_i + (1 - E_h) t_ij                      (Eq. (8)-(9))
+// an identity: y is evaluated ONCE per call, in FP64, and kept in fp32 (kernel P), and every iteration (kernel A) is a
+// pure stream over (X_i, label of m; y, sqrt(q), label of n) with no gather and no FP64 per match.
+//
+// Kernel P (k_depth_prep): per candidate match of every edge, n = match[e][m]; valid <=> the GN step's rule (R12) and both
+// pixels labelled; record (y [3] fp32 from the FP64 difference, sqrt(q) = w_i w_j or 0 if invalid) and the label of n.
+// Kernel A (k_depth_edge): one CTA (4 warps) per (edge, tile of image rows of i), in kernel 1's order (edges sorted by
+// keyframe, the tiles of an edge together, so X_i and its labels are shared through L2).  A warp's work item is a patch
+// of 32 columns x 4 rows: every lane owns one column, i.e. four vertically adjacent pixels, which mostly share their
+// segment on both sides.  All loads are per-lane cp.async into a two-stage shared-memory ring one item ahead (a lane
+// only reads what it copied itself: no barrier).  Two pixels at a time in the two lanes of packed fp32x2 instructions.
+// Precision: the per-segment constants E_g, E_h and (1 - E_h) t_ij are computed in FP64 and carried as unevaluated
+// fp32 pairs (hi, lo); res is two nested fused multiply-adds on the leading parts (each rounds an exact sum once) plus the
+// trailing parts, so it is as accurate as the FP64 difference rounded to fp32 up to a random 2^-24 of its larger terms --
+// the rounding the stored y carries anyway; everything after res is fp32; fp32 partial sums hold at most 128 terms,
+// every sum from there up is FP64.
+// Binning WITHOUT floating-point atomics, bit-reproducible: a lane first merges the records of its four pixels that
+// share the label of its first valid pixel; that record goes through one warp phase per item and side, the few others
+// (stray matches, a segment boundary inside the patch) are queued in shared memory and take a phase per 32 of them.  A
+// phase (bin_phase): match.any groups the lanes by label, every group is summed in fp32 by a fixed tree of shuffles and
+// its first lane adds the total to the warp's FP64 bin.  The warps' bins are added in a fixed order -> one record
+// [2 sides][n_seg][g, H] + cost per (edge, tile).
 // Kernel B (k_depth_update): one thread per segment gathers its records through the keyframe -> edge CSR, adds boundary
 // and prior terms, takes the damped clipped step into a second eta buffer.  Kernel C sums the objective.
 //
@@ -35,21 +49,33 @@ namespace sim3ba {
 
 namespace {
 
-constexpr int kDpThreads = 256;
-constexpr int kDpWarps = kDpThreads / 32;
-constexpr int kDpMaxSeg = 512;       // labels per keyframe (the paper's SLIC pass: M_k ~ 200); 16 KB of bins per warp at 512
-#ifndef SIM3BA_DP_CTAS
-#define SIM3BA_DP_CTAS 2
-#endif
+constexpr int kDpWarps = 4;
+constexpr int kDpThreads = 32 * kDpWarps;
+constexpr int kDpMaxSeg = 512;       // labels per keyframe (the paper's SLIC pass: M_k ~ 200)
+constexpr int kDpRows = 4;           // rows of a warp item (pixels per lane)
+constexpr int kDpCols = 32;          // columns of a warp item (one per lane)
 #ifndef SIM3BA_DP_TILE_PX
 #define SIM3BA_DP_TILE_PX 16384
 #endif
 constexpr int kDpTilePx = SIM3BA_DP_TILE_PX;
-constexpr int kDpIterPx = 2 * kDpThreads;   // pixels of the tile one CTA iteration covers (two adjacent pixels per thread)
+constexpr int kDpStages = 2;         // ring of items per warp: copies run one item ahead
+constexpr int kDpQueue = 128;        // per-warp queue of (bin, g, H) records waiting for a phase (power of two)
+// per-warp shared memory: every ring array is [stage][row][lane], so a warp's 32 lanes touch 32 consecutive words / float4
+constexpr size_t kDpOffXi = 0;                                                          // float4 [kDpStages][4][32]
+constexpr size_t kDpOffRec = kDpOffXi + sizeof(float4) * kDpStages * kDpRows * 32;      // float4 [kDpStages][4][32]
+constexpr size_t kDpOffLi = kDpOffRec + sizeof(float4) * kDpStages * kDpRows * 32;      // int32  [kDpStages][4][32]
+constexpr size_t kDpOffLh = kDpOffLi + sizeof(int32_t) * kDpStages * kDpRows * 32;      // int32  [kDpStages][4][32]
+constexpr size_t kDpOffQ = kDpOffLh + sizeof(int32_t) * kDpStages * kDpRows * 32;       // int32 bin, float g, float H  [kDpQueue] each
+constexpr size_t kDpWarpBytes = kDpOffQ + 12 * kDpQueue;                                // 11776 bytes per warp
 
 struct DepthDev {
   double inv_sigma, huber_k, lambda_smooth, lambda_prior, lambda_lm, eta_max;
 };
+
+__device__ __forceinline__ uint32_t dp_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void dp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void dp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -57,177 +83,326 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// One binning phase: every lane offers (key, a, b) -- key < 0 = nothing -- and bins[key][0..1] += (a, b) over the warp,
-// deterministically.  match.any gives every lane the mask of the lanes carrying its key: a lane alone with its key (a
-// stray match landing in some far segment) adds straight to the bin -- distinct keys, so these adds do not meet; a key
-// shared by several lanes takes one fp32 butterfly over the warp with the other lanes contributing zero (a fixed tree,
-// <= 32 x 2 terms) and its first lane adds the total.  The usual warp (one or two segments, a few strays) takes one or
-// two butterflies.
-__device__ __forceinline__ void bin_phase(double* bins, int key, float a, float b, int lane) {
-  const unsigned peers = __match_any_sync(0xffffffffu, key >= 0 ? key : -1 - lane);   // nothing to offer: a unique key
-  const bool single = key >= 0 && peers == (1u << lane);
-  if (single) { bins[2 * key] += (double)a; bins[2 * key + 1] += (double)b; }
-  unsigned active = __ballot_sync(0xffffffffu, key >= 0 && !single);
-  while (active) {
-    const int leader = __ffs(active) - 1;
-    const unsigned grp = __shfl_sync(0xffffffffu, peers, leader);
-    const bool mine = (grp >> lane) & 1u;
-    f2 x = mine ? make_float2(a, b) : make_float2(0.f, 0.f);
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) x = x + make_float2(__shfl_xor_sync(0xffffffffu, x.x, o), __shfl_xor_sync(0xffffffffu, x.y, o));
-    if (lane == leader) { bins[2 * key] += (double)x.x; bins[2 * key + 1] += (double)x.y; }
-    active &= ~grp;
-  }
-  __syncwarp();                                                // the next phase's adds may come from other lanes
-}
-
-// The two matches (A, B) of every lane -> bins: equal keys are merged in the lane first (adjacent pixels mostly share
-// their segment), then one phase for the A slots and, if any lane still holds a B, one for the B slots.
-__device__ __forceinline__ void bin_pair(double* bins, int keyA, int keyB, f2 a, f2 b, int lane) {
-  if (keyA >= 0 && keyA == keyB) { a.x += a.y; b.x += b.y; keyB = -1; }
-  else if (keyA < 0 && keyB >= 0) { keyA = keyB; a.x = a.y; b.x = b.y; keyB = -1; }
-  bin_phase(bins, keyA, a.x, b.x, lane);
-  if (__any_sync(0xffffffffu, keyB >= 0)) bin_phase(bins, keyB, a.y, b.y, lane);
-}
-
-struct DepthStream {     // the streamed loads of one CTA iteration: two adjacent pixels m, m + 1 of keyframe i
-  int nA, nB, lgA, lgB;
-  float4 aA, aB;
-};
-
-__global__ void __launch_bounds__(kDpThreads, SIM3BA_DP_CTAS)
-k_depth_edge(const float4* __restrict__ pm, const int32_t* __restrict__ match, const int32_t* __restrict__ edges,
-             const int32_t* __restrict__ grp_edge, const int32_t* __restrict__ labels, const double* __restrict__ eta,
-             const double* __restrict__ poses, int HW, int n_seg, int tiles, int per, DepthDev prm, double* __restrict__ partial) {
-  extern __shared__ __align__(16) unsigned char dp_smem[];
-  // [kDpWarps][2 sides][n_seg][2] FP64 bins | [2][n_seg] exp(eta) FP64 | [2][n_seg] exp(eta) fp32 | [kDpWarps] cost
-  double* s_bins = reinterpret_cast<double*>(dp_smem);
-  double* s_exp = s_bins + (size_t)kDpWarps * 4 * n_seg;
-  double* s_cost = s_exp + 2 * n_seg;
-  float* s_expf = reinterpret_cast<float*>(s_cost + kDpWarps);
-  // launch order = kernel 1's: the edges sorted by (i, j), all tiles of an edge together, so the CTAs in flight cover a
-  // few neighbouring keyframes completely and X_i, X_j and the labels are fetched from HBM once and shared through L2
-  const int k = blockIdx.x / tiles, tile = blockIdx.x - k * tiles, e = grp_edge[k];
+// Kernel P: the eta-independent part of every candidate match, once per structure pass.
+__global__ void __launch_bounds__(256)
+k_depth_prep(const float4* __restrict__ pm, const int32_t* __restrict__ match, const int32_t* __restrict__ edges,
+             const int32_t* __restrict__ labels, const double* __restrict__ poses, int HW, int n_seg, int chunks,
+             float4* __restrict__ rec, int32_t* __restrict__ lab_n) {
+  const int e = blockIdx.x / chunks, chunk = blockIdx.x - e * chunks;
   const int i = edges[2 * e], j = edges[2 * e + 1];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  for (int q = tid; q < kDpWarps * 4 * n_seg; q += kDpThreads) s_bins[q] = 0.0;
-  for (int q = tid; q < 2 * n_seg; q += kDpThreads) {
-    const double ev = exp(eta[(size_t)(q < n_seg ? i : j) * n_seg + (q < n_seg ? q : q - n_seg)]);
-    s_exp[q] = ev;
-    s_expf[q] = (float)ev;
-  }
-  __syncthreads();
   const Sim3d T = relative_pose(load_pose(poses + 8 * i), load_pose(poses + 8 * j));   // T_ij
   double sR[9];
 #pragma unroll
   for (int q = 0; q < 9; ++q) sR[q] = T.s * T.R[q];
-  const float tf[3] = {(float)T.t[0], (float)T.t[1], (float)T.t[2]};
   const float4* __restrict__ Pi = pm + (size_t)i * HW;
   const float4* __restrict__ Pj = pm + (size_t)j * HW;
   const int32_t* __restrict__ mt = match + (size_t)e * HW;
   const int32_t* __restrict__ li = labels + (size_t)i * HW;
   const int32_t* __restrict__ lj = labels + (size_t)j * HW;
-  const int m0 = tile * per, m1 = min(HW, m0 + per);
+  const int per = (HW + chunks - 1) / chunks;
+  const int m1 = min(HW, (chunk + 1) * per);
+  for (int m = chunk * per + threadIdx.x; m < m1; m += 256) {
+    const int n = __ldcs(mt + m);
+    float4 out = make_float4(0.f, 0.f, 0.f, 0.f);
+    int lh = -1;
+    if ((unsigned)n < (unsigned)HW) {
+      const float4 a = Pi[m], b = Pj[n];
+      const int lg = li[m];
+      lh = lj[n];
+      if (a.w >= 0.f && b.w >= 0.f && (unsigned)lg < (unsigned)n_seg && (unsigned)lh < (unsigned)n_seg) {
+        const double X0 = (double)b.x, X1 = (double)b.y, X2 = (double)b.z;
+        out.x = (float)(fma(sR[0], X0, fma(sR[1], X1, fma(sR[2], X2, T.t[0]))) - (double)a.x);
+        out.y = (float)(fma(sR[3], X0, fma(sR[4], X1, fma(sR[5], X2, T.t[1]))) - (double)a.y);
+        out.z = (float)(fma(sR[6], X0, fma(sR[7], X1, fma(sR[8], X2, T.t[2]))) - (double)a.z);
+        out.w = a.w * b.w;                                       // sqrt(q) = w_i w_j (w = c^(1/4)) > 0
+      } else {
+        lh = -1;
+      }
+    }
+    rec[(size_t)e * HW + m] = out;                               // w = 0 marks "no term"
+    lab_n[(size_t)e * HW + m] = lh;
+  }
+}
+
+// One binning phase: every lane offers (bin, a, b) -- bin < 0 = nothing -- and bins[bin][0..1] += (a, b) over the warp,
+// deterministically.  match.any gives every lane the mask of the lanes sharing its bin.  A lane alone with its bin adds
+// straight to it (distinct bins: these adds do not meet).  One or two shared bins (the usual patch: one or two segments)
+// take one fp32 butterfly each over the warp, the other lanes contributing zero -- a fixed tree.  More shared bins (a
+// phase of queued strays) are all reduced at once by a tree over the peer masks: in every round a lane adds the value of
+// its next peer above and the odd-ranked lanes of every group drop out, so the rounds needed are log2 of the largest
+// group and the order of the additions is fixed by the lane numbers.  The first lane of a group adds its total to the bin.
+__device__ __forceinline__ void bin_phase(double* bins, int bin, float a, float b, int lane) {
+  const unsigned peers = __match_any_sync(0xffffffffu, bin >= 0 ? bin : -1 - lane);   // nothing to offer: a unique key
+  const bool single = peers == (1u << lane);
+  const bool first = (peers & (0u - peers)) == (1u << lane);
+  unsigned active = __ballot_sync(0xffffffffu, bin >= 0 && first && !single);          // first lanes of the shared bins
+  if (__popc(active) <= 2) {
+    if (bin >= 0 && single) { bins[2 * bin] += (double)a; bins[2 * bin + 1] += (double)b; }
+    while (active) {
+      const int leader = __ffs(active) - 1;
+      const unsigned grp = __shfl_sync(0xffffffffu, peers, leader);
+      const bool mine = (grp >> lane) & 1u;
+      f2 x = mine ? make_float2(a, b) : make_float2(0.f, 0.f);
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) x = x + make_float2(__shfl_xor_sync(0xffffffffu, x.x, o), __shfl_xor_sync(0xffffffffu, x.y, o));
+      if (lane == leader) { bins[2 * bin] += (double)x.x; bins[2 * bin + 1] += (double)x.y; }
+      active &= active - 1;
+    }
+  } else {
+    int rank = __popc(peers & ((1u << lane) - 1u));
+    unsigned above = peers & (0xfffffffeu << lane);
+    while (__any_sync(0xffffffffu, above != 0u)) {
+      const int next = __ffs(above);                             // 1 + lane of the next peer above, 0 if none
+      const float ta = __shfl_sync(0xffffffffu, a, (next - 1) & 31), tb = __shfl_sync(0xffffffffu, b, (next - 1) & 31);
+      if (next) { a += ta; b += tb; }
+      above &= __ballot_sync(0xffffffffu, !(rank & 1));          // odd-ranked lanes have been absorbed: out of every mask
+      rank >>= 1;
+    }
+    if (bin >= 0 && first) { bins[2 * bin] += (double)a; bins[2 * bin + 1] += (double)b; }
+  }
+  __syncwarp();                                                  // the next phase's adds may come from other lanes
+}
+
+struct DpQueue {       // per-warp queue of records waiting for a phase; head / tail are warp-uniform
+  int32_t* bin;
+  float *a, *b;
+  int head, tail;
+};
+
+// lanes with `put` append (bin, a, b) in lane order
+__device__ __forceinline__ void dp_push(DpQueue& q, bool put, int bin, float a, float b, int lane) {
+  const unsigned bal = __ballot_sync(0xffffffffu, put);
+  if (bal == 0u) return;
+  if (put) {
+    const int pos = (q.tail + __popc(bal & ((1u << lane) - 1u))) & (kDpQueue - 1);
+    q.bin[pos] = bin; q.a[pos] = a; q.b[pos] = b;
+  }
+  q.tail += __popc(bal);
+}
+
+// full phases while 32 records wait; `all`: also the remainder
+__device__ __forceinline__ void dp_drain(DpQueue& q, double* bins, bool all, int lane) {
+  while (q.tail - q.head >= 32 || (all && q.tail > q.head)) {
+    __syncwarp();                                                // the records were written by other lanes
+    const bool have = lane < q.tail - q.head;
+    const int pos = (q.head + lane) & (kDpQueue - 1);
+    bin_phase(bins, have ? q.bin[pos] : -1, have ? q.a[pos] : 0.f, have ? q.b[pos] : 0.f, lane);
+    q.head += min(32, q.tail - q.head);
+  }
+}
+
+// The four records (key, a, b) of a lane -- its four vertically adjacent pixels -- of one side (`base` = first bin of the
+// side): those sharing the key of the lane's first valid pixel are merged and go through one phase; the others are queued.
+__device__ __forceinline__ void bin_records(double* bins, DpQueue& q, int base, const int (&key)[kDpRows], const float (&a)[kDpRows],
+                                            const float (&b)[kDpRows], int lane) {
+  const int K = key[0] >= 0 ? key[0] : key[1] >= 0 ? key[1] : key[2] >= 0 ? key[2] : key[3];
+  float sa = 0.f, sb = 0.f;
+  bool extra[kDpRows];
+#pragma unroll
+  for (int r = 0; r < kDpRows; ++r) {
+    const bool same = key[r] == K;
+    sa += same ? a[r] : 0.f;
+    sb += same ? b[r] : 0.f;
+    extra[r] = key[r] >= 0 && !same;
+  }
+  bin_phase(bins, K >= 0 ? base + K : -1, sa, sb, lane);
+#pragma unroll
+  for (int r = 1; r < kDpRows; ++r) dp_push(q, extra[r], base + key[r], a[r], b[r], lane);
+  dp_drain(q, bins, false, lane);
+}
+
+__global__ void __launch_bounds__(kDpThreads)
+k_depth_edge(const float4* __restrict__ pm, const float4* __restrict__ rec, const int32_t* __restrict__ lab_n,
+             const int32_t* __restrict__ edges, const int32_t* __restrict__ grp_edge, const int32_t* __restrict__ labels,
+             const double* __restrict__ eta, const double* __restrict__ poses, int H, int W, int n_seg, int tiles, int tile_rows,
+             DepthDev prm, double* __restrict__ partial) {
+  extern __shared__ __align__(16) unsigned char dp_smem[];
+  // [kDpWarps] rings + queues | [kDpWarps][2 sides][n_seg][2] FP64 bins | [kDpWarps] cost |
+  // [n_seg] 8 floats: E_h (hi, lo), (1 - E_h) t_ij [3] (hi, lo) | [n_seg] float2 E_g (hi, lo)
+  double* s_bins = reinterpret_cast<double*>(dp_smem + kDpWarpBytes * kDpWarps);
+  double* s_cost = s_bins + (size_t)kDpWarps * 4 * n_seg;
+  float4* s_Eh = reinterpret_cast<float4*>(s_cost + kDpWarps);      // two float4 per label (16-byte aligned: 128 n_seg + 32 bytes in)
+  float2* s_Eg = reinterpret_cast<float2*>(s_Eh + 2 * n_seg);
+  // launch order = kernel 1's: the edges sorted by (i, j), all tiles of an edge together, so the CTAs in flight cover a
+  // few neighbouring keyframes completely and X_i and its labels are fetched from HBM once and shared through L2
+  const int k = blockIdx.x / tiles, tile = blockIdx.x - k * tiles, e = grp_edge[k];
+  const int i = edges[2 * e], j = edges[2 * e + 1];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int HW = H * W;
+  const Sim3d T = relative_pose(load_pose(poses + 8 * i), load_pose(poses + 8 * j));   // T_ij
+  for (int q = tid; q < kDpWarps * 4 * n_seg; q += kDpThreads) s_bins[q] = 0.0;
+  auto split = [](double v, float& hi, float& lo) { hi = (float)v; lo = (float)(v - (double)hi); };
+  for (int q = tid; q < n_seg; q += kDpThreads) {
+    float2 g;
+    split(exp(eta[(size_t)i * n_seg + q]), g.x, g.y);
+    s_Eg[q] = g;
+    const double eh = eta[(size_t)j * n_seg + q], ome = -expm1(eh);           // 1 - E_h
+    float4 h0, h1;
+    split(exp(eh), h0.x, h0.y);
+    split(ome * T.t[0], h0.z, h0.w);
+    split(ome * T.t[1], h1.x, h1.y);
+    split(ome * T.t[2], h1.z, h1.w);
+    s_Eh[2 * q] = h0;
+    s_Eh[2 * q + 1] = h1;
+  }
+  __syncthreads();
+  const float tf[3] = {(float)T.t[0], (float)T.t[1], (float)T.t[2]};
+  const float4* __restrict__ Pi = pm + (size_t)i * HW;
+  const float4* __restrict__ Rc = rec + (size_t)e * HW;
+  const int32_t* __restrict__ li = labels + (size_t)i * HW;
+  const int32_t* __restrict__ lh = lab_n + (size_t)e * HW;
   const float isg = (float)prm.inv_sigma, hk = (float)prm.huber_k;
   const float s_cap = isg * isg, k_cap = hk * isg, hk2 = hk * hk;
   double* my_bins = s_bins + (size_t)warp * 4 * n_seg;
-  // Software pipeline over the CTA's iterations (warp-uniform trip count: the binning uses full-warp shuffles): the
-  // streamed loads (match index, X_i, label of m) run two iterations ahead, the gathers they address (X_j, label of n) one.
-  const int niter = (m1 - m0 + kDpIterPx - 1) / kDpIterPx;
-  auto load_stream = [&](int it, DepthStream& s) {
-    const int m = m0 + it * kDpIterPx + 2 * tid;
-    s.nA = s.nB = -1;
-    if (it < niter) {
-      if (m < m1) { s.nA = __ldcs(mt + m); s.aA = Pi[m]; s.lgA = li[m]; }
-      if (m + 1 < m1) { s.nB = __ldcs(mt + m + 1); s.aB = Pi[m + 1]; s.lgB = li[m + 1]; }
-    }
+  unsigned char* wb = dp_smem + kDpWarpBytes * warp;
+  float4* r_Xi = reinterpret_cast<float4*>(wb + kDpOffXi);
+  float4* r_rec = reinterpret_cast<float4*>(wb + kDpOffRec);
+  int32_t* r_li = reinterpret_cast<int32_t*>(wb + kDpOffLi);
+  int32_t* r_lh = reinterpret_cast<int32_t*>(wb + kDpOffLh);
+  DpQueue queue;
+  queue.bin = reinterpret_cast<int32_t*>(wb + kDpOffQ);
+  queue.a = reinterpret_cast<float*>(queue.bin + kDpQueue);
+  queue.b = queue.a + kDpQueue;
+  queue.head = queue.tail = 0;
+
+  // the tile: image rows [row_lo, row_hi); its items: (block of 32 columns, quad of rows); the blocks are dealt round-robin to the warps
+  const int row_lo = tile * tile_rows, row_hi = min(H, row_lo + tile_rows);
+  const int nblk = (W + kDpCols - 1) / kDpCols;
+  const int my_blks = nblk > warp ? (nblk - warp + kDpWarps - 1) / kDpWarps : 0;           // blocks of 32 columns of this warp
+  const int my_items = my_blks * ((row_hi - row_lo + kDpRows - 1) / kDpRows);              // warp-uniform trip count
+  // Copies of the warp's next item into the next ring stage; pixels outside the tile / the image are masked.  Items are
+  // dealt so that a warp walks DOWN a block of 32 columns (quad of rows by quad of rows) before it moves to its next
+  // block: the four source pointers just advance by four image rows, no index arithmetic per copy.
+  const int nrq = (row_hi - row_lo + kDpRows - 1) / kDpRows;
+  const uint32_t u_Xi = dp_smem_u32(r_Xi) + 16u * lane, u_rec = dp_smem_u32(r_rec) + 16u * lane;
+  const uint32_t u_li = dp_smem_u32(r_li) + 4u * lane, u_lh = dp_smem_u32(r_lh) + 4u * lane;
+  const size_t rs16 = (size_t)W * 16, rs4 = (size_t)W * 4;      // bytes per image row
+  int is_t = 0, is_rq = 0, is_col = warp * kDpCols + lane;      // state of the item to be issued next
+  const char *gXi = nullptr, *gRc = nullptr, *gli = nullptr, *glh = nullptr;
+  auto seek = [&]() {                                           // pointers to (row_lo, is_col); a masked column keeps them in range
+    const size_t m0 = (size_t)row_lo * W + min(is_col, W - 1);
+    gXi = reinterpret_cast<const char*>(Pi + m0);
+    gRc = reinterpret_cast<const char*>(Rc + m0);
+    gli = reinterpret_cast<const char*>(li + m0);
+    glh = reinterpret_cast<const char*>(lh + m0);
   };
-  auto load_gather = [&](int n, float4& b, int& lh) {
-    if ((unsigned)n < (unsigned)HW) { b = Pj[n]; lh = lj[n]; }
-  };
-  const float4 none = make_float4(0.f, 0.f, 0.f, -1.f);
-  DepthStream s0, s1, s2;
-  s0.aA = s0.aB = s1.aA = s1.aB = s2.aA = s2.aB = none;
-  s0.lgA = s0.lgB = s1.lgA = s1.lgB = s2.lgA = s2.lgB = -1;
-  float4 bA0 = none, bB0 = none, bA1 = none, bB1 = none;
-  int lhA0 = -1, lhB0 = -1, lhA1 = -1, lhB1 = -1;
-  load_stream(0, s0);
-  load_stream(1, s1);
-  load_gather(s0.nA, bA0, lhA0);
-  load_gather(s0.nB, bB0, lhB0);
-  f2 c_wr2 = make_float2(0.f, 0.f), c_min = make_float2(0.f, 0.f);   // sum om res^2, sum min(q res^2 / sigma^2, kappa^2): <= 8 iterations x 3
-  double cost = 0.0;
-  for (int it = 0; it < niter; ++it) {
-    load_stream(it + 2, s2);
-    load_gather(s1.nA, bA1, lhA1);
-    load_gather(s1.nB, bB1, lhB1);
-    const bool vA = (unsigned)s0.nA < (unsigned)HW && s0.aA.w >= 0.f && bA0.w >= 0.f && (unsigned)s0.lgA < (unsigned)n_seg &&
-                    (unsigned)lhA0 < (unsigned)n_seg;
-    const bool vB = (unsigned)s0.nB < (unsigned)HW && s0.aB.w >= 0.f && bB0.w >= 0.f && (unsigned)s0.lgB < (unsigned)n_seg &&
-                    (unsigned)lhB0 < (unsigned)n_seg;
-    const int kgA = vA ? s0.lgA : -1, kgB = vB ? s0.lgB : -1, khA = vA ? lhA0 : -1, khB = vB ? lhB0 : -1;
-    f2 vg = make_float2(0.f, 0.f), Hg = vg, vh = vg, Hh = vg;
-    if (__any_sync(0xffffffffu, vA || vB)) {                    // whole invalid bands are skipped warp-uniformly
-      // res = s_ij R_ij (e^eta_h X_j) + t_ij - e^eta_g X_i in FP64, rounded once; masked lanes run on zeros
-      const int gA = vA ? s0.lgA : 0, gB = vB ? s0.lgB : 0, hA = vA ? lhA0 : 0, hB = vB ? lhB0 : 0;
-      f2 res[3], xi[3];
-      {
-        const float4 a = s0.aA, b = bA0;
-        const double eg = s_exp[gA], eh = s_exp[n_seg + hA];
-        const double X0 = eh * (double)b.x, X1 = eh * (double)b.y, X2 = eh * (double)b.z;
-        res[0].x = (float)fma(-eg, (double)a.x, fma(sR[0], X0, fma(sR[1], X1, fma(sR[2], X2, T.t[0]))));
-        res[1].x = (float)fma(-eg, (double)a.y, fma(sR[3], X0, fma(sR[4], X1, fma(sR[5], X2, T.t[1]))));
-        res[2].x = (float)fma(-eg, (double)a.z, fma(sR[6], X0, fma(sR[7], X1, fma(sR[8], X2, T.t[2]))));
-        const float ef = s_expf[gA];
-        xi[0].x = ef * a.x; xi[1].x = ef * a.y; xi[2].x = ef * a.z;
-      }
-      {
-        const float4 a = s0.aB, b = bB0;
-        const double eg = s_exp[gB], eh = s_exp[n_seg + hB];
-        const double X0 = eh * (double)b.x, X1 = eh * (double)b.y, X2 = eh * (double)b.z;
-        res[0].y = (float)fma(-eg, (double)a.x, fma(sR[0], X0, fma(sR[1], X1, fma(sR[2], X2, T.t[0]))));
-        res[1].y = (float)fma(-eg, (double)a.y, fma(sR[3], X0, fma(sR[4], X1, fma(sR[5], X2, T.t[1]))));
-        res[2].y = (float)fma(-eg, (double)a.z, fma(sR[6], X0, fma(sR[7], X1, fma(sR[8], X2, T.t[2]))));
-        const float ef = s_expf[gB];
-        xi[0].y = ef * a.x; xi[1].y = ef * a.y; xi[2].y = ef * a.z;
-      }
-      // sqrt(q) = w_i w_j (w = c^(1/4)), 0 for a masked lane: all its weights vanish
-      f2 sq = make_float2(s0.aA.w * bA0.w, s0.aB.w * bB0.w);
-      sq.x = vA ? sq.x : 0.f;
-      sq.y = vB ? sq.y : 0.f;
-      const f2 q = sq * sq;
-      const f2 sc = q * bc(s_cap), kc = sq * bc(k_cap);       // q / sigma^2 and kappa sqrt(q) / sigma
+  seek();
+  auto issue = [&]() {
+    if (is_t < my_items) {
+      const int row0 = row_lo + is_rq * kDpRows, st = (is_t % kDpStages) * kDpRows * 32;
+      const bool col_ok = is_col < W;
+      if (__all_sync(0xffffffffu, col_ok) && row0 + kDpRows <= row_hi) {            // interior item: sixteen plain copies
 #pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        // omega = q w / sigma^2 = min(q / sigma^2, kappa sqrt(q) / (sigma |res|));  rho = omega res^2 - min(q res^2 / sigma^2, kappa^2) / 2
-        const f2 t = kc * make_float2(rcp(fabsf(res[c].x)), rcp(fabsf(res[c].y)));
-        const f2 om = make_float2(fminf(sc.x, t.x), fminf(sc.y, t.y));     // fminf(s, NaN) = s (masked lane, res = 0)
-        const f2 f = om * res[c];
-        c_wr2 = fma2(f, res[c], c_wr2);
-        const f2 r2 = (sc * res[c]) * res[c];
-        c_min = c_min + make_float2(fminf(r2.x, hk2), fminf(r2.y, hk2));
-        const f2 Jh = (res[c] + xi[c]) + bc(-tf[c]);            // J_h = s_ij R_ij X_j(eta) = res - t_ij + X_i(eta)
-        vg = fma2(-f, xi[c], vg);                               // J_g = -X_i(eta)
-        Hg = fma2(om * xi[c], xi[c], Hg);
-        vh = fma2(f, Jh, vh);
-        Hh = fma2(om * Jh, Jh, Hh);
+        for (int r = 0; r < kDpRows; ++r) {
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(u_Xi + 16u * (st + 32 * r)), "l"(gXi + r * rs16) : "memory");
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(u_rec + 16u * (st + 32 * r)), "l"(gRc + r * rs16) : "memory");
+          asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(u_li + 4u * (st + 32 * r)), "l"(gli + r * rs4) : "memory");
+          asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(u_lh + 4u * (st + 32 * r)), "l"(glh + r * rs4) : "memory");
+        }
+      } else {
+#pragma unroll
+        for (int r = 0; r < kDpRows; ++r) {
+          if (col_ok && row0 + r < row_hi) {
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(u_Xi + 16u * (st + 32 * r)), "l"(gXi + r * rs16) : "memory");
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(u_rec + 16u * (st + 32 * r)), "l"(gRc + r * rs16) : "memory");
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(u_li + 4u * (st + 32 * r)), "l"(gli + r * rs4) : "memory");
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(u_lh + 4u * (st + 32 * r)), "l"(glh + r * rs4) : "memory");
+          } else {
+            r_Xi[st + 32 * r + lane] = make_float4(0.f, 0.f, 0.f, -1.f);     // finite values for the masked lanes' arithmetic
+            r_rec[st + 32 * r + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+            r_li[st + 32 * r + lane] = -1;
+            r_lh[st + 32 * r + lane] = -1;
+          }
+        }
       }
-      bin_pair(my_bins, kgA, kgB, vg, Hg, lane);
-      bin_pair(my_bins + 2 * n_seg, khA, khB, vh, Hh, lane);
+      ++is_t;
+      if (++is_rq == nrq) {                                      // next block of columns of this warp
+        is_rq = 0;
+        is_col += kDpWarps * kDpCols;
+        seek();
+      } else {
+        gXi += kDpRows * rs16; gRc += kDpRows * rs16; gli += kDpRows * rs4; glh += kDpRows * rs4;
+      }
     }
-    if ((it & 7) == 7) {                                        // fp32 partials of <= 48 terms -> FP64
+    dp_commit();                                                 // (possibly empty) group: uniform accounting
+  };
+  issue();
+  f2 c_wr2 = make_float2(0.f, 0.f), c_min = make_float2(0.f, 0.f);   // sum om res^2, sum min(q res^2 / sigma^2, kappa^2): <= 4 items x 6 terms
+  double cost = 0.0;
+  for (int t = 0; t < my_items; ++t) {
+    issue();
+    dp_wait<1>();                                                // item t has landed
+    const int st = (t % kDpStages) * kDpRows * 32 + lane;
+    int kg[kDpRows], kh[kDpRows];
+    float vg[kDpRows], Hg[kDpRows], vh[kDpRows], Hh[kDpRows];
+    bool any_valid = false;
+#pragma unroll
+    for (int r = 0; r < kDpRows; ++r) {
+      kh[r] = r_lh[st + 32 * r];                                 // >= 0 <=> the match counts (kernel P)
+      kg[r] = kh[r] >= 0 ? r_li[st + 32 * r] : -1;
+      vg[r] = Hg[r] = vh[r] = Hh[r] = 0.f;
+      any_valid |= kh[r] >= 0;
+    }
+    if (__any_sync(0xffffffffu, any_valid)) {                    // whole invalid bands are skipped warp-uniformly
+#pragma unroll
+      for (int p = 0; p < kDpRows; p += 2) {                     // rows p, p + 1 in the two lanes of the packed arithmetic
+        const float4 aA = r_Xi[st + 32 * p], yA = r_rec[st + 32 * p], aB = r_Xi[st + 32 * (p + 1)], yB = r_rec[st + 32 * (p + 1)];
+        const float2 gA = s_Eg[max(kg[p], 0)], gB = s_Eg[max(kg[p + 1], 0)];
+        const float4 hA0 = s_Eh[2 * max(kh[p], 0)], hA1 = s_Eh[2 * max(kh[p], 0) + 1];
+        const float4 hB0 = s_Eh[2 * max(kh[p + 1], 0)], hB1 = s_Eh[2 * max(kh[p + 1], 0) + 1];
+        const f2 a[3] = {make_float2(aA.x, aB.x), make_float2(aA.y, aB.y), make_float2(aA.z, aB.z)};
+        const f2 y[3] = {make_float2(yA.x, yB.x), make_float2(yA.y, yB.y), make_float2(yA.z, yB.z)};
+        const f2 ct_hi[3] = {make_float2(hA0.z, hB0.z), make_float2(hA1.x, hB1.x), make_float2(hA1.z, hB1.z)};
+        const f2 ct_lo[3] = {make_float2(hA0.w, hB0.w), make_float2(hA1.y, hB1.y), make_float2(hA1.w, hB1.w)};
+        const f2 Eg = make_float2(gA.x, gB.x), Eh = make_float2(hA0.x, hB0.x);
+        // d = E_h - E_g as an unevaluated pair (dh, dl): the difference of the leading parts is exact whenever the two
+        // scales lie within a factor of two of each other (Sterbenz), and otherwise |res| is of the order of |d| |X_i| itself
+        const f2 dh = Eh + (-Eg);
+        const f2 dl = make_float2(hA0.y, hB0.y) + (-make_float2(gA.y, gB.y));
+        // sqrt(q) = w_i w_j from kernel P, 0 for a masked lane: all its weights vanish
+        const f2 sq = make_float2(yA.w, yB.w);
+        const f2 q = sq * sq;
+        const f2 sc = q * bc(s_cap), kc = sq * bc(k_cap);        // q / sigma^2 and kappa sqrt(q) / sigma
+        f2 pvg = make_float2(0.f, 0.f), pHg = pvg, pvh = pvg, pHh = pvg;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          // res = E_h y + [(E_h - E_g) X_i + (1 - E_h) t]: two nested fused multiply-adds on the leading parts -- each rounds
+          // its exact sum once, so what is lost is 2^-24 of the partial result, random from match to match like the rounding y
+          // itself carries -- plus the trailing parts, which carry the per-segment (systematic) bits
+          const f2 res = fma2(Eh, y[c], fma2(dh, a[c], ct_hi[c])) + fma2(dl, a[c], ct_lo[c]);
+          const f2 xi = Eg * a[c];                               // X_i(eta)
+          // omega = q w / sigma^2 = min(q / sigma^2, kappa sqrt(q) / (sigma |res|));  rho = omega res^2 - min(q res^2 / sigma^2, kappa^2) / 2
+          const f2 tt = kc * make_float2(rcp(fabsf(res.x)), rcp(fabsf(res.y)));
+          const f2 om = make_float2(fminf(sc.x, tt.x), fminf(sc.y, tt.y));     // fminf(s, NaN) = s (masked lane: sq = 0)
+          const f2 f = om * res;
+          c_wr2 = fma2(f, res, c_wr2);
+          const f2 r2 = (sc * res) * res;
+          c_min = c_min + make_float2(fminf(r2.x, hk2), fminf(r2.y, hk2));
+          const f2 Jh = (res + xi) + bc(-tf[c]);                 // J_h = s_ij R_ij X_j(eta) = res - t_ij + X_i(eta)
+          pvg = fma2(-f, xi, pvg);                               // J_g = -X_i(eta)
+          pHg = fma2(om * xi, xi, pHg);
+          pvh = fma2(f, Jh, pvh);
+          pHh = fma2(om * Jh, Jh, pHh);
+        }
+        vg[p] = pvg.x; vg[p + 1] = pvg.y; Hg[p] = pHg.x; Hg[p + 1] = pHg.y;
+        vh[p] = pvh.x; vh[p + 1] = pvh.y; Hh[p] = pHh.x; Hh[p + 1] = pHh.y;
+      }
+      bin_records(my_bins, queue, 0, kg, vg, Hg, lane);
+      bin_records(my_bins, queue, n_seg, kh, vh, Hh, lane);
+    }
+    if ((t & 3) == 3) {                                          // fp32 partials of <= 48 terms -> FP64
       cost += (double)(c_wr2.x + c_wr2.y) - 0.5 * (double)(c_min.x + c_min.y);
       c_wr2 = c_min = make_float2(0.f, 0.f);
     }
-    s0 = s1; bA0 = bA1; bB0 = bB1; lhA0 = lhA1; lhB0 = lhB1;
-    s1 = s2;
   }
+  dp_wait<0>();
+  dp_drain(queue, my_bins, true, lane);
   cost += (double)(c_wr2.x + c_wr2.y) - 0.5 * (double)(c_min.x + c_min.y);
   cost = warp_sum(cost);
   if (lane == 0) s_cost[warp] = cost;
   __syncthreads();
   double* out = partial + ((size_t)e * tiles + tile) * (4 * n_seg + 1);
-  for (int q = tid; q < 4 * n_seg; q += kDpThreads) {          // q = (side, label, {g, H})
+  for (int q = tid; q < 4 * n_seg; q += kDpThreads) {           // q = (side, label, {g, H})
     double v = 0.0;
 #pragma unroll
     for (int w = 0; w < kDpWarps; ++w) v += s_bins[(size_t)w * 4 * n_seg + q];
@@ -318,13 +493,13 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
                              const int32_t* h_anchor, int n_anchor, const sim3ba_depth_params& p, int n_iters, double* d_eta,
                              double* h_cost) {
   const int n_total = c->N * n_seg;
-  // tiles of ~kDpTilePx pixels (the per-CTA setup is ~2000 shared-memory words), at least ~4 CTAs per SM in the grid
+  // tiles of whole image rows, ~kDpTilePx pixels each (the per-CTA setup is ~2000 shared-memory words), at least ~4 CTAs per SM in the grid
   const int E1 = std::max(c->E, 1);
-  const int tiles0 = std::max(1, std::min(std::max((c->HW + kDpTilePx - 1) / kDpTilePx, (592 + E1 - 1) / E1), std::max(c->HW / kDpIterPx, 1)));
-  const int per = ((c->HW + tiles0 - 1) / tiles0 + 63) / 64 * 64;     // pixels per tile: a multiple of a warp's 64-pixel chunk
-  const int tiles = (c->HW + per - 1) / per;
+  const int want_tiles = std::max((c->HW + kDpTilePx - 1) / kDpTilePx, (592 + E1 - 1) / E1);
+  const int tile_rows = std::max(kDpRows, ((c->H + want_tiles - 1) / want_tiles + kDpRows - 1) / kDpRows * kDpRows);
+  const int tiles = (c->H + tile_rows - 1) / tile_rows;
   const int rec = 4 * n_seg + 1;
-  const size_t smem = ((size_t)kDpWarps * 4 * n_seg + 2 * n_seg + kDpWarps) * sizeof(double) + (size_t)2 * n_seg * sizeof(float);
+  const size_t smem = kDpWarpBytes * kDpWarps + ((size_t)kDpWarps * 4 * n_seg + kDpWarps) * sizeof(double) + (size_t)n_seg * 40;
   if (smem > c->depth_smem) {
     cudaError_t ea = cudaFuncSetAttribute(k_depth_edge, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (ea != cudaSuccess) return ea;
@@ -350,6 +525,8 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
   int32_t *d_sp_ptr = nullptr, *d_sp_other = nullptr, *d_pairs = nullptr;
   double *d_sp_delta = nullptr, *d_delta = nullptr, *d_partial = nullptr, *d_eta2 = nullptr, *d_cost = nullptr;
   uint8_t* d_anchor = nullptr;
+  float4* d_rec = nullptr;        // kernel P's per-candidate records: y [3], sqrt(q) -- 20 bytes per candidate with the label below
+  int32_t* d_labn = nullptr;
   cudaError_t e = cudaSuccess;
   auto ok = [&](cudaError_t r) { if (e == cudaSuccess) e = r; return e == cudaSuccess; };
   ok(up(&d_sp_ptr, sp_ptr, c->stream)); ok(up(&d_sp_other, sp_other, c->stream)); ok(up(&d_sp_delta, sp_delta, c->stream));
@@ -357,11 +534,20 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
   ok(dmalloc(reinterpret_cast<void**>(&d_partial), std::max<size_t>((size_t)c->E * tiles * rec, 1) * sizeof(double)));
   ok(dmalloc(reinterpret_cast<void**>(&d_eta2), std::max<size_t>(n_total, 1) * sizeof(double)));
   ok(dmalloc(reinterpret_cast<void**>(&d_cost), std::max(n_iters, 1) * sizeof(double)));
+  const size_t EHW = (size_t)c->E * c->HW;
+  ok(dmalloc(reinterpret_cast<void**>(&d_rec), std::max<size_t>(EHW, 1) * sizeof(float4)));
+  ok(dmalloc(reinterpret_cast<void**>(&d_labn), std::max<size_t>(EHW, 1) * sizeof(int32_t)));
+  if (e == cudaSuccess && c->E > 0 && n_iters > 0) {
+    const int chunks = std::max(1, std::min((c->HW + 4095) / 4096, 65535));
+    k_depth_prep<<<c->E * chunks, 256, 0, c->stream>>>(pm_init, c->match, c->edges, d_labels, c->poses, c->HW, n_seg, chunks, d_rec, d_labn);
+    ++c->launches;
+    ok(cudaGetLastError());
+  }
   double *cur = d_eta, *nxt = d_eta2;
   for (int it = 0; it < n_iters && e == cudaSuccess; ++it) {
     if (c->E > 0)
-      k_depth_edge<<<c->E * tiles, kDpThreads, smem, c->stream>>>(pm_init, c->match, c->edges, c->grp_edge, d_labels, cur, c->poses, c->HW, n_seg, tiles,
-                                                                 per, dev, d_partial);
+      k_depth_edge<<<c->E * tiles, kDpThreads, smem, c->stream>>>(pm_init, d_rec, d_labn, c->edges, c->grp_edge, d_labels, cur, c->poses, c->H, c->W,
+                                                                 n_seg, tiles, tile_rows, dev, d_partial);
     k_depth_cost<<<1, 256, 0, c->stream>>>(d_partial, c->E * tiles, rec, cur, n_total, d_pairs, d_delta, n_pairs, dev, d_cost + it);
     k_depth_update<<<(n_total + 127) / 128, 128, 0, c->stream>>>(d_partial, cur, nxt, c->edges, c->kf_ptr, c->kf_edge, d_sp_ptr, d_sp_other,
                                                                  d_sp_delta, d_anchor, n_seg, n_total, tiles, dev);
@@ -374,7 +560,7 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
   cudaError_t es = cudaStreamSynchronize(c->stream);          // the host vectors and temporaries go out of scope
   if (e == cudaSuccess) e = es;
   dfree(d_sp_ptr); dfree(d_sp_other); dfree(d_sp_delta); dfree(d_pairs); dfree(d_delta); dfree(d_anchor);
-  dfree(d_partial); dfree(d_eta2); dfree(d_cost);
+  dfree(d_partial); dfree(d_eta2); dfree(d_cost); dfree(d_rec); dfree(d_labn);
   return e;
 }
 
