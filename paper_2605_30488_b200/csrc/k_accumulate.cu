@@ -35,8 +35,8 @@ constexpr int kStages = 2;                     // ring of gathered X_j pairs per
                                                // no stored 1/|X_i| (14.1 KB + 1 KB reserved per one-warp CTA) let 14 warps share the 228 KB
                                                // of an SM.  Measured on C2: 12 warps / 3 stages 177.6 us, 13 / 2 171.3, 14 / 2 165.8; 16 warps
                                                // with the index buffer refilled in halves 167.8 (not kept)
-constexpr float kCancel = 1.0f / 1024.0f;      // |x|^2 < kCancel |X_i|^2: x = X_i + del has lost 5 bits or more, take the FP64 x instead
-constexpr int kSlots = kPartialStride;         // 40 reduction slots (layout: sim3ba_internal.cuh)
+constexpr float kCancel = 1.0f / 16384.0f;     // |x|^2 < kCancel |X_i|^2: x = X_i + del has lost 7 bits or more -> the match is deferred to FP64
+constexpr int kSlots = 40;                     // reduction slots of a record (layout: sim3ba_internal.cuh)
 constexpr int kAccSlots = 37;                  // slots that carry floating-point sums
 
 // shared-memory carve-up of k_accumulate (dynamic); every array is sliced per warp
@@ -94,7 +94,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 __device__ __forceinline__ void accumulate_pair(f2 (&acc)[kAccSlots], const f2 del0, const f2 del1, const f2 del2,
                                                 const f2 x0, const f2 x1, const f2 x2, f2 d2,
                                                 const f2 Xi0, const f2 Xi1, const f2 Xi2, const f2 rdi,
-                                                const f2 sq, const DevParams& prm, const bool any_direct, const bool dirA, const bool dirB) {
+                                                const f2 sq, const DevParams& prm) {
   const f2 di = fma2(Xi0, Xi0, fma2(Xi1, Xi1, Xi2 * Xi2)) * rdi;   // |X_i| (rdi is clamped: 0 for X_i = 0)
   d2.x = fmaxf(d2.x, 1e-20f); d2.y = fmaxf(d2.y, 1e-20f);
   const f2 rd = make_float2(rsq(d2.x), rsq(d2.y));
@@ -104,16 +104,10 @@ __device__ __forceinline__ void accumulate_pair(f2 (&acc)[kAccSlots], const f2 d
   const f2 den = d + di;
   const f2 e3d = fma2(del0, x0 + Xi0, fma2(del1, x1 + Xi1, del2 * (x2 + Xi2))) * make_float2(rcp(den.x), rcp(den.y));
   const f2 gsc = (e3d * rd) * rdi;
-  f2 e0 = fma2(del0, rd, -(Xi0 * gsc));
-  f2 e1 = fma2(del1, rd, -(Xi1 * gsc));
-  f2 e2 = fma2(del2, rd, -(Xi2 * gsc));
-  f2 e3 = e3d;
-  if (any_direct) {   // warp-uniform and rare: lanes whose x came from the FP64 path (|x| << |X_i|, so |del| ~ |X_i|: nothing cancels
-                      // in the plain differences, whereas del / |x| would carry 2^-24 |del| / |x|) take e = [u - u_i; |x| - |X_i|] as written
-    const f2 t0 = fma2(-Xi0, rdi, u0), t1 = fma2(-Xi1, rdi, u1), t2 = fma2(-Xi2, rdi, u2), t3 = d + (-di);
-    if (dirA) { e0.x = t0.x; e1.x = t1.x; e2.x = t2.x; e3.x = t3.x; }
-    if (dirB) { e0.y = t0.y; e1.y = t1.y; e2.y = t2.y; e3.y = t3.y; }
-  }
+  const f2 e0 = fma2(del0, rd, -(Xi0 * gsc));
+  const f2 e1 = fma2(del1, rd, -(Xi1 * gsc));
+  const f2 e2 = fma2(del2, rd, -(Xi2 * gsc));
+  const f2 e3 = e3d;
   // q = sqrt(c_i c_j); s_c = q / sigma_c^2; omega_c = q w_c / sigma_c^2 = min(s_c, kappa sqrt(q) / (sigma_c |e_c|));
   // rho_c = omega_c e_c^2 - min(s_c e_c^2, kappa^2) / 2
   const f2 q = sq * sq;
@@ -238,7 +232,8 @@ __device__ __forceinline__ void warp_reduce_slots(const float (&acc)[kSlots], do
 __global__ void __launch_bounds__(kAccThreads, kAccCtasPerSm)
 k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, const int32_t* __restrict__ edges,
              const int32_t* __restrict__ grp_kf, const int32_t* __restrict__ grp_ptr, const int32_t* __restrict__ grp_edge,
-             const double* __restrict__ edgeT, double* __restrict__ partials, int HW, int tiles, int idx_tma, DevParams prm) {
+             const double* __restrict__ edgeT, double* __restrict__ partials, unsigned short* __restrict__ def_masks,
+             int32_t* __restrict__ def_flag, int HW, int tiles, int idx_tma, DevParams prm) {
   extern __shared__ __align__(128) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   unsigned char* wb = smem + warp * kWarpBytes;                               // this warp's region
@@ -307,6 +302,7 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
   };
   auto pj_of = [&](int k) -> const float4* { return pm + (size_t)edges[2 * grp_edge[e_beg + k] + 1] * HW; };
 
+  static_assert(2 * kPairs <= 16, "one 16-bit mask of deferred matches per lane and record");
   static_assert(kStages - 1 <= kPairs, "the prologue stays inside the first edge");
   if (n_e > 0) {
     wait_idx(0);
@@ -332,6 +328,7 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
 #pragma unroll
     for (int q = 0; q < kAccSlots; ++q) acc[q] = make_float2(0.f, 0.f);
     unsigned int cnt = 0, sum_m = 0, sum_n = 0;   // <= 16 terms each < 2^28: no overflow (HW <= 2^28 checked at create)
+    unsigned defmask = 0u;                        // this thread's deferred matches of the edge (16 bits)
 
     // delta = T_ij X_j - X_i in FP64: |delta| ~ noise << |x|; in fp32 it would carry ~ulp(|x|) per match
     auto delta = [&](const float4 Xj, float xi0, float xi1, float xi2, float& d0, float& d1, float& d2_) {
@@ -372,32 +369,16 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
         delta(XA1, P0.y, P0.w, P1.y, del0.y, del1.y, del2.y);
         f2 x0 = Xi0 + del0, x1 = Xi1 + del1, x2 = Xi2 + del2;   // x = T_ij X_j
         f2 d2 = fma2(x0, x0, fma2(x1, x1, x2 * x2));
-        // X_i + del carries 2^-24 |del|: where the sum cancels (a stray match mapped to within |X_i| / 32 of the camera
-        // centre; the 1 / |x|^2 terms of the Jacobian then dominate its edge's block) x is the FP64 value rounded.  Rare: one
-        // warp-uniform test per pair.
-        const bool tA = vA && d2.x < d2i.x * kCancel, tB = vB && d2.y < d2i.y * kCancel;
-        const bool any_t = __any_sync(0xffffffffu, tA || tB);
-        {
-          if (any_t) {
-            if (tA) {
-              const double a = (double)XA0.x, b = (double)XA0.y, c = (double)XA0.z;
-              x0.x = (float)fma(Td[0], a, fma(Td[1], b, fma(Td[2], c, Td[9])));
-              x1.x = (float)fma(Td[3], a, fma(Td[4], b, fma(Td[5], c, Td[10])));
-              x2.x = (float)fma(Td[6], a, fma(Td[7], b, fma(Td[8], c, Td[11])));
-            }
-            if (tB) {
-              const double a = (double)XA1.x, b = (double)XA1.y, c = (double)XA1.z;
-              x0.y = (float)fma(Td[0], a, fma(Td[1], b, fma(Td[2], c, Td[9])));
-              x1.y = (float)fma(Td[3], a, fma(Td[4], b, fma(Td[5], c, Td[10])));
-              x2.y = (float)fma(Td[6], a, fma(Td[7], b, fma(Td[8], c, Td[11])));
-            }
-            d2 = fma2(x0, x0, fma2(x1, x1, x2 * x2));
-          }
-        }
+        // X_i + del carries 2^-24 |del|: where the sum cancels (a stray match mapped to within |X_i| / 128 of the camera
+        // centre; the 1 / |x|^2 terms of the Jacobian then dominate its edge's block) the match is DEFERRED: its pixel goes
+        // into the record's bit mask, its lane sits out with zero weight, and k_deferred evaluates it in FP64.  About one match
+        // in 1e5; no branch here.
+        const bool dA = vA && d2.x < d2i.x * kCancel, dB = vB && d2.y < d2i.y * kCancel;
+        defmask |= (dA ? 1u : 0u) << (2 * p) | (dB ? 2u : 0u) << (2 * p);   // bit 2p: match A of pair p, bit 2p + 1: match B
         f2 sq = make_float2(P1.z, P1.w) * make_float2(XA0.w, XA1.w);
-        sq.x = vA ? sq.x : 0.f;
-        sq.y = vB ? sq.y : 0.f;
-        accumulate_pair(acc, del0, del1, del2, x0, x1, x2, d2, Xi0, Xi1, Xi2, rdi, sq, prm, any_t, tA, tB);
+        sq.x = (vA && !dA) ? sq.x : 0.f;
+        sq.y = (vB && !dB) ? sq.y : 0.f;
+        accumulate_pair(acc, del0, del1, del2, x0, x1, x2, d2, Xi0, Xi1, Xi2, rdi, sq, prm);
         const unsigned mA = vA ? 0xffffffffu : 0u, mB = vB ? 0xffffffffu : 0u;
         cnt += (mA & 1u) + (mB & 1u);
         sum_m += ((unsigned)pa & mA) + ((unsigned)pb & mB);
@@ -417,8 +398,15 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
       float accs[kSlots];
 #pragma unroll
       for (int q = 0; q < kSlots; ++q) accs[q] = (q < kAccSlots) ? acc[q].x + acc[q].y : 0.f;
-      warp_reduce_slots(accs, partials + ((size_t)e * (tiles * kWarps) + tile * kWarps + warp) * kPartialStride, lane,
-                        (unsigned long long)cnt, chk);
+      double* rec = partials + ((size_t)e * (tiles * kWarps) + tile * kWarps + warp) * kPartialStride;
+      warp_reduce_slots(accs, rec, lane, (unsigned long long)cnt, chk);
+      // deferred matches: slot kSlotDef = the lanes that hold some (0 almost always); then their 16-bit masks and the edge's flag
+      const unsigned lanes_def = __ballot_sync(0xffffffffu, defmask != 0u);
+      if (lane == 0) reinterpret_cast<unsigned long long*>(rec)[kSlotDef] = lanes_def;
+      if (lanes_def) {
+        def_masks[((size_t)e * (tiles * kWarps) + tile * kWarps + warp) * 32 + lane] = (unsigned short)defmask;
+        if (lane == 0) atomicOr(def_flag + e, 1);
+      }
     }
     __syncwarp();   // every lane is done with index buffer k & 1 (free for edge k + 2)
   }
@@ -426,9 +414,10 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
 
 // a1: per-edge pose prep, T_ij = T_i^-1 T_j -> s_ij R_ij [9] row-major, t_ij [3], FP64
 __global__ void __launch_bounds__(128)
-k_edge_prep(const double* __restrict__ poses, const int32_t* __restrict__ edges, double* __restrict__ edgeT, int E) {
+k_edge_prep(const double* __restrict__ poses, const int32_t* __restrict__ edges, double* __restrict__ edgeT, int32_t* __restrict__ def_flag, int E) {
   const int e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= E) return;
+  def_flag[e] = 0;                                             // no deferred matches yet at these poses (kernel 1 marks the edge)
   const Sim3d Tij = relative_pose(load_pose(poses + 8 * edges[2 * e]), load_pose(poses + 8 * edges[2 * e + 1]));
   double* o = edgeT + (size_t)e * 12;
 #pragma unroll
@@ -441,11 +430,91 @@ k_edge_prep(const double* __restrict__ poses, const int32_t* __restrict__ edges,
 // 0 .. kFinGroups - 1), then the adjoint congruence A_e = Ad^T M Ad, b_e = Ad^T c with Ad = Ad_{T_i^-1}.
 // Two shapes: 6 groups / 256 threads, and 24 groups / 1024 threads for few edges with many records (latency of the serial
 // record loop against the number of resident CTAs); the choice depends on (E, records) only, so results stay reproducible.
+// One DEFERRED match (pixel m of i, see kernel 1) in FP64, straight from the definitions: x = T_ij X_j[n], e = [u - u_i; d - d_i]
+// (Eq. (1)), J_xi = [[(I - u u^T)/d, -[u]x, 0], [u^T, 0, d]] (Eq. (6)), omega_c = q min(1, kappa/|r_c|)/sigma_c^2
+// (PAPER.md:76); its terms are added to the slots of the edge's sums (layout: sim3ba_internal.cuh).
+struct RareParams { double sigma_ray, sigma_dist, huber_k; };
+__device__ __forceinline__ void add_deferred_match(double* __restrict__ sum, const float4 Xi4, const float4 Xj4, const double* __restrict__ T, RareParams rp) {
+  const double Xj[3] = {(double)Xj4.x, (double)Xj4.y, (double)Xj4.z}, Xi[3] = {(double)Xi4.x, (double)Xi4.y, (double)Xi4.z};
+  double x[3];
+  for (int r = 0; r < 3; ++r) x[r] = fma(T[3 * r], Xj[0], fma(T[3 * r + 1], Xj[1], fma(T[3 * r + 2], Xj[2], T[9 + r])));
+  const double d = fmax(sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]), 1e-12);
+  const double di = fmax(sqrt(Xi[0] * Xi[0] + Xi[1] * Xi[1] + Xi[2] * Xi[2]), 1e-12);
+  const double u[3] = {x[0] / d, x[1] / d, x[2] / d};
+  const double e[4] = {u[0] - Xi[0] / di, u[1] - Xi[1] / di, u[2] - Xi[2] / di, d - di};
+  const double sq = (double)Xi4.w * (double)Xj4.w, q = sq * sq;            // w = c^(1/4)
+  double J[4][7];
+  for (int r = 0; r < 3; ++r) {
+    for (int c = 0; c < 3; ++c) J[r][c] = ((r == c ? 1.0 : 0.0) - u[r] * u[c]) / d;
+    J[r][6] = 0.0;
+    J[3][r] = u[r];
+    J[3][3 + r] = 0.0;
+  }
+  J[0][3] = 0.0;   J[0][4] = u[2];  J[0][5] = -u[1];                        // -[u]x
+  J[1][3] = -u[2]; J[1][4] = 0.0;   J[1][5] = u[0];
+  J[2][3] = u[1];  J[2][4] = -u[0]; J[2][5] = 0.0;
+  J[3][6] = d;
+  for (int c = 0; c < 4; ++c) {
+    const double sig = c < 3 ? rp.sigma_ray : rp.sigma_dist;
+    const double r = sq * e[c] / sig, ar = fabs(r);
+    const double om = q * (ar <= rp.huber_k ? 1.0 : rp.huber_k / ar) / (sig * sig);
+    sum[35] += om * e[c] * e[c];
+    sum[36] += fmin(r * r, rp.huber_k * rp.huber_k);
+    for (int a = 0; a < 7; ++a) {
+      sum[28 + a] += om * J[c][a] * e[c];
+      for (int b = a; b < 7; ++b) sum[a * 7 - a * (a - 1) / 2 + (b - a)] += om * J[c][a] * J[c][b];
+    }
+  }
+}
+
+// The deferred matches of every edge: one warp per edge.  A lane visits the records lane, lane + 32, ... of the edge; a record
+// whose slot kSlotDef is non-zero names the lanes of kernel 1 that hold deferred matches; def_masks has their 16-bit masks (bit
+// 2p: pixel 64 p + lane of the record's 512-pixel slice, bit 2p + 1: pixel 64 p + 32 + lane).  Sums in FP64: per lane in record / lane / bit order, then a
+// butterfly over the lanes -- a fixed order.  def_sums [E][kSlots]: slots 0..36 as in a record.
+__global__ void __launch_bounds__(32)
+k_deferred(const double* __restrict__ partials, const unsigned short* __restrict__ def_masks, const int32_t* __restrict__ def_flag, int records,
+           const int32_t* __restrict__ edges, const float4* __restrict__ pm, const int32_t* __restrict__ match,
+           const double* __restrict__ edgeT, int HW, RareParams rp, double* __restrict__ def_sums) {
+  const int e = blockIdx.x, lane = threadIdx.x;
+  if (def_flag[e] == 0) return;                               // almost every edge: k_finalize does not read def_sums then
+  const double* p = partials + (size_t)e * records * kPartialStride;
+  double sum[kAccSlots];
+#pragma unroll
+  for (int q = 0; q < kAccSlots; ++q) sum[q] = 0.0;
+  const int i = edges[2 * e], j = edges[2 * e + 1];
+  for (int c = lane; c < records; c += 32) {
+    const double* r = p + (size_t)c * kPartialStride;
+    unsigned lanes = (unsigned)reinterpret_cast<const unsigned long long*>(r)[kSlotDef];
+    while (lanes) {
+      const int l = __ffs(lanes) - 1;
+      lanes &= lanes - 1;
+      unsigned bits = def_masks[((size_t)e * records + c) * 32 + l];
+      while (bits) {
+        const int b = __ffs(bits) - 1;
+        bits &= bits - 1;
+        const int m = c * kWarpPx + 64 * (b >> 1) + 32 * (b & 1) + l;
+        if (m >= HW) continue;
+        const int n = match[(size_t)e * HW + m];
+        add_deferred_match(sum, pm[(size_t)i * HW + m], pm[(size_t)j * HW + n], edgeT + (size_t)e * 12, rp);
+      }
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < kAccSlots; ++q) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum[q] += __shfl_xor_sync(0xffffffffu, sum[q], o);
+  }
+  if (lane == 0) {
+#pragma unroll
+    for (int q = 0; q < kAccSlots; ++q) def_sums[(size_t)e * kSlots + q] = sum[q];
+  }
+}
+
 template <int kFinGroups>
 __global__ void __launch_bounds__(kFinGroups * 40 + 16)
 k_finalize(const double* __restrict__ partials, const int32_t* __restrict__ edges, const double* __restrict__ poses,
            double* __restrict__ blocks35, double* __restrict__ edge_cost, int32_t* __restrict__ n_valid,
-           unsigned long long* __restrict__ checksum, int records) {
+           unsigned long long* __restrict__ checksum, int records, const double* __restrict__ def_sums, const int32_t* __restrict__ def_flag) {
   __shared__ double s_part[kFinGroups][kSlots];
   __shared__ double s_sum[kSlots];
   __shared__ double s_M[49], s_Ad[49], s_T[49];
@@ -457,7 +526,7 @@ k_finalize(const double* __restrict__ partials, const int32_t* __restrict__ edge
       double v = 0.0;
       for (int c = grp; c < records; c += kFinGroups) v += p[(size_t)c * kPartialStride + q];
       s_part[grp][q] = v;
-    } else {   // integer slots (and the unused one): exact in any order
+    } else {   // integer slots (and the deferred-lane masks, unused here): exact in any order
       unsigned long long v = 0ull;
       for (int c = grp; c < records; c += kFinGroups) v += reinterpret_cast<const unsigned long long*>(p + (size_t)c * kPartialStride)[q];
       reinterpret_cast<unsigned long long*>(&s_part[grp][0])[q] = v;
@@ -477,6 +546,7 @@ k_finalize(const double* __restrict__ partials, const int32_t* __restrict__ edge
     for (int grp = 0; grp < kFinGroups; ++grp) v += reinterpret_cast<const unsigned long long*>(&s_part[grp][0])[t];
     if (t == kSlotCnt) n_valid[e] = (int32_t)v; else checksum[e] = v;
   }
+  if (t < kSlotCnt && def_flag[e] != 0) s_sum[t] += def_sums[(size_t)e * kSlots + t];   // the deferred matches of the edge, evaluated in FP64 (k_deferred)
   __syncthreads();
   if (t < 49) {
     const int r = t / 7, c = t % 7;
@@ -552,24 +622,26 @@ cudaError_t launch_accumulate(Ctx* c) {
   p.k_over_sigma_ray = c->prm.huber_k / c->prm.sigma_ray;
   p.k_over_sigma_dist = c->prm.huber_k / c->prm.sigma_dist;
   p.huber_k2 = c->prm.huber_k * c->prm.huber_k;
-  k_edge_prep<<<(c->E + 127) / 128, 128, 0, c->stream>>>(c->poses, c->edges, c->edgeT, c->E);
+  k_edge_prep<<<(c->E + 127) / 128, 128, 0, c->stream>>>(c->poses, c->edges, c->edgeT, c->def_flag, c->E);
   cudaError_t err = cudaGetLastError();
   if (err != cudaSuccess) return err;
   // TMA bulk copies of the match indices need 16-byte granules and addresses
   const int idx_tma = (c->HW % 4 == 0) && (reinterpret_cast<uintptr_t>(c->match) % 16 == 0);
   k_accumulate<<<c->n_groups * c->chunks, kAccThreads, kAccSmem, c->stream>>>(
-      c->pm, c->match, c->edges, c->grp_kf, c->grp_ptr, c->grp_edge, c->edgeT, c->partials, c->HW, c->chunks, idx_tma, p);
+      c->pm, c->match, c->edges, c->grp_kf, c->grp_ptr, c->grp_edge, c->edgeT, c->partials, c->def_masks, c->def_flag, c->HW, c->chunks, idx_tma, p);
   err = cudaGetLastError();
   if (err != cudaSuccess) return err;
   if (c->profiling) cudaEventRecord(c->ev[1], c->stream);
   const int records = c->chunks * (kAccThreads / 32);
+  const RareParams rp{(double)c->prm.sigma_ray, (double)c->prm.sigma_dist, (double)c->prm.huber_k};
+  k_deferred<<<c->E, 32, 0, c->stream>>>(c->partials, c->def_masks, c->def_flag, records, c->edges, c->pm, c->match, c->edgeT, c->HW, rp, c->def_sums);
   if (records >= 256 && c->E <= 600)
     k_finalize<24><<<c->E, 24 * 40 + 16, 0, c->stream>>>(c->partials, c->edges, c->poses, c->blocks35, c->edge_cost, c->n_valid,
-                                                         c->checksum, records);
+                                                         c->checksum, records, c->def_sums, c->def_flag);
   else
     k_finalize<6><<<c->E, 6 * 40 + 16, 0, c->stream>>>(c->partials, c->edges, c->poses, c->blocks35, c->edge_cost, c->n_valid,
-                                                       c->checksum, records);
-  c->launches += 3;
+                                                       c->checksum, records, c->def_sums, c->def_flag);
+  c->launches += 4;
   return cudaGetLastError();
 }
 

@@ -136,7 +136,7 @@ cudaError_t upload(T** dst, const std::vector<T>& src, cudaStream_t s) {
 void free_all(Ctx* c) {
   dfree(c->pm); dfree(c->pm0); dfree(c->edges); dfree(c->grp_kf); dfree(c->grp_ptr); dfree(c->grp_edge); dfree(c->edgeT); dfree(c->fixed_mask); dfree(c->poses);
   dfree(c->kf_ptr); dfree(c->kf_edge); dfree(c->pair_kf); dfree(c->pair_ptr); dfree(c->pair_edge);
-  dfree(c->partials); dfree(c->blocks35); dfree(c->edge_cost); dfree(c->n_valid); dfree(c->checksum);
+  dfree(c->partials); dfree(c->def_sums); dfree(c->def_masks); dfree(c->def_flag); dfree(c->blocks35); dfree(c->edge_cost); dfree(c->n_valid); dfree(c->checksum);
   dfree(c->Hd); dfree(c->L); dfree(c->g); dfree(c->rhs); dfree(c->ysol); dfree(c->Dinv); dfree(c->pairhi_ptr);
   free_plan(c->plan_sparse); free_plan(c->plan_dense); free_bb_plan(c->plan_bb);
   dfree(c->tau); dfree(c->total_cost); dfree(c->fail_flag); dfree(c->d_eps_used); dfree(c->bar); dfree(c->solve_stamps);
@@ -293,6 +293,9 @@ int sim3ba_create(sim3ba_ctx** out, int32_t n_kf, int32_t height, int32_t width,
   CUB(dev_alloc(&c->poses, (size_t)8 * c->N));
   CUB(dev_alloc(&c->partials, (size_t)c->E * c->chunks * (kAccThreads / 32) * kPartialStride));
   CUB(dev_alloc(&c->blocks35, (size_t)c->E * 35));
+  CUB(dev_alloc(&c->def_sums, (size_t)c->E * 40));
+  CUB(dev_alloc(&c->def_masks, (size_t)c->E * c->chunks * (kAccThreads / 32) * 32));
+  CUB(dev_alloc(&c->def_flag, (size_t)c->E));
   CUB(dev_alloc(&c->edge_cost, (size_t)c->E));
   CUB(dev_alloc(&c->n_valid, (size_t)c->E));
   CUB(dev_alloc(&c->checksum, (size_t)c->E));

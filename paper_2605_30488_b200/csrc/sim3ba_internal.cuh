@@ -30,9 +30,12 @@ constexpr int kAccThreads = 32;      // accumulate CTA: ONE warp -- warps are in
 constexpr int kTilePx = 16 * kAccThreads;   // pixels of a keyframe handled by one accumulate CTA (512 contiguous per warp)
 // doubles per (edge, 512-pixel warp slice) partial record: [0..27] upper triangle of M = sum J_xi^T Omega J_xi (row-major,
 // r <= c; (3,6), (4,6), (5,6) are structurally zero), [28..34] c = sum J_xi^T Omega e, [35] sum w r^2,
-// [36] sum min(r^2, kappa^2) (robust cost = [35] - [36]/2), [37] n_valid (int64 bits), [38] checksum (uint64 bits)
+// [36] sum min(r^2, kappa^2) (robust cost = [35] - [36]/2), [37] n_valid (int64 bits), [38] checksum (uint64 bits),
+// [39] ballot of the lanes of kernel 1 holding DEFERRED matches (int64 bits; 0 almost always): matches whose x = X_i + delta
+// cancels (|x| << |X_i|) are left out of kernel 1's fp32 sums and evaluated in FP64 by k_deferred; their per-lane 16-bit masks
+// go to Ctx::def_masks, the edge is marked in Ctx::def_flag
 constexpr int kPartialStride = 40;
-constexpr int kSlotCnt = 37, kSlotChk = 38;
+constexpr int kSlotCnt = 37, kSlotChk = 38, kSlotDef = 39;
 constexpr int kNB = 64;              // Cholesky block size
 
 struct DevParams {       // robust-kernel constants, fp32, passed by value to kernel 1
@@ -120,6 +123,9 @@ struct Ctx {
   std::vector<uint8_t> h_fixed;
   // per-edge results
   double* partials = nullptr;      // [E][chunks * warps per CTA][kPartialStride]: one record per (edge, 512-pixel slice)
+  double* def_sums = nullptr;      // [E][40]: FP64 sums over the deferred matches of an edge (k_deferred), slots as in a record
+  unsigned short* def_masks = nullptr;   // [E][records][32]: per record and lane of kernel 1, the 16-bit mask of its deferred matches (written only where a record has some)
+  int32_t* def_flag = nullptr;     // [E]: non-zero if the edge has deferred matches at the current poses (zeroed by k_edge_prep)
   double* blocks35 = nullptr;      // [E][35]
   double* edge_cost = nullptr;     // [E]
   int32_t* n_valid = nullptr;      // [E]
