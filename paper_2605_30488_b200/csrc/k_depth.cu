@@ -86,9 +86,10 @@ __device__ __forceinline__ double warp_sum(double v) {
 // Kernel P: the eta-independent part of every candidate match, once per structure pass.
 __global__ void __launch_bounds__(256)
 k_depth_prep(const float4* __restrict__ pm, const int32_t* __restrict__ match, const int32_t* __restrict__ edges,
-             const int32_t* __restrict__ labels, const double* __restrict__ poses, int HW, int n_seg, int chunks,
+             const int32_t* __restrict__ grp_edge, const int32_t* __restrict__ labels, const double* __restrict__ poses, int HW, int n_seg, int chunks,
              float4* __restrict__ rec, int32_t* __restrict__ lab_n) {
-  const int e = blockIdx.x / chunks, chunk = blockIdx.x - e * chunks;
+  // kernel 1's launch order (edges sorted by keyframe i): a keyframe's pointmap and labels are fetched from HBM once
+  const int k = blockIdx.x / chunks, chunk = blockIdx.x - k * chunks, e = grp_edge[k];
   const int i = edges[2 * e], j = edges[2 * e + 1];
   const Sim3d T = relative_pose(load_pose(poses + 8 * i), load_pose(poses + 8 * j));   // T_ij
   double sR[9];
@@ -101,26 +102,41 @@ k_depth_prep(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
   const int32_t* __restrict__ lj = labels + (size_t)j * HW;
   const int per = (HW + chunks - 1) / chunks;
   const int m1 = min(HW, (chunk + 1) * per);
-  for (int m = chunk * per + threadIdx.x; m < m1; m += 256) {
-    const int n = __ldcs(mt + m);
-    float4 out = make_float4(0.f, 0.f, 0.f, 0.f);
-    int lh = -1;
-    if ((unsigned)n < (unsigned)HW) {
-      const float4 a = Pi[m], b = Pj[n];
-      const int lg = li[m];
-      lh = lj[n];
-      if (a.w >= 0.f && b.w >= 0.f && (unsigned)lg < (unsigned)n_seg && (unsigned)lh < (unsigned)n_seg) {
-        const double X0 = (double)b.x, X1 = (double)b.y, X2 = (double)b.z;
-        out.x = (float)(fma(sR[0], X0, fma(sR[1], X1, fma(sR[2], X2, T.t[0]))) - (double)a.x);
-        out.y = (float)(fma(sR[3], X0, fma(sR[4], X1, fma(sR[5], X2, T.t[1]))) - (double)a.y);
-        out.z = (float)(fma(sR[6], X0, fma(sR[7], X1, fma(sR[8], X2, T.t[2]))) - (double)a.z);
-        out.w = a.w * b.w;                                       // sqrt(q) = w_i w_j (w = c^(1/4)) > 0
-      } else {
-        lh = -1;
-      }
+  constexpr int kB = 4;                                          // matches in flight per thread: all loads of a batch are issued before its arithmetic
+  for (int mb = chunk * per + threadIdx.x; mb < m1; mb += 256 * kB) {
+    int n[kB], lg[kB], lh[kB];
+    float4 a[kB], b[kB];
+#pragma unroll
+    for (int u = 0; u < kB; ++u) {
+      const int m = mb + 256 * u;
+      n[u] = m < m1 ? __ldcs(mt + m) : -1;
     }
-    rec[(size_t)e * HW + m] = out;                               // w = 0 marks "no term"
-    lab_n[(size_t)e * HW + m] = lh;
+#pragma unroll
+    for (int u = 0; u < kB; ++u) {
+      const int m = mb + 256 * u;
+      const bool in = (unsigned)n[u] < (unsigned)HW;
+      a[u] = in ? Pi[m] : make_float4(0.f, 0.f, 0.f, -1.f);
+      lg[u] = in ? li[m] : -1;
+      b[u] = in ? Pj[n[u]] : make_float4(0.f, 0.f, 0.f, -1.f);
+      lh[u] = in ? lj[n[u]] : -1;
+    }
+#pragma unroll
+    for (int u = 0; u < kB; ++u) {
+      const int m = mb + 256 * u;
+      if (m >= m1) break;
+      float4 out = make_float4(0.f, 0.f, 0.f, 0.f);
+      int lab = -1;
+      if (a[u].w >= 0.f && b[u].w >= 0.f && (unsigned)lg[u] < (unsigned)n_seg && (unsigned)lh[u] < (unsigned)n_seg) {
+        const double X0 = (double)b[u].x, X1 = (double)b[u].y, X2 = (double)b[u].z;
+        out.x = (float)(fma(sR[0], X0, fma(sR[1], X1, fma(sR[2], X2, T.t[0]))) - (double)a[u].x);
+        out.y = (float)(fma(sR[3], X0, fma(sR[4], X1, fma(sR[5], X2, T.t[1]))) - (double)a[u].y);
+        out.z = (float)(fma(sR[6], X0, fma(sR[7], X1, fma(sR[8], X2, T.t[2]))) - (double)a[u].z);
+        out.w = a[u].w * b[u].w;                                 // sqrt(q) = w_i w_j (w = c^(1/4)) > 0
+        lab = lh[u];
+      }
+      __stcs(rec + (size_t)e * HW + m, out);                     // w = 0 marks "no term"
+      __stcs(lab_n + (size_t)e * HW + m, lab);
+    }
   }
 }
 
@@ -539,7 +555,7 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
   ok(dmalloc(reinterpret_cast<void**>(&d_labn), std::max<size_t>(EHW, 1) * sizeof(int32_t)));
   if (e == cudaSuccess && c->E > 0 && n_iters > 0) {
     const int chunks = std::max(1, std::min((c->HW + 4095) / 4096, 65535));
-    k_depth_prep<<<c->E * chunks, 256, 0, c->stream>>>(pm_init, c->match, c->edges, d_labels, c->poses, c->HW, n_seg, chunks, d_rec, d_labn);
+    k_depth_prep<<<c->E * chunks, 256, 0, c->stream>>>(pm_init, c->match, c->edges, c->grp_edge, d_labels, c->poses, c->HW, n_seg, chunks, d_rec, d_labn);
     ++c->launches;
     ok(cudaGetLastError());
   }
