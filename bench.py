@@ -405,10 +405,17 @@ def run_ours(args):
             costs = w.ba.depth_refine(labels, d.n_seg, d.pairs, d.delta, d.anchor_kf, eta, n_dit)
             ev1.record()
             torch.cuda.synchronize()
+            it_ms = ev0.elapsed_time(ev1) / n_dit
+            dbytes = 20.0 * g.n_edges * g.hw + 20.0 * g.n_kf * g.hw      # per iteration: record + label per candidate, X_i + label per pixel
             depth["per_labelling"].append({
                 "labels": "4x8 grid (BASELINE config 5: 32 segments per keyframe)" if irregular == 0 else
                           "jittered superpixels (the paper's M_k ~ 200, PAPER.md:126)",
-                "segments_per_kf": d.n_seg, "ms_per_iteration": ev0.elapsed_time(ev1) / n_dit,
+                "segments_per_kf": d.n_seg, "ms_per_iteration": it_ms,
+                "roofline": {"bound": "hbm", "kernel": "k_depth_edge", "algorithmic_bytes_per_iteration": dbytes,
+                             "achieved": dbytes / (it_ms * 1e-3) / 1e9, "peak": load_peaks()[0], "unit": "GB/s",
+                             "frac": dbytes / (it_ms * 1e-3) / 1e9 / load_peaks()[0],
+                             "note": "time = the whole iteration (k_depth_edge + objective + update kernels) plus a tenth of the "
+                                     "once-per-pass k_depth_prep"},
                 "objective_first_last": [float(costs[0]), float(costs[-1])]})
             if irregular == 0 and args.config == 5:
                 h_lab = torch.from_numpy(d.labels).pin_memory()

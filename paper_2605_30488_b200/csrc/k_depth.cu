@@ -70,6 +70,7 @@ constexpr size_t kDpWarpBytes = kDpOffQ + 12 * kDpQueue;                        
 
 struct DepthDev {
   double inv_sigma, huber_k, lambda_smooth, lambda_prior, lambda_lm, eta_max;
+  float s_cap, k_cap, hk2;     // 1 / sigma^2, kappa / sigma, kappa^2 in fp32 (host-computed: the per-match arithmetic's constants)
 };
 
 __device__ __forceinline__ uint32_t dp_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -148,34 +149,45 @@ k_depth_prep(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
 // its next peer above and the odd-ranked lanes of every group drop out, so the rounds needed are log2 of the largest
 // group and the order of the additions is fixed by the lane numbers.  The first lane of a group adds its total to the bin.
 __device__ __forceinline__ void bin_phase(double* bins, int bin, float a, float b, int lane) {
-  const unsigned peers = __match_any_sync(0xffffffffu, bin >= 0 ? bin : -1 - lane);   // nothing to offer: a unique key
-  const bool single = peers == (1u << lane);
-  const bool first = (peers & (0u - peers)) == (1u << lane);
-  unsigned active = __ballot_sync(0xffffffffu, bin >= 0 && first && !single);          // first lanes of the shared bins
-  if (__popc(active) <= 2) {
-    if (bin >= 0 && single) { bins[2 * bin] += (double)a; bins[2 * bin + 1] += (double)b; }
-    while (active) {
-      const int leader = __ffs(active) - 1;
-      const unsigned grp = __shfl_sync(0xffffffffu, peers, leader);
-      const bool mine = (grp >> lane) & 1u;
-      f2 x = mine ? make_float2(a, b) : make_float2(0.f, 0.f);
+  bool add;                                                      // a lane adds at most once per phase: (a, b) end up holding its total
+  const int bin0 = __shfl_sync(0xffffffffu, bin, 0);
+  if (__all_sync(0xffffffffu, bin == bin0)) {                    // the usual patch: one segment across the warp's 32 columns
+    f2 x = make_float2(a, b);
 #pragma unroll
-      for (int o = 1; o < 32; o <<= 1) x = x + make_float2(__shfl_xor_sync(0xffffffffu, x.x, o), __shfl_xor_sync(0xffffffffu, x.y, o));
-      if (lane == leader) { bins[2 * bin] += (double)x.x; bins[2 * bin + 1] += (double)x.y; }
-      active &= active - 1;
-    }
+    for (int o = 1; o < 32; o <<= 1) x = x + make_float2(__shfl_xor_sync(0xffffffffu, x.x, o), __shfl_xor_sync(0xffffffffu, x.y, o));
+    a = x.x; b = x.y;
+    add = lane == 0 && bin >= 0;
   } else {
-    int rank = __popc(peers & ((1u << lane) - 1u));
-    unsigned above = peers & (0xfffffffeu << lane);
-    while (__any_sync(0xffffffffu, above != 0u)) {
-      const int next = __ffs(above);                             // 1 + lane of the next peer above, 0 if none
-      const float ta = __shfl_sync(0xffffffffu, a, (next - 1) & 31), tb = __shfl_sync(0xffffffffu, b, (next - 1) & 31);
-      if (next) { a += ta; b += tb; }
-      above &= __ballot_sync(0xffffffffu, !(rank & 1));          // odd-ranked lanes have been absorbed: out of every mask
-      rank >>= 1;
+    const unsigned peers = __match_any_sync(0xffffffffu, bin >= 0 ? bin : -1 - lane);   // nothing to offer: a unique key
+    const bool single = peers == (1u << lane);
+    const bool first = (peers & (0u - peers)) == (1u << lane);
+    unsigned active = __ballot_sync(0xffffffffu, bin >= 0 && first && !single);          // first lanes of the shared bins
+    add = bin >= 0 && first;
+    if (__popc(active) <= 2) {
+      const float a0 = a, b0 = b;
+      while (active) {
+        const int leader = __ffs(active) - 1;
+        const unsigned grp = __shfl_sync(0xffffffffu, peers, leader);
+        const bool mine = (grp >> lane) & 1u;
+        f2 x = mine ? make_float2(a0, b0) : make_float2(0.f, 0.f);
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) x = x + make_float2(__shfl_xor_sync(0xffffffffu, x.x, o), __shfl_xor_sync(0xffffffffu, x.y, o));
+        if (lane == leader) { a = x.x; b = x.y; }
+        active &= active - 1;
+      }
+    } else {
+      int rank = __popc(peers & ((1u << lane) - 1u));
+      unsigned above = peers & (0xfffffffeu << lane);
+      while (__any_sync(0xffffffffu, above != 0u)) {
+        const int next = __ffs(above);                           // 1 + lane of the next peer above, 0 if none
+        const float ta = __shfl_sync(0xffffffffu, a, (next - 1) & 31), tb = __shfl_sync(0xffffffffu, b, (next - 1) & 31);
+        if (next) { a += ta; b += tb; }
+        above &= __ballot_sync(0xffffffffu, !(rank & 1));        // odd-ranked lanes have been absorbed: out of every mask
+        rank >>= 1;
+      }
     }
-    if (bin >= 0 && first) { bins[2 * bin] += (double)a; bins[2 * bin + 1] += (double)b; }
   }
+  if (add) { bins[2 * bin] += (double)a; bins[2 * bin + 1] += (double)b; }   // distinct bins: these adds do not meet
   __syncwarp();                                                  // the next phase's adds may come from other lanes
 }
 
@@ -267,8 +279,7 @@ k_depth_edge(const float4* __restrict__ pm, const float4* __restrict__ rec, cons
   const float4* __restrict__ Rc = rec + (size_t)e * HW;
   const int32_t* __restrict__ li = labels + (size_t)i * HW;
   const int32_t* __restrict__ lh = lab_n + (size_t)e * HW;
-  const float isg = (float)prm.inv_sigma, hk = (float)prm.huber_k;
-  const float s_cap = isg * isg, k_cap = hk * isg, hk2 = hk * hk;
+  const float s_cap = prm.s_cap, k_cap = prm.k_cap, hk2 = prm.hk2;
   double* my_bins = s_bins + (size_t)warp * 4 * n_seg;
   unsigned char* wb = dp_smem + kDpWarpBytes * warp;
   float4* r_Xi = reinterpret_cast<float4*>(wb + kDpOffXi);
@@ -461,20 +472,21 @@ __global__ void k_depth_update(const double* __restrict__ partial, const double*
   eta_out[s] = es + step;
 }
 
-__global__ void __launch_bounds__(256)
+constexpr int kDpCostThreads = 1024;
+__global__ void __launch_bounds__(kDpCostThreads)
 k_depth_cost(const double* __restrict__ partial, int n_rec, int rec, const double* __restrict__ eta, int n_total,
              const int32_t* __restrict__ pairs, const double* __restrict__ delta, int n_pairs, DepthDev prm, double* __restrict__ out) {
-  __shared__ double s[256];
+  __shared__ double s[kDpCostThreads];
   double v = 0.0;
-  for (int q = threadIdx.x; q < n_rec; q += 256) v += partial[(size_t)q * rec + rec - 1];
-  for (int q = threadIdx.x; q < n_pairs; q += 256) {
+  for (int q = threadIdx.x; q < n_rec; q += kDpCostThreads) v += partial[(size_t)q * rec + rec - 1];
+  for (int q = threadIdx.x; q < n_pairs; q += kDpCostThreads) {
     const double d = eta[pairs[2 * q]] - eta[pairs[2 * q + 1]] + delta[q];
     v += 0.5 * prm.lambda_smooth * d * d;
   }
-  for (int q = threadIdx.x; q < n_total; q += 256) v += 0.5 * prm.lambda_prior * eta[q] * eta[q];
+  for (int q = threadIdx.x; q < n_total; q += kDpCostThreads) v += 0.5 * prm.lambda_prior * eta[q] * eta[q];
   s[threadIdx.x] = v;
   __syncthreads();
-  for (int o = 128; o > 0; o >>= 1) {
+  for (int o = kDpCostThreads / 2; o > 0; o >>= 1) {
     if (threadIdx.x < o) s[threadIdx.x] += s[threadIdx.x + o];
     __syncthreads();
   }
@@ -522,7 +534,11 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
     c->depth_smem = smem;
   }
   const float4* pm_init = c->pm0 ? c->pm0 : c->pm;               // pristine X_init (Eq. (8)): see sim3ba_apply_depth
-  DepthDev dev{1.0 / (double)p.sigma_point, (double)p.huber_k, p.lambda_smooth, p.lambda_prior, p.lambda_lm, p.eta_max};
+  DepthDev dev{1.0 / (double)p.sigma_point, (double)p.huber_k, p.lambda_smooth, p.lambda_prior, p.lambda_lm, p.eta_max, 0.f, 0.f, 0.f};
+  {
+    const float isg = (float)dev.inv_sigma, hk = (float)dev.huber_k;
+    dev.s_cap = isg * isg; dev.k_cap = hk * isg; dev.hk2 = hk * hk;
+  }
   // segment -> boundary pairs CSR (host), the sign of Delta folded in: d = eta_s - eta_other + delta'
   std::vector<int32_t> sp_ptr(n_total + 1, 0), sp_other(2 * (size_t)n_pairs), pairs(h_pairs, h_pairs + 2 * (size_t)n_pairs);
   std::vector<double> sp_delta(2 * (size_t)n_pairs), delta(h_delta, h_delta + n_pairs);
@@ -564,7 +580,7 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
     if (c->E > 0)
       k_depth_edge<<<c->E * tiles, kDpThreads, smem, c->stream>>>(pm_init, d_rec, d_labn, c->edges, c->grp_edge, d_labels, cur, c->poses, c->H, c->W,
                                                                  n_seg, tiles, tile_rows, dev, d_partial);
-    k_depth_cost<<<1, 256, 0, c->stream>>>(d_partial, c->E * tiles, rec, cur, n_total, d_pairs, d_delta, n_pairs, dev, d_cost + it);
+    k_depth_cost<<<1, kDpCostThreads, 0, c->stream>>>(d_partial, c->E * tiles, rec, cur, n_total, d_pairs, d_delta, n_pairs, dev, d_cost + it);
     k_depth_update<<<(n_total + 127) / 128, 128, 0, c->stream>>>(d_partial, cur, nxt, c->edges, c->kf_ptr, c->kf_edge, d_sp_ptr, d_sp_other,
                                                                  d_sp_delta, d_anchor, n_seg, n_total, tiles, dev);
     c->launches += 3;
