@@ -49,8 +49,7 @@ namespace sim3ba {
 
 namespace {
 
-constexpr int kDpWarps = 4;
-constexpr int kDpThreads = 32 * kDpWarps;
+constexpr int kDpMaxWarps = 4;      // warps per CTA: 4 up to 64 segments per keyframe, 2 above (the per-warp bins grow with n_seg: more CTAs fit an SM)
 constexpr int kDpMaxSeg = 512;       // labels per keyframe (the paper's SLIC pass: M_k ~ 200)
 constexpr int kDpRows = 4;           // rows of a warp item (pixels per lane)
 constexpr int kDpCols = 32;          // columns of a warp item (one per lane)
@@ -239,12 +238,13 @@ __device__ __forceinline__ void bin_records(double* bins, DpQueue& q, int base, 
   dp_drain(q, bins, false, lane);
 }
 
-__global__ void __launch_bounds__(kDpThreads)
+__global__ void __launch_bounds__(32 * kDpMaxWarps)
 k_depth_edge(const float4* __restrict__ pm, const float4* __restrict__ rec, const int32_t* __restrict__ lab_n,
              const int32_t* __restrict__ edges, const int32_t* __restrict__ grp_edge, const int32_t* __restrict__ labels,
              const double* __restrict__ eta, const double* __restrict__ poses, int H, int W, int n_seg, int tiles, int tile_rows,
              DepthDev prm, double* __restrict__ partial) {
   extern __shared__ __align__(16) unsigned char dp_smem[];
+  const int kDpWarps = blockDim.x >> 5, kDpThreads = blockDim.x;   // 4 or 2 warps (see the launcher)
   // [kDpWarps] rings + queues | [kDpWarps][2 sides][n_seg][2] FP64 bins | [kDpWarps] cost |
   // [n_seg] 8 floats: E_h (hi, lo), (1 - E_h) t_ij [3] (hi, lo) | [n_seg] float2 E_g (hi, lo)
   double* s_bins = reinterpret_cast<double*>(dp_smem + kDpWarpBytes * kDpWarps);
@@ -431,13 +431,11 @@ k_depth_edge(const float4* __restrict__ pm, const float4* __restrict__ rec, cons
   double* out = partial + ((size_t)e * tiles + tile) * (4 * n_seg + 1);
   for (int q = tid; q < 4 * n_seg; q += kDpThreads) {           // q = (side, label, {g, H})
     double v = 0.0;
-#pragma unroll
     for (int w = 0; w < kDpWarps; ++w) v += s_bins[(size_t)w * 4 * n_seg + q];
     out[q] = v;
   }
   if (tid == 0) {
     double v = 0.0;
-#pragma unroll
     for (int w = 0; w < kDpWarps; ++w) v += s_cost[w];
     out[4 * n_seg] = v;
   }
@@ -527,6 +525,7 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
   const int tile_rows = std::max(kDpRows, ((c->H + want_tiles - 1) / want_tiles + kDpRows - 1) / kDpRows * kDpRows);
   const int tiles = (c->H + tile_rows - 1) / tile_rows;
   const int rec = 4 * n_seg + 1;
+  const int kDpWarps = n_seg <= 64 ? kDpMaxWarps : 2, kDpThreads = 32 * kDpWarps;
   const size_t smem = kDpWarpBytes * kDpWarps + ((size_t)kDpWarps * 4 * n_seg + kDpWarps) * sizeof(double) + (size_t)n_seg * 40;
   if (smem > c->depth_smem) {
     cudaError_t ea = cudaFuncSetAttribute(k_depth_edge, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
