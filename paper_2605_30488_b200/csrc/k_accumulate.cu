@@ -35,7 +35,7 @@ constexpr int kStages = 2;                     // ring of gathered X_j pairs per
                                                // no stored 1/|X_i| (14.1 KB + 1 KB reserved per one-warp CTA) let 14 warps share the 228 KB
                                                // of an SM.  Measured on C2: 12 warps / 3 stages 177.6 us, 13 / 2 171.3, 14 / 2 165.8; 16 warps
                                                // with the index buffer refilled in halves 167.8 (not kept)
-constexpr float kCancel = 1.0f / 16384.0f;     // |x|^2 < kCancel |X_i|^2: x = X_i + del has lost 7 bits or more -> the match is deferred to FP64
+constexpr float kCancel = 1.0f / 1024.0f;      // |x|^2 < kCancel |X_i|^2: x = X_i + del has lost 5 bits or more -> the match is deferred to FP64
 constexpr int kSlots = 40;                     // reduction slots of a record (layout: sim3ba_internal.cuh)
 constexpr int kAccSlots = 37;                  // slots that carry floating-point sums
 
@@ -369,10 +369,10 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
         delta(XA1, P0.y, P0.w, P1.y, del0.y, del1.y, del2.y);
         f2 x0 = Xi0 + del0, x1 = Xi1 + del1, x2 = Xi2 + del2;   // x = T_ij X_j
         f2 d2 = fma2(x0, x0, fma2(x1, x1, x2 * x2));
-        // X_i + del carries 2^-24 |del|: where the sum cancels (a stray match mapped to within |X_i| / 128 of the camera
+        // X_i + del carries 2^-24 |del|: where the sum cancels (a stray match mapped to within |X_i| / 32 of the camera
         // centre; the 1 / |x|^2 terms of the Jacobian then dominate its edge's block) the match is DEFERRED: its pixel goes
         // into the record's bit mask, its lane sits out with zero weight, and k_deferred evaluates it in FP64.  About one match
-        // in 1e5; no branch here.
+        // in 1e4; no branch here.
         const bool dA = vA && d2.x < d2i.x * kCancel, dB = vB && d2.y < d2i.y * kCancel;
         defmask |= (dA ? 1u : 0u) << (2 * p) | (dB ? 2u : 0u) << (2 * p);   // bit 2p: match A of pair p, bit 2p + 1: match B
         f2 sq = make_float2(P1.z, P1.w) * make_float2(XA0.w, XA1.w);
