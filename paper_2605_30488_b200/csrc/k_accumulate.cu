@@ -17,8 +17,11 @@
 //
 // Precision plan: delta = T_ij X_j - X_i in FP64 (the one cancellation of the residual); everything
 // after it, the per-thread partial sums (<= 8 terms per lane, 16 per thread) and the first two levels of
-// the warp tree (<= 64 terms) in fp32; every sum from there upwards (warp, edge, adjoint congruence) in FP64.  No floating-point
-// atomics: the reduction order is fixed, results are run-to-run identical.
+// the warp tree (<= 64 terms) in fp32; every sum from there upwards (warp, edge, adjoint congruence) in FP64.  The rare
+// matches whose x = X_i + delta itself cancels (|x| < |X_i| / 32: a stray match mapped next to the camera centre) are
+// DEFERRED: kernel 1 leaves them out of its fp32 sums and marks them, k_deferred evaluates them in FP64 from the
+// definitions, k_finalize adds them to the edge.  No floating-point atomics: every reduction has a fixed order,
+// results are run-to-run identical.
 #include "f32x2.cuh"
 #include "sim3ba_internal.cuh"
 #include "sim3_math.cuh"

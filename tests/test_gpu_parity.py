@@ -330,6 +330,33 @@ def test_edge_cases_validity_confmin_multiple_gauges():
     ba.close()
 
 
+def test_matches_mapped_next_to_the_camera_centre():
+    """Matches whose transformed point x = T_ij X_j lands within |X_i| / 32 ... |X_i| / 1e5 of camera i's centre: X_i + delta
+    cancels there and the 1 / |x|^2 terms of the Jacobian make such a match dominate its edge's block.  The device defers them
+    to an FP64 evaluation (k_deferred); the blocks must still meet the 1e-4 bar -- and the match set stays bit-exact."""
+    g = make_config(1, height=40, width=60)
+    prm = oracle_params("paper")
+    rng = np.random.default_rng(5)
+    for e in range(0, g.n_edges, 2):
+        i, j = (int(v) for v in g.edges[e])
+        Ti, Tj = orc.pose_to_srt(g.poses_init[i]), orc.pose_to_srt(g.poses_init[j])
+        s, R, t = orc.sim3_mul(orc.sim3_inv(*Ti), Tj)                       # T_ij at the start poses
+        ms = rng.choice(np.flatnonzero(g.match[e] >= 0), size=12, replace=False)
+        for q, m in enumerate(ms):
+            n = int(g.match[e, m])
+            scale = np.linalg.norm(g.points[i, m]) * 10.0 ** (-1.6 - 0.3 * q)   # |x| = |X_i| / 40 ... / 8e4
+            x = scale * rng.normal(size=3) / np.sqrt(3.0)
+            g.points[j, n] = (R.T @ (x - t) / s).astype(np.float32)             # X_j = T_ij^-1 x
+    ba = make_solver(g, prm)
+    check_system(ba, g, g.poses_init, prm, "near-centre/paper")
+    # the same graph twice: the deferred path is part of the fixed reduction order
+    blk_a = ba.edge_blocks().cpu().numpy()
+    set_poses(ba, g.poses_init)
+    ba.build_system()
+    assert np.array_equal(blk_a, ba.edge_blocks().cpu().numpy())
+    ba.close()
+
+
 def test_create_rejects_bad_arguments():
     import torch
     from paper_2605_30488_b200 import Sim3BA, Sim3BAError, make_params
