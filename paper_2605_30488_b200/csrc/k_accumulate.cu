@@ -470,22 +470,23 @@ __device__ __forceinline__ void add_deferred_match(double* __restrict__ sum, con
   }
 }
 
-// The deferred matches of every edge: one warp per edge.  A lane visits the records lane, lane + 32, ... of the edge; a record
+// The deferred matches of every edge: one CTA of four warps per edge.  A thread visits the records tid, tid + 128, ... of the edge; a record
 // whose slot kSlotDef is non-zero names the lanes of kernel 1 that hold deferred matches; def_masks has their 16-bit masks (bit
-// 2p: pixel 64 p + lane of the record's 512-pixel slice, bit 2p + 1: pixel 64 p + 32 + lane).  Sums in FP64: per lane in record / lane / bit order, then a
-// butterfly over the lanes -- a fixed order.  def_sums [E][kSlots]: slots 0..36 as in a record.
-__global__ void __launch_bounds__(32)
+// 2p: pixel 64 p + lane of the record's 512-pixel slice, bit 2p + 1: pixel 64 p + 32 + lane).  Sums in FP64, in a fixed order.  def_sums [E][kSlots]: slots 0..36 as in a record.
+constexpr int kDefWarps = 4;
+__global__ void __launch_bounds__(32 * kDefWarps)
 k_deferred(const double* __restrict__ partials, const unsigned short* __restrict__ def_masks, const int32_t* __restrict__ def_flag, int records,
            const int32_t* __restrict__ edges, const float4* __restrict__ pm, const int32_t* __restrict__ match,
            const double* __restrict__ edgeT, int HW, RareParams rp, double* __restrict__ def_sums) {
-  const int e = blockIdx.x, lane = threadIdx.x;
+  __shared__ double s_w[kDefWarps][kSlots];
+  const int e = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (def_flag[e] == 0) return;                               // almost every edge: k_finalize does not read def_sums then
   const double* p = partials + (size_t)e * records * kPartialStride;
   double sum[kAccSlots];
 #pragma unroll
   for (int q = 0; q < kAccSlots; ++q) sum[q] = 0.0;
   const int i = edges[2 * e], j = edges[2 * e + 1];
-  for (int c = lane; c < records; c += 32) {
+  for (int c = tid; c < records; c += 32 * kDefWarps) {       // thread tid: records tid, tid + 128, ...
     const double* r = p + (size_t)c * kPartialStride;
     unsigned lanes = (unsigned)reinterpret_cast<const unsigned long long*>(r)[kSlotDef];
     while (lanes) {
@@ -502,6 +503,7 @@ k_deferred(const double* __restrict__ partials, const unsigned short* __restrict
       }
     }
   }
+  // per thread in record / lane / bit order, butterfly over the lanes, then the warps in order: a fixed order
 #pragma unroll
   for (int q = 0; q < kAccSlots; ++q) {
 #pragma unroll
@@ -509,7 +511,14 @@ k_deferred(const double* __restrict__ partials, const unsigned short* __restrict
   }
   if (lane == 0) {
 #pragma unroll
-    for (int q = 0; q < kAccSlots; ++q) def_sums[(size_t)e * kSlots + q] = sum[q];
+    for (int q = 0; q < kAccSlots; ++q) s_w[warp][q] = sum[q];
+  }
+  __syncthreads();
+  if (tid < kAccSlots) {
+    double v = 0.0;
+#pragma unroll
+    for (int w = 0; w < kDefWarps; ++w) v += s_w[w][tid];
+    def_sums[(size_t)e * kSlots + tid] = v;
   }
 }
 
@@ -637,7 +646,7 @@ cudaError_t launch_accumulate(Ctx* c) {
   if (c->profiling) cudaEventRecord(c->ev[1], c->stream);
   const int records = c->chunks * (kAccThreads / 32);
   const RareParams rp{(double)c->prm.sigma_ray, (double)c->prm.sigma_dist, (double)c->prm.huber_k};
-  k_deferred<<<c->E, 32, 0, c->stream>>>(c->partials, c->def_masks, c->def_flag, records, c->edges, c->pm, c->match, c->edgeT, c->HW, rp, c->def_sums);
+  k_deferred<<<c->E, 32 * kDefWarps, 0, c->stream>>>(c->partials, c->def_masks, c->def_flag, records, c->edges, c->pm, c->match, c->edgeT, c->HW, rp, c->def_sums);
   if (records >= 256 && c->E <= 600)
     k_finalize<24><<<c->E, 24 * 40 + 16, 0, c->stream>>>(c->partials, c->edges, c->poses, c->blocks35, c->edge_cost, c->n_valid,
                                                          c->checksum, records, c->def_sums, c->def_flag);
