@@ -56,6 +56,31 @@ def test_depth_refine_matches_oracle(preset, irregular, big):
     ba.close()
 
 
+def test_depth_refine_full_size_config2_paper_segment_count():
+    """BASELINE configs[1] at full size (32 keyframes 512x384, 96 edges, 1.9e7 candidate matches -- the tile / patch / ring
+    configuration the bench times) with ~200 irregular segments per keyframe, the paper's M_k: eta after two
+    iterations and the objective against the oracle."""
+    import torch
+    from sim3ba_inputs import make_config
+    g = make_config(2)
+    d = make_depth_inputs(g, irregular=200)
+    prm = oracle_params("config")
+    dprm = dp.DepthParams()
+    ba = make_solver(g, prm)
+    set_poses(ba, g.poses_init)
+    M = g.n_kf * d.n_seg
+    eta0 = np.random.default_rng(3).normal(0, 0.02, M)
+    for k in d.anchor_kf:
+        eta0[k * d.n_seg:(k + 1) * d.n_seg] = 0.0
+    eta = torch.from_numpy(eta0.copy()).cuda()
+    cost = ba.depth_refine(torch.from_numpy(d.labels).cuda(), d.n_seg, d.pairs, d.delta, d.anchor_kf, eta, 2)
+    ref, ref_cost = dp.depth_refine(g.poses_init, g.points, g.conf, g.edges, g.match, d.labels, d.n_seg, eta0, d.pairs, d.delta, d.anchor_kf,
+                                    dprm, 2)
+    assert rel(eta.cpu().numpy() - eta0, ref - eta0) <= 1e-6
+    assert rel(cost, ref_cost) <= 1e-7
+    ba.close()
+
+
 def scaled_points(g, d, eta):
     """X(eta) = exp(eta_g) X_init (Eq. (8)) as the fp32 pointmaps the next pose pass sees, in NumPy float64."""
     scale = np.ones((g.n_kf, g.hw))
