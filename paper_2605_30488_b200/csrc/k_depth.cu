@@ -207,34 +207,67 @@ __device__ __forceinline__ void dp_push(DpQueue& q, bool put, int bin, float a, 
   q.tail += __popc(bal);
 }
 
-// full phases while 32 records wait; `all`: also the remainder
-__device__ __forceinline__ void dp_drain(DpQueue& q, double* bins, bool all, int lane) {
-  while (q.tail - q.head >= 32 || (all && q.tail > q.head)) {
+// full phases while 32 records wait; `all`: also the remainder.  The loop is a function of its own (one copy of the phase
+// code instead of one per call site); the test in front of it is all that the common case executes.
+__device__ __noinline__ int dp_drain_loop(const int32_t* qbin, const float* qa, const float* qb, int head, int tail, double* bins, bool all, int lane) {
+  while (tail - head >= 32 || (all && tail > head)) {
     __syncwarp();                                                // the records were written by other lanes
-    const bool have = lane < q.tail - q.head;
-    const int pos = (q.head + lane) & (kDpQueue - 1);
-    bin_phase(bins, have ? q.bin[pos] : -1, have ? q.a[pos] : 0.f, have ? q.b[pos] : 0.f, lane);
-    q.head += min(32, q.tail - q.head);
+    const bool have = lane < tail - head;
+    const int pos = (head + lane) & (kDpQueue - 1);
+    bin_phase(bins, have ? qbin[pos] : -1, have ? qa[pos] : 0.f, have ? qb[pos] : 0.f, lane);
+    head += min(32, tail - head);
   }
+  return head;
+}
+__device__ __forceinline__ void dp_drain(DpQueue& q, double* bins, bool all, int lane) {
+  if (q.tail - q.head >= 32 || (all && q.tail > q.head)) q.head = dp_drain_loop(q.bin, q.a, q.b, q.head, q.tail, bins, all, lane);
 }
 
+// A lane walks DOWN one image column, so the segment of its pixels -- on both sides -- stays the same for many patches.  Per side
+// it keeps ONE running record in registers: the label K and the sums (g, H) as an unevaluated fp32 pair hi + lo (TwoSum: the
+// record is as accurate as one rounding of its exact sum, however long it runs).  Nothing is exchanged between lanes while
+// the label lasts; the record goes to the queue when the label changes, and at the end of the warp's work.
+struct DpRun {
+  int K;                 // -2: empty
+  f2 hi, lo;             // (g, H)
+};
+
 // The four records (key, a, b) of a lane -- its four vertically adjacent pixels -- of one side (`base` = first bin of the
-// side): those sharing the key of the lane's first valid pixel are merged and go through one phase; the others are queued.
-__device__ __forceinline__ void bin_records(double* bins, DpQueue& q, int base, const int (&key)[kDpRows], const float (&a)[kDpRows],
-                                            const float (&b)[kDpRows], int lane) {
-  const int K = key[0] >= 0 ? key[0] : key[1] >= 0 ? key[1] : key[2] >= 0 ? key[2] : key[3];
-  float sa = 0.f, sb = 0.f;
+// side): those of the running label (or, if none of the four carries it, of the lane's first valid pixel, which then
+// becomes the running label) are added to the running record; the others (stray matches, a boundary inside the patch) are
+// queued.  Every decision depends on the lane's own data only and the queue is filled in lane order: a fixed order.
+__device__ __forceinline__ void bin_records(double* bins, DpQueue& q, DpRun& run, int base, const int (&key)[kDpRows],
+                                            const float (&a)[kDpRows], const float (&b)[kDpRows], int lane) {
+  bool hit = false;
+#pragma unroll
+  for (int r = 0; r < kDpRows; ++r) hit |= key[r] == run.K;      // run.K is never -1: an invalid pixel does not hit
+  const int first = key[0] >= 0 ? key[0] : key[1] >= 0 ? key[1] : key[2] >= 0 ? key[2] : key[3];
+  const int K = hit ? run.K : first;
+  f2 s = make_float2(0.f, 0.f);
   bool extra[kDpRows];
 #pragma unroll
   for (int r = 0; r < kDpRows; ++r) {
     const bool same = key[r] == K;
-    sa += same ? a[r] : 0.f;
-    sb += same ? b[r] : 0.f;
+    s.x += same ? a[r] : 0.f;
+    s.y += same ? b[r] : 0.f;
     extra[r] = key[r] >= 0 && !same;
   }
-  bin_phase(bins, K >= 0 ? base + K : -1, sa, sb, lane);
+  const f2 out = run.hi + run.lo;
+  dp_push(q, !hit && K >= 0 && run.K >= 0, base + run.K, out.x, out.y, lane);     // the label has changed: the old record leaves
+  dp_drain(q, bins, false, lane);
+  if (hit) {                                                      // hi + lo += s, error-free (Knuth's TwoSum on both lanes)
+    const f2 t = run.hi + s;
+    const f2 bb = t + (-run.hi);
+    const f2 e = (run.hi + (-(t + (-bb)))) + (s + (-bb));
+    run.hi = t;
+    run.lo = run.lo + e;
+  } else if (K >= 0) {
+    run.K = K;
+    run.hi = s;
+    run.lo = make_float2(0.f, 0.f);
+  }
 #pragma unroll
-  for (int r = 1; r < kDpRows; ++r) dp_push(q, extra[r], base + key[r], a[r], b[r], lane);
+  for (int r = 0; r < kDpRows; ++r) dp_push(q, extra[r], base + key[r], a[r], b[r], lane);   // at most three per lane
   dp_drain(q, bins, false, lane);
 }
 
@@ -291,6 +324,9 @@ k_depth_edge(const float4* __restrict__ pm, const float4* __restrict__ rec, cons
   queue.a = reinterpret_cast<float*>(queue.bin + kDpQueue);
   queue.b = queue.a + kDpQueue;
   queue.head = queue.tail = 0;
+  DpRun run_g, run_h;                                            // running records of the lane's column, side i and side j
+  run_g.K = run_h.K = -2;
+  run_g.hi = run_g.lo = run_h.hi = run_h.lo = make_float2(0.f, 0.f);
 
   // the tile: image rows [row_lo, row_hi); its items: (block of 32 columns, quad of rows); the blocks are dealt round-robin to the warps
   const int row_lo = tile * tile_rows, row_hi = min(H, row_lo + tile_rows);
@@ -414,8 +450,8 @@ k_depth_edge(const float4* __restrict__ pm, const float4* __restrict__ rec, cons
         vg[p] = pvg.x; vg[p + 1] = pvg.y; Hg[p] = pHg.x; Hg[p + 1] = pHg.y;
         vh[p] = pvh.x; vh[p + 1] = pvh.y; Hh[p] = pHh.x; Hh[p + 1] = pHh.y;
       }
-      bin_records(my_bins, queue, 0, kg, vg, Hg, lane);
-      bin_records(my_bins, queue, n_seg, kh, vh, Hh, lane);
+      bin_records(my_bins, queue, run_g, 0, kg, vg, Hg, lane);
+      bin_records(my_bins, queue, run_h, n_seg, kh, vh, Hh, lane);
     }
     if ((t & 3) == 3) {                                          // fp32 partials of <= 48 terms -> FP64
       cost += (double)(c_wr2.x + c_wr2.y) - 0.5 * (double)(c_min.x + c_min.y);
@@ -423,7 +459,13 @@ k_depth_edge(const float4* __restrict__ pm, const float4* __restrict__ rec, cons
     }
   }
   dp_wait<0>();
-  dp_drain(queue, my_bins, true, lane);
+  {
+    const f2 og = run_g.hi + run_g.lo, oh = run_h.hi + run_h.lo;
+    dp_push(queue, run_g.K >= 0, run_g.K, og.x, og.y, lane);
+    dp_drain(queue, my_bins, false, lane);
+    dp_push(queue, run_h.K >= 0, n_seg + run_h.K, oh.x, oh.y, lane);
+    dp_drain(queue, my_bins, true, lane);
+  }
   cost += (double)(c_wr2.x + c_wr2.y) - 0.5 * (double)(c_min.x + c_min.y);
   cost = warp_sum(cost);
   if (lane == 0) s_cost[warp] = cost;
