@@ -41,6 +41,10 @@ constexpr int kStages = 2;                     // ring of gathered X_j pairs per
 constexpr float kCancel = 1.0f / 1024.0f;      // |x|^2 < kCancel |X_i|^2: x = X_i + del has lost 5 bits or more -> the match is deferred to FP64
 constexpr int kSlots = 40;                     // reduction slots of a record (layout: sim3ba_internal.cuh)
 constexpr int kAccSlots = 37;                  // slots that carry floating-point sums
+#ifndef SIM3BA_ACC_UNROLL
+#define SIM3BA_ACC_UNROLL 4
+#endif
+constexpr int kPairUnroll = SIM3BA_ACC_UNROLL;  // unrolling of the pair loop (8 pairs per edge and slice)
 
 // shared-memory carve-up of k_accumulate (dynamic); every array is sliced per warp
 // one contiguous region per warp, so that every shared-memory address of the pair loop is (warp base + lane * size) + constant
@@ -341,7 +345,7 @@ k_accumulate(const float4* __restrict__ pm, const int32_t* __restrict__ match, c
       d2_ = (float)fma(Td[6], Xjx, fma(Td[7], Xjy, fma(Td[8], Xjz, Td[11] - (double)xi2)));
     };
 
-#pragma unroll 4
+#pragma unroll kPairUnroll
     for (int p = 0; p < kPairs; ++p) {
       // issue the gathers of the pair kStages - 1 ahead (of this edge, or of the next edge) into the slot freed last iteration
       {
