@@ -256,7 +256,7 @@ int sim3ba_get_launch_count(sim3ba_ctx* ctx, int64_t* h_count);
 
 /* Device time in milliseconds of the phases of the last sim3ba_step / build / solve, measured
  * with CUDA events on the context's stream: [0] kernel 1 (per-match accumulate, a1-a5 partials),
- * [1] kernel 2 (per-edge reduce + adjoint congruence, gradient, cost), [2] damped tile assembly (a6, first
+ * [1] kernel 2 (FP64 evaluation of the deferred matches, per-edge reduce + adjoint congruence, gradient, cost), [2] damped tile assembly (a6, first
  * attempt), [3] factor + triangular solves (a7, incl. re-assembly of later attempts), [4] retraction (a8),
  * [5..7] reserved (0).  Synchronises.  Only recorded after sim3ba_set_profiling(ctx, 1). */
 int sim3ba_set_profiling(sim3ba_ctx* ctx, int32_t enable);
