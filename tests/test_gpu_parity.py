@@ -357,6 +357,35 @@ def test_matches_mapped_next_to_the_camera_centre():
     ba.close()
 
 
+def test_empty_graphs():
+    """No edges at all (every keyframe is then held only by eps_r: tau = 0, the poses do not move) and a graph that consists
+    of the gauge keyframe alone."""
+    import torch
+    from paper_2605_30488_b200 import Sim3BA
+    from tests.gpu_common import gpu_params
+    g = make_config(1, height=8, width=8)
+    prm = oracle_params("config")
+    dev = torch.device("cuda:0")
+    empty_e = torch.zeros((0, 2), dtype=torch.int32, device=dev)
+    empty_m = torch.zeros((0, g.hw), dtype=torch.int32, device=dev)
+    for n_kf in (g.n_kf, 1):
+        pts, cf = torch.from_numpy(g.points[:n_kf]).to(dev), torch.from_numpy(g.conf[:n_kf]).to(dev)
+        ba = Sim3BA(pts, cf, empty_e, empty_m, [0], gpu_params(prm), 8, 8)
+        p0 = torch.from_numpy(g.poses_init[:n_kf].copy()).to(dev)
+        ba.set_poses(p0)
+        ba.build_system()
+        ba.solve()
+        tau, attempts, eps, cost = ba.update()
+        ref = orc.solve(np.zeros((7 * n_kf, 7 * n_kf)), np.zeros(7 * n_kf), [0], prm)
+        assert attempts == ref.attempts == 1 and eps == prm.eps0 and cost == 0.0
+        assert np.all(tau.cpu().numpy() == 0.0) and np.all(ref.tau == 0.0)
+        ba.set_poses(p0)
+        ba.step()
+        assert np.array_equal(ba.get_poses().cpu().numpy(), g.poses_init[:n_kf])
+        assert ba.edge_stats()[0].numel() == 0
+        ba.close()
+
+
 def test_create_rejects_bad_arguments():
     import torch
     from paper_2605_30488_b200 import Sim3BA, Sim3BAError, make_params
