@@ -58,6 +58,13 @@ def test_create_validates_before_touching_the_device(lib):
     bad = make_params(huber_k=-1.0)
     assert lib.sim3ba_create(C.byref(out), 2, 4, 4, 1, one, one, one, one, fixed, 1, C.byref(bad), None) == -1
     assert b"param" in lib.sim3ba_last_error(None)
+    # maximum sizes: more than 2^28 pixels per keyframe (the per-slice index sums are 32-bit), more than 2^20 unknowns
+    assert lib.sim3ba_create(C.byref(out), 2, 1 << 15, (1 << 13) + 1, 1, one, one, one, one, fixed, 1, C.byref(prm), None) == -1
+    assert lib.sim3ba_create(C.byref(out), (1 << 20) // 7 + 1, 4, 4, 1, one, one, one, one, fixed, 1, C.byref(prm), None) == -1
+    assert b"oversized" in lib.sim3ba_last_error(None)
+    # the host jobs check their arguments the same way
+    assert lib.sim3ba_optimize_host(2, 4, 4, 1, None, one, one, one, fixed, 1, C.byref(prm), one, 1, one, None, None) == -1
+    assert lib.sim3ba_probe_fp64(None, None, None) == -1
 
 
 def test_product_path_fails_loudly_without_gpu(lib):
