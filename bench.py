@@ -141,10 +141,14 @@ def barrier():
 
 # ------------------------------------------------------------------------------------------------
 def workload_description(g, cfg_id):
+    from sim3ba_inputs import config_params
     s = g.spec
     name = f"BASELINE configs[{cfg_id - 1}] {s.name}" if cfg_id else s.name
+    lam = config_params(cfg_id).get("lm_lambda", 0.0)
     return {"workload": f"{name}: {g.n_kf} keyframes {s.width}x{s.height}, "
-                        f"{g.n_edges} edges, {int(s.p_out * 100)}% outlier matches, preset sigma=1 kappa=0.05",
+                        f"{g.n_edges} edges, {int(s.p_out * 100)}% outlier matches, preset sigma=1 kappa=0.05"
+                        + (f", lambda={lam:g} (Eq. 7 damping: the undamped step leaves the basin on this chain, DESIGN.md section 11)" if lam else ""),
+            "lm_lambda": lam,
             "n_kf": g.n_kf, "hw": g.hw, "n_edges": g.n_edges, "system_n": 7 * g.n_kf,
             "candidates_per_step": int(g.n_edges) * int(g.hw), "gn_iters_per_pose_reset": s.n_iters}
 
@@ -172,12 +176,12 @@ def pin_in_place(a):
 class Workload:
     """A graph resident on the device behind a libsim3ba context, with its seeded start."""
 
-    def __init__(self, g, dev, pinned: bool):
+    def __init__(self, g, dev, pinned: bool, cfg_id: int = 0):
         import torch
-        from sim3ba_inputs import PRESETS
+        from sim3ba_inputs import config_params
         from paper_2605_30488_b200 import Sim3BA, make_params
         self.g, self.dev = g, dev
-        self.preset = PRESETS["config"]
+        self.preset = config_params(cfg_id)          # the preset + what this config adds (C5: lm_lambda)
         mk = pin_in_place if pinned else torch.from_numpy
         self.h_pts, self.h_cf, self.h_ed, self.h_mt = mk(g.points), mk(g.conf), torch.from_numpy(g.edges), mk(g.match)
         torch.cuda.synchronize()
@@ -277,7 +281,7 @@ def rooflines(w: Workload, cfg_id, ph, ms_per_step, hbm_peak, peak_src, n_sms, s
 
 def per_config_entry(cfg_id, g, dev, flush, steps, hbm_peak, peak_src, n_sms, sm_max_mhz, fp64_peaks):
     import torch
-    w = Workload(g, dev, pinned=False)
+    w = Workload(g, dev, pinned=False, cfg_id=cfg_id)
     w.steps(3, flush, timed=False)
     ms = w.steps(steps, flush) / steps
     ph, sp = w.phases(min(steps, 10), flush)
@@ -330,10 +334,10 @@ def run_ours(args):
     # gigabytes of page-locked memory makes the kernel copy those pages for every child.
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        from sim3ba_inputs import PRESETS
-        cpu = cpu_baseline(g, PRESETS["config"], budget_s=8.0)
+        from sim3ba_inputs import config_params
+        cpu = cpu_baseline(g, config_params(args.config), budget_s=8.0)
     # inputs start in pinned host memory; the graph upload is the one-off part of the end-to-end job
-    w = Workload(g, dev, pinned=True)
+    w = Workload(g, dev, pinned=True, cfg_id=args.config)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
     sampler = ClockSampler(local)
@@ -594,9 +598,9 @@ def run_reference(args):
     if rank != 0:
         return
     from oracle.edge_pool import host_cores
-    from sim3ba_inputs import PRESETS, make_config
+    from sim3ba_inputs import config_params, make_config
     g = make_config(args.config)
-    preset = PRESETS["config"]
+    preset = config_params(args.config)
     cores = host_cores()
     # bounded sample per step so that the whole --steps K --warmup W run ends within a couple of minutes
     per_step_s = min(3.0, max(0.25, 60.0 / max(1, args.steps + args.warmup)))

@@ -32,13 +32,22 @@ static_assert(kBand == 3, "the trailing update of the border blocks is written o
 
 // phase time stamps of the persistent kernel (only with sim3ba_set_profiling: a.stamps is NULL otherwise), read back by
 // sim3ba_get_solve_phase_us: [0] start, [1] assembled, [2] segments eliminated, [3] barrier passed, [4] Schur rows done,
-// [5] border system solved, [6] back-substitution done (stamps of the last attempt)
+// [5] border system solved, [6] back-substitution done by the LAST CTA (stamps of the last attempt; [0..5] are CTA 0's,
+// each taken behind a grid barrier or timing a phase that ends in one)
 #define BB_STAMP(i)                                                                  \
   do {                                                                               \
     if (a.stamps != nullptr && blockIdx.x == 0 && threadIdx.x == 0) {                \
       unsigned long long t_;                                                         \
       asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                         \
       a.stamps[i] = t_;                                                              \
+    }                                                                                \
+  } while (0)
+#define BB_STAMP_LAST(i)                                                             \
+  do {                                                                               \
+    if (a.stamps != nullptr && threadIdx.x == 0) {                                   \
+      unsigned long long t_;                                                         \
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                         \
+      atomicMax(a.stamps + (i), t_);                                                 \
     }                                                                                \
   } while (0)
 
@@ -583,7 +592,7 @@ k_solve_bb(BBArgs a) {
       for (int q = blockIdx.x * kSolveThreads + tid; q < 7 * a.n_bord; q += G * kSolveThreads)
         a.tau[7 * a.bord_kf[q / 7] + q % 7] = __ldcg(a.B.tau + q);
     }
-    BB_STAMP(6);
+    BB_STAMP_LAST(6);
     solved = true;
     break;
   }

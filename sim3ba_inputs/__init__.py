@@ -5,5 +5,5 @@ pixel-match maps shaped like the five workloads of BASELINE.json (DESIGN.md "Inp
 contains none of the method's arithmetic (no residual, Jacobian, normal equations, Sim(3) Exp/Log,
 solve) and imports neither ``oracle/`` nor the CUDA package.
 """
-from .graphs import (CONFIGS, DepthInputs, Graph, GraphSpec, PRESETS, clean_variant, make_config, make_depth_inputs,  # noqa: F401
-                     make_graph)
+from .graphs import (CONFIG_PARAMS, CONFIGS, DepthInputs, Graph, GraphSpec, PRESETS, clean_variant, config_params,  # noqa: F401
+                     make_config, make_depth_inputs, make_graph)

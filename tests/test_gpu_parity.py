@@ -13,7 +13,7 @@ import pytest
 
 from oracle import sim3_gn_oracle as orc
 from oracle.edge_pool import build_system_parallel
-from sim3ba_inputs import CONFIGS, make_config, make_graph
+from sim3ba_inputs import CONFIG_PARAMS, CONFIGS, make_config, make_graph
 from tests.gpu_common import (TOL_BLOCK, TOL_TAU, blocks35_from_oracle, free_idx, make_solver, oracle_params,
                               parity_log, rel, set_poses, start_poses, sym_from_lower)
 
@@ -419,7 +419,7 @@ def test_config2_full_size_all_edges():
     ba.close()
 
 
-@pytest.mark.parametrize("k,preset", [(3, "config"), (3, "paper"), (4, "config"), (4, "paper"), (5, "config")])
+@pytest.mark.parametrize("k,preset", [(3, "config"), (3, "paper"), (4, "config"), (4, "paper"), (5, "config"), (5, "bench")])
 def test_full_size_vs_oracle(k, preset):
     """BASELINE configs[2..4] at FULL size, in the launch configuration bench.py times (C3: 200 keyframes 512x384, 608
     edges; C4: 1000 keyframes 256x192, 3036 edges, n = 7000; C5: 2000 keyframes 512x384, 6003 edges, 1.18e9 candidate
@@ -428,9 +428,11 @@ def test_full_size_vs_oracle(k, preset):
     is where cond(H) ~ 1e8-1e10 amplifies the fp32 per-match arithmetic).  The unchanged NumPy
     oracle runs edge-parallel on the host cores (oracle/edge_pool.py).  C3 starts from the independent per-agent gauges
     brought together by the oracle's gauge synchronisation; the device's own sim3ba_gauge_sync on the same
-    raw start must land on the same poses."""
+    raw start must land on the same poses.  (5, "bench"): config 5 with the parameters bench.py runs it with
+    (sim3ba_inputs.config_params: the Eq. (7) damping lambda = 1e-4), followed by the five iterations of the config on the
+    device: one factorisation attempt each and a cost that falls every iteration -- undamped, this chain leaves the basin."""
     g = make_config(k)
-    prm = oracle_params(preset)
+    prm = oracle_params("config", **CONFIG_PARAMS.get(k, {})) if preset == "bench" else oracle_params(preset)
     ba = make_solver(g, prm)
     bk, ref = ba.bookkeeping(), orc.bookkeeping(g.n_kf, g.edges)
     for key in ref:
@@ -446,4 +448,15 @@ def test_full_size_vs_oracle(k, preset):
         assert np.allclose(dev[:, 3:7], sgn * p0[:, 3:7], rtol=0, atol=1e-9) and np.allclose(dev[:, 7], p0[:, 7], rtol=1e-9)
     check_system(ba, g, p0, prm, f"C{k}-full/{preset}/it0", pool=True)
     assert ba.bb_info()["valid"] == 1
+    if preset == "bench":
+        set_poses(ba, p0)
+        costs = []
+        for _ in range(g.spec.n_iters):
+            ba.build_system()
+            ba.solve()
+            _, attempts, _, cost = ba.update()
+            assert attempts == 1
+            costs.append(cost)
+            ba.retract()
+        assert all(b < a for a, b in zip(costs, costs[1:])), costs
     ba.close()

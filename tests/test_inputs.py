@@ -41,3 +41,12 @@ def test_reduced_config3_has_two_gauges():
     assert g.agent[g.edges[e, 0 if moving_is_i else 1]] == 1
     s_ratio = g.poses_init_raw[6:, 7] / g.poses_gt[6:, 7]
     assert 0.25 < s_ratio.mean() < 3.5
+
+
+def test_config_params_are_the_preset_plus_the_damping_of_config5():
+    from oracle import sim3_gn_oracle as orc
+    from sim3ba_inputs import PRESETS, config_params
+    for k in (1, 2, 3, 4):
+        assert config_params(k) == PRESETS["config"] and config_params(k, "paper") == PRESETS["paper"]
+    assert config_params(5) == dict(PRESETS["config"], lm_lambda=1e-4)
+    assert orc.Params(**config_params(5)).lm_lambda == 1e-4 and orc.Params(**config_params(2)).lm_lambda == 0.0
