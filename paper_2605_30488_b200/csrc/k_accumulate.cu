@@ -130,9 +130,10 @@ __device__ __forceinline__ void accumulate_pair(f2 (&acc)[kAccSlots], const f2 d
       const f2 t = kk[c] * make_float2(rcp(fabsf(ee[c].x)), rcp(fabsf(ee[c].y)));
       om[c] = make_float2(fminf(ss[c].x, t.x), fminf(ss[c].y, t.y));   // fminf(s, NaN) = s (masked lane, e = 0)
       f[c] = om[c] * ee[c];
-      acc[35] = fma2(f[c], ee[c], acc[35]);                            // sum w r^2
-      const f2 r2 = (ss[c] * ee[c]) * ee[c];
-      acc[36] = acc[36] + make_float2(fminf(r2.x, prm.huber_k2), fminf(r2.y, prm.huber_k2));   // sum min(r^2, k^2)
+      const f2 fe = f[c] * ee[c];
+      acc[35] = acc[35] + fe;                                          // sum w r^2
+      // sum min(r^2, k^2) with r^2 = s e^2: where the weight is not clamped fe IS r^2 (<= k^2); where it is, fe = k |r| >= k^2
+      acc[36] = acc[36] + make_float2(fminf(fe.x, prm.huber_k2), fminf(fe.y, prm.huber_k2));
     }
   }
   const f2 a = om[0], b = om[1], c = om[2], w3 = om[3];
