@@ -316,14 +316,21 @@ def _perturb(pose: np.ndarray, rng: np.random.Generator) -> np.ndarray:
     return _compose(d, pose)
 
 
-def make_graph(spec: GraphSpec) -> Graph:
+def make_graph(spec: GraphSpec, edges: Optional[np.ndarray] = None, valid_frac: float = 0.8) -> Graph:
+    """The graph of a spec.  ``edges`` ([E, 2] keyframe pairs) replaces the spec's own edge list by an arbitrary topology
+    (tests: hubs, duplicate and reversed pairs, isolated keyframes); those edges all get ``valid_frac``."""
     scene = _make_scene(spec)
     poses_gt = _make_gt_poses(spec)
     o = _scene_offsets(spec)
     N, HW = spec.n_kf, spec.hw
     points = np.empty((N, HW, 3), dtype=np.float32)
     conf = np.empty((N, HW), dtype=np.float32)
-    edges, kind, frac = _make_edges(spec)
+    if edges is None:
+        edges, kind, frac = _make_edges(spec)
+    else:
+        edges = np.ascontiguousarray(edges, dtype=np.int32).reshape(-1, 2)
+        assert edges.size == 0 or (edges.min() >= 0 and edges.max() < N)
+        kind, frac = np.zeros(edges.shape[0], dtype=np.int8), np.full(edges.shape[0], float(valid_frac))
     E = edges.shape[0]
     match = np.empty((E, HW), dtype=np.int32)
 

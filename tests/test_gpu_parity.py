@@ -330,6 +330,44 @@ def test_edge_cases_validity_confmin_multiple_gauges():
     ba.close()
 
 
+@pytest.mark.parametrize("seed", range(48))
+def test_random_topologies_lockstep(seed):
+    """Arbitrary connected topologies instead of the configs' chains: 2..12 (a dozen seeds: 30..60) keyframes of 30x20 pixels (one full 512-pixel
+    slice and a ragged one), a random spanning tree plus random extra edges with duplicate and reversed pairs, every third
+    seed with a hub keyframe that half of the extra edges leave (many edges share one staged X_i slice), one or two gauge
+    keyframes anywhere, both presets, with and without the Eq. (7) damping, all three solver plans (the band + border plan
+    is valid for some of these graphs only; the library falls back to the tile plan by itself)."""
+    rng = np.random.default_rng(1000 + seed)
+    n_kf = int(rng.integers(2, 13)) if seed < 36 else int(rng.integers(30, 61))      # the last dozen: several 64-row tile columns
+    spec = CONFIGS[1].scaled(name=f"fuzz{seed}", seed=100 + seed, n_agents=1, kf_per_agent=n_kf, height=20, width=30, n_inter=0)
+    order = rng.permutation(n_kf)
+    edges = [(int(order[k]), int(order[rng.integers(0, k)])) for k in range(1, n_kf)]            # spanning tree
+    hub = int(rng.integers(0, n_kf)) if seed % 3 == 0 else -1
+    for _ in range(int(rng.integers(0, 2 * n_kf))):
+        i = hub if (hub >= 0 and rng.random() < 0.5) else int(rng.integers(0, n_kf))
+        j = int(rng.integers(0, n_kf - 1))
+        j += j >= i
+        edges.append((i, j))
+    if len(edges) > 1:
+        edges.append(edges[0])                               # the same pair twice
+        edges.append((edges[1][1], edges[1][0]))             # and one pair in both directions
+    edges = [edges[k] for k in rng.permutation(len(edges))]
+    g = make_graph(spec, edges=np.asarray(edges, dtype=np.int32), valid_frac=float(rng.uniform(0.3, 0.95)))
+    fixed = sorted(set(int(k) for k in rng.choice(n_kf, size=min(n_kf - 1, int(rng.integers(1, 3))), replace=False)))
+    g.fixed_kf = np.asarray(fixed, dtype=np.int32)
+    prm = oracle_params(["config", "paper"][seed % 2], lm_lambda=[0.0, 1e-3][(seed // 2) % 2])
+    ba = make_solver(g, prm)
+    bk, ref = ba.bookkeeping(), orc.bookkeeping(g.n_kf, g.edges)
+    for key in ref:
+        assert np.array_equal(bk[key], ref[key]), key
+    ba.set_solver_mode([2, 0, 1][seed % 3])
+    poses = g.poses_init
+    for it in range(2):
+        _, sol = check_system(ba, g, poses, prm, f"fuzz{seed}/it{it}")
+        poses = orc.retract(poses, sol.tau)
+    ba.close()
+
+
 def test_matches_mapped_next_to_the_camera_centre():
     """Matches whose transformed point x = T_ij X_j lands within |X_i| / 32 ... |X_i| / 1e5 of camera i's centre: X_i + delta
     cancels there and the 1 / |x|^2 terms of the Jacobian make such a match dominate its edge's block.  The device defers them
