@@ -370,11 +370,9 @@ __device__ void bb_schur_row(const BBArgs& a, double* buf, int b) {
 // the update: thread 0 alone produces d_{p+1} and 1 / d_{p+1} (its Newton chain) while warps 2..7 apply pivot p to the
 // rest of the trailing matrix and warp 1 takes column p of the forward solve.  1 / d = 0 marks a pivot that is <= 0 or not finite.
 __device__ __forceinline__ double fast_rcp(double p) {
-  const float pf = (float)p;
-  if (!(pf > 1e-30f && pf < 1e30f)) return 1.0 / p;
-  float rf;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rf) : "f"(pf));
-  double y = (double)rf;
+  if (!(p > 1e-30 && p < 1e30)) return 1.0 / p;
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(p));    // MUFU.RCP64H: ~2^-22, then two Newton steps
   double e = fma(-p, y, 1.0);
   y = fma(y, e, y);
   e = fma(-p, y, 1.0);

@@ -65,14 +65,13 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// 1 / sqrt(p) to full double precision from the fp32 MUFU estimate and two Newton steps (relative error 2e-7 -> 6e-14
-// -> 5e-27 before rounding); pivots outside the comfortable fp32 range take the library routine
+// 1 / sqrt(p) to full double precision from the FP64 MUFU estimate (rsqrt.approx.ftz.f64 = MUFU.RSQ64H on the high word:
+// relative error ~2^-22, no conversion to fp32 and back on the pivot chain) and two Newton steps (2e-7 -> 6e-14 -> 5e-27
+// before rounding); pivots outside a comfortable range take the library routine
 __device__ __forceinline__ double fast_rsqrt(double p) {
-  const float pf = (float)p;
-  if (!(pf > 1e-30f && pf < 1e30f)) return rsqrt(p);
-  float rf;
-  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rf) : "f"(pf));
-  double y = (double)rf;
+  if (!(p > 1e-30 && p < 1e30)) return rsqrt(p);
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(p));
   const double h = 0.5 * p;
   y = y * fma(-h * y, y, 1.5);
   y = y * fma(-h * y, y, 1.5);
