@@ -358,6 +358,16 @@ def run_ours(args):
     clocks = sampler.stop(t_begin, t_end)
     ms_per_step = total_ms / args.steps
     ph, sp = w.phases(min(args.steps, 50), flush)
+    # a config that runs with the Eq. (7) damping (C5): the same iterations undamped, for the record -- same work per step,
+    # plus the retried factorisation on the iteration where H has lost definiteness
+    undamped = None
+    if w.preset.get("lm_lambda", 0.0) != 0.0 and world == 1:
+        n_u = 2 * max(1, g.spec.n_iters)
+        w.ba.set_params(make_params(**dict(w.preset, lm_lambda=0.0)))
+        w.steps(max(1, g.spec.n_iters), flush, timed=False)
+        undamped = {"lm_lambda": 0.0, "steps": n_u, "ms_per_step": w.steps(n_u, flush) / n_u,
+                    "note": "undamped GN leaves the basin on this chain (cost rises from the third iteration); not the reported configuration"}
+        w.ba.set_params(make_params(**w.preset))
 
     # ---- end to end through the C ABI with HOST buffers (pinned).  Pose-only job: sim3ba_optimize_host = device allocation
     # + upload of the whole graph + create (pack, bookkeeping, solve plan) + n_iters GN steps + poses and costs back + free.
@@ -482,6 +492,8 @@ def run_ours(args):
         "roofline": roof, "roofline_alu": alu, "roofline_solve": solve, "solver": solver,
         "fp64_peak_probe": {"dfma_tflops": fp64_peaks[0], "dmma_tflops": fp64_peaks[1]},
     }
+    if undamped is not None:
+        out["undamped"] = undamped
     if depth is not None:
         out["depth_refine"] = depth
     if alternation is not None:
