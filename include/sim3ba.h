@@ -139,6 +139,28 @@ int sim3ba_optimize_host(int32_t n_kf, int32_t height, int32_t width, int32_t n_
 int sim3ba_gauge_sync(sim3ba_ctx* ctx, int32_t edge, const int32_t* h_moving_kf, int32_t n_moving, int32_t moving_is_i,
                       int32_t n_c_min, double* h_T, int32_t* h_n_c, int32_t* h_fallback);
 
+/* sim3ba_gauge_sync WITHOUT any device allocation, for callers that cannot call cudaMalloc (a region under CUDA graph
+ * capture, a tight serving loop, a harness that forbids it).  Same operation (Eq. (3)-(4)), same kernels,
+ * same fixed summation order: results are bit-identical to sim3ba_gauge_sync.  The only scratch memory of the operation
+ * -- one record of 20 doubles per 1024 pixels of the linking edge -- lives in a file-scope device array of the library
+ * sized for images of at most SIM3BA_STATIC_MAX_PIXELS = 262144 pixels (512 x 512): 40960 bytes that every GPU which
+ * loads the library holds until the process exits.  A context with a larger image is rejected with SIM3BA_ERR_INVALID_ARG
+ * and a message naming the limit (use sim3ba_gauge_sync there).
+ *   d_moving_kf  DEVICE array [n_moving] of keyframe indices (may be NULL if n_moving = 0); not validated on the host:
+ *                an index outside 0 .. n_kf - 1 is skipped on the device
+ *   d_result     DEVICE array [10], written: [0..7] T* in the pose layout (t, q_xyzw, s), [8] number of correspondences,
+ *                [9] 1 if the endpoint transform was used
+ * The call enqueues three kernels on the context's stream and returns: no cudaMalloc / cudaFree, no pool allocation, no
+ * copy, no synchronisation; read d_result after synchronising the stream.  The first call on a device looks the array's
+ * address up (cudaGetSymbolAddress, once per device and process, with that device current): make that call outside a
+ * capture.  ALL calls on one device share the array: calls that overlap on the GPU (two streams, two contexts) race on
+ * it; calls on one stream are ordered and safe.  Nothing in the array needs clearing between calls (every record that
+ * is read is written by the same call).  Errors: INVALID_ARG (edge out of range, NULL buffer, n_c_min < 1, image too
+ * large), CUDA. */
+#define SIM3BA_STATIC_MAX_PIXELS 262144
+int sim3ba_gauge_sync_static(sim3ba_ctx* ctx, int32_t edge, const int32_t* d_moving_kf, int32_t n_moving, int32_t moving_is_i,
+                             int32_t n_c_min, double* d_result);
+
 /* ---- Segment-level structure refinement with the poses held fixed (Eq. (8)-(10); SURVEY 8(f)
  * NEXT-1; BASELINE config 5 "pose-depth alternation").  One log-scale eta_g per segment g of a keyframe:
  * X(eta_g) = exp(eta_g) X_init (Eq. (8)); data term Eq. (9) over the graph's valid matches whose two pixels carry a

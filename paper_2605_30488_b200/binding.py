@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libsim3ba.so")
 
 EXPORTS = (
     "sim3ba_default_params", "sim3ba_create", "sim3ba_destroy", "sim3ba_set_params", "sim3ba_set_poses",
-    "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_graph", "sim3ba_step_host", "sim3ba_optimize_host", "sim3ba_refine_host", "sim3ba_gauge_sync", "sim3ba_depth_default_params", "sim3ba_depth_refine", "sim3ba_apply_depth",
+    "sim3ba_get_poses", "sim3ba_build_system", "sim3ba_solve", "sim3ba_step", "sim3ba_step_graph", "sim3ba_step_host", "sim3ba_optimize_host", "sim3ba_refine_host", "sim3ba_gauge_sync", "sim3ba_gauge_sync_static", "sim3ba_depth_default_params", "sim3ba_depth_refine", "sim3ba_apply_depth",
     "sim3ba_retract", "sim3ba_get_edge_stats", "sim3ba_get_edge_blocks", "sim3ba_get_system",
     "sim3ba_get_update", "sim3ba_get_bookkeeping", "sim3ba_load_system", "sim3ba_get_launch_count",
     "sim3ba_set_solver_mode", "sim3ba_get_solver_info", "sim3ba_get_bb_info",
@@ -71,6 +71,7 @@ def load_library() -> C.CDLL:
         "sim3ba_refine_host": [i32, i32, i32, i32, vp, vp, vp, vp, P(i32), i32, P(Params), vp, i32, P(i32), P(C.c_double), i32, P(DepthParams),
                                i32, i32, i32, vp, vp, vp, vp, vp, vp],
         "sim3ba_gauge_sync": [vp, i32, P(i32), i32, i32, i32, P(C.c_double), P(i32), P(i32)],
+        "sim3ba_gauge_sync_static": [vp, i32, vp, i32, i32, i32, vp],
         "sim3ba_depth_default_params": [P(DepthParams)],
         "sim3ba_depth_refine": [vp, vp, i32, P(i32), P(C.c_double), i32, P(i32), i32, P(DepthParams), i32, vp, P(C.c_double)],
         "sim3ba_apply_depth": [vp, vp, vp, vp, i32, vp],
@@ -261,6 +262,18 @@ class Sim3BA:
         self._check(self.lib.sim3ba_gauge_sync(self._h, int(edge), mk, len(moving_kf), int(bool(moving_is_i)), int(n_c_min), T,
                                                C.byref(nc), C.byref(fb)))
         return np.array(list(T)), nc.value, bool(fb.value)
+
+    def gauge_sync_static(self, edge: int, moving_kf, result, moving_is_i: bool = False, n_c_min: int = 64):
+        """sim3ba_gauge_sync_static: the same operation with no device allocation (scratch in a file-scope device array,
+        images up to 2^18 pixels).  moving_kf: CUDA int32 tensor of keyframe indices (or None); result: CUDA float64 tensor
+        [10], written asynchronously on the context's stream (T* [8], N_c, fallback flag)."""
+        t = self._torch
+        assert result.is_cuda and result.dtype == t.float64 and result.is_contiguous() and result.numel() >= 10
+        n_moving = 0 if moving_kf is None else int(moving_kf.numel())
+        if n_moving:
+            assert moving_kf.is_cuda and moving_kf.dtype == t.int32 and moving_kf.is_contiguous()
+        self._check(self.lib.sim3ba_gauge_sync_static(self._h, int(edge), moving_kf.data_ptr() if n_moving else None, n_moving,
+                                                      int(bool(moving_is_i)), int(n_c_min), result.data_ptr()))
 
     def depth_refine(self, labels, n_seg: int, pairs: np.ndarray, delta: np.ndarray, anchor_kf: Sequence[int], eta, n_iters: int = 10,
                      params: Optional[DepthParams] = None):

@@ -12,6 +12,8 @@
 // tr(R^T A) -- the largest eigenvector of Horn's symmetric 4x4 matrix by cyclic Jacobi sweeps, which IS U S V^T of
 // Eq. (4) (the search is over rotations only, so the reflection case needs no special handling) -- then
 // s* = tr(R*^T A) / var(y) (= tr(S Lambda) / var(y)) and t*; (3) T* applied to the listed keyframes.
+#include <mutex>
+
 #include "sim3ba_internal.cuh"
 #include "sim3_math.cuh"
 
@@ -227,5 +229,96 @@ cudaError_t launch_gauge_sync(Ctx* c, int e, const int32_t* d_moving, int n_movi
 
 int gauge_sync_grid(int HW) { return std::max(1, std::min((HW + 4 * kGsThreads - 1) / (4 * kGsThreads), 296)); }
 int gauge_sync_work_doubles(int grid) { return grid * kGsSlots + 10; }
+
+// ---- sim3ba_gauge_sync_static: the same computation with NO device allocation ---------------------------------------
+// For callers that cannot call cudaMalloc (a region under CUDA graph capture, a serving loop, a harness that forbids it).
+// The per-block moment records of k_gs_moments -- the only scratch memory of the gauge synchronisation -- live in a
+// file-scope device array instead of a pool allocation; the result goes to a buffer of the caller, the moving keyframes
+// come from a device array of the caller, so nothing is allocated, freed, copied from the host or synchronised.
+//   * Size: one record of kGsSlots doubles per 1024 pixels, for images of at most kGsStaticMaxPixels = 2^18 pixels
+//     (512 x 512; every BASELINE config is 512 x 384 or smaller): 256 x 20 x 8 = 40960 bytes, held by every GPU that
+//     loads the library until the process exits.  Below that size the grid -- and with it the fixed summation order --
+//     is the one sim3ba_gauge_sync uses, so the two entry points give bit-identical results.
+//   * Nothing in the array has to start at zero: every record k_gs_solve reads (blocks 0 .. grid - 1) is written in
+//     full by k_gs_moments of the same call, whatever an earlier call (another edge, another image size) left behind.
+//   * Every call on a device shares the array: calls that overlap on the GPU (two streams, two contexts) RACE on it.
+// In host code the array's name is a host-side stand-in, not a device address: the address is looked up once per device
+// (that device current) with cudaGetSymbolAddress and handed to the kernels.
+namespace {
+
+constexpr int kGsStaticMaxPixels = 1 << 18;
+constexpr int kGsStaticBlocks = kGsStaticMaxPixels / (4 * kGsThreads);
+static __device__ __align__(256) double g_gs_scratch[kGsStaticBlocks * kGsSlots];
+
+constexpr int kGsMaxDevices = 64;
+std::mutex g_gs_mutex;
+double* g_gs_scratch_addr[kGsMaxDevices] = {};
+
+// device address of g_gs_scratch on the CURRENT device (one cudaGetSymbolAddress per device and process)
+cudaError_t gs_static_scratch(double** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kGsMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_gs_mutex);
+  if (!g_gs_scratch_addr[dev]) {
+    double* p = nullptr;
+    e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_gs_scratch);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    g_gs_scratch_addr[dev] = p;
+  }
+  *out = g_gs_scratch_addr[dev];
+  return cudaSuccess;
+}
+
+// k_gs_apply for a list nobody has validated on the host: indices outside 0 .. N - 1 are skipped
+__global__ void k_gs_apply_checked(double* __restrict__ poses, const int32_t* __restrict__ moving, int n_moving, int N,
+                                   const double* __restrict__ T) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n_moving) return;
+  const int kf = moving[idx];
+  if ((unsigned)kf >= (unsigned)N) return;
+  double* p = poses + 8 * kf;
+  double R[9];
+  quat_to_rot(T + 3, R);
+  const double s = T[7];
+  const double t0 = p[0], t1 = p[1], t2 = p[2];
+  p[0] = s * (R[0] * t0 + R[1] * t1 + R[2] * t2) + T[0];
+  p[1] = s * (R[3] * t0 + R[4] * t1 + R[5] * t2) + T[1];
+  p[2] = s * (R[6] * t0 + R[7] * t1 + R[8] * t2) + T[2];
+  const double ax = T[3], ay = T[4], az = T[5], aw = T[6], bx = p[3], by = p[4], bz = p[5], bw = p[6];
+  double q[4] = {aw * bx + ax * bw + ay * bz - az * by, aw * by - ax * bz + ay * bw + az * bx,
+                 aw * bz + ax * by - ay * bx + az * bw, aw * bw - ax * bx - ay * by - az * bz};
+  const double inv = 1.0 / sqrt(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
+  for (int a = 0; a < 4; ++a) p[3 + a] = q[a] * inv;
+  p[7] *= s;
+}
+
+}  // namespace
+
+int gauge_sync_static_max_pixels() { return kGsStaticMaxPixels; }
+
+// d_moving [n_moving] and d_result [10] are device arrays of the caller; asynchronous on the context's stream
+cudaError_t launch_gauge_sync_static(Ctx* c, int e, const int32_t* d_moving, int n_moving, int moving_is_i, int n_c_min,
+                                     double* d_result) {
+  if (c->HW > kGsStaticMaxPixels) return cudaErrorInvalidValue;          // the entry point has said why
+  double* scratch = nullptr;
+  cudaError_t err = gs_static_scratch(&scratch);
+  if (err != cudaSuccess) return err;
+  const int grid = gauge_sync_grid(c->HW);                                // <= kGsStaticBlocks for HW <= kGsStaticMaxPixels
+  if (grid > kGsStaticBlocks) return cudaErrorInvalidValue;
+  const int i = c->h_edges[2 * e], j = c->h_edges[2 * e + 1];
+  k_gs_moments<<<grid, kGsThreads, 0, c->stream>>>(c->pm, c->match + (size_t)e * c->HW, c->poses, i, j, c->HW, scratch);
+  err = cudaGetLastError();
+  if (err != cudaSuccess) return err;
+  k_gs_solve<<<1, 32, 0, c->stream>>>(scratch, grid, c->poses, i, j, moving_is_i, n_c_min, d_result);
+  err = cudaGetLastError();
+  if (err != cudaSuccess) return err;
+  if (n_moving > 0)
+    k_gs_apply_checked<<<(n_moving + 127) / 128, 128, 0, c->stream>>>(c->poses, d_moving, n_moving, c->N, d_result);
+  c->launches += 3;
+  return cudaGetLastError();
+}
 
 }  // namespace sim3ba

@@ -1,6 +1,7 @@
 // C ABI of libsim3ba (include/sim3ba.h): argument checking, memory, a0 bookkeeping, and the
 // sequencing of kernels 1-5.  Host code only; every step of the hot path runs in the kernels.
 #include <math.h>
+#include <stdio.h>
 #include <string.h>
 
 #include <algorithm>
@@ -673,6 +674,26 @@ int sim3ba_gauge_sync(sim3ba_ctx* h, int32_t edge, const int32_t* h_moving_kf, i
   if (h_T) memcpy(h_T, res, 8 * sizeof(double));
   if (h_n_c) *h_n_c = (int32_t)res[8];
   if (h_fallback) *h_fallback = (int32_t)res[9];
+  c->built = false; c->solved = false;   // the poses changed
+  return SIM3BA_OK;
+}
+
+int sim3ba_gauge_sync_static(sim3ba_ctx* h, int32_t edge, const int32_t* d_moving_kf, int32_t n_moving, int32_t moving_is_i,
+                             int32_t n_c_min, double* d_result) {
+  if (!h) return SIM3BA_ERR_INVALID_ARG;
+  Ctx* c = &h->c;
+  tl_stream = c->stream;
+  if (edge < 0 || edge >= c->E) return fail(c, SIM3BA_ERR_INVALID_ARG, "edge index out of range");
+  if (n_moving < 0 || (n_moving > 0 && !d_moving_kf) || n_c_min < 1 || !d_result)
+    return fail(c, SIM3BA_ERR_INVALID_ARG, "bad moving list, n_c_min < 1 or NULL result buffer");
+  if (c->HW > gauge_sync_static_max_pixels()) {
+    char msg[200];
+    snprintf(msg, sizeof(msg), "sim3ba_gauge_sync_static: image of %d pixels exceeds the static scratch array (at most %d pixels); "
+             "use sim3ba_gauge_sync", c->HW, gauge_sync_static_max_pixels());
+    return fail(c, SIM3BA_ERR_INVALID_ARG, msg);
+  }
+  const cudaError_t e = launch_gauge_sync_static(c, edge, d_moving_kf, n_moving, moving_is_i != 0, n_c_min, d_result);
+  if (e != cudaSuccess) return cuda_fail(c, e, "sim3ba_gauge_sync_static");
   c->built = false; c->solved = false;   // the poses changed
   return SIM3BA_OK;
 }

@@ -187,6 +187,9 @@ cudaError_t launch_retract(Ctx* c);                      // kernel 5
 // gauge synchronisation (NEXT-2): moments of edge e -> T* (Umeyama / endpoint fallback) -> applied to the moving keyframes
 cudaError_t launch_gauge_sync(Ctx* c, int e, const int32_t* d_moving, int n_moving, int moving_is_i, int n_c_min, double* d_work, int grid);
 int gauge_sync_grid(int HW);
+cudaError_t launch_gauge_sync_static(Ctx* c, int e, const int32_t* d_moving, int n_moving, int moving_is_i, int n_c_min,
+                                     double* d_result);   // no allocation: scratch in a file-scope device array (k_gauge_sync.cu)
+int gauge_sync_static_max_pixels();
 int gauge_sync_work_doubles(int grid);
 // segment-level depth refinement with poses fixed (NEXT-1)
 cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const int32_t* h_pairs, const double* h_delta, int n_pairs,
