@@ -147,7 +147,7 @@ def workload_description(g, cfg_id):
     lam = config_params(cfg_id).get("lm_lambda", 0.0)
     return {"workload": f"{name}: {g.n_kf} keyframes {s.width}x{s.height}, "
                         f"{g.n_edges} edges, {int(s.p_out * 100)}% outlier matches, preset sigma=1 kappa=0.05"
-                        + (f", lambda={lam:g} (Eq. 7 damping: the undamped step leaves the basin on this chain, DESIGN.md section 11)" if lam else ""),
+                        + (f", lambda={lam:g} (Eq. 7 damping: the undamped step leaves the basin on this chain, DESIGN.md section 5)" if lam else ""),
             "lm_lambda": lam,
             "n_kf": g.n_kf, "hw": g.hw, "n_edges": g.n_edges, "system_n": 7 * g.n_kf,
             "candidates_per_step": int(g.n_edges) * int(g.hw), "gn_iters_per_pose_reset": s.n_iters}
