@@ -369,17 +369,6 @@ __device__ void bb_schur_row(const BBArgs& a, double* buf, int b) {
 // pivot c), so there is no square root and no scaling pass.  One barrier per pivot, and the pivot chain is taken off
 // the update: thread 0 alone produces d_{p+1} and 1 / d_{p+1} (its Newton chain) while warps 2..7 apply pivot p to the
 // rest of the trailing matrix and warp 1 takes column p of the forward solve.  1 / d = 0 marks a pivot that is <= 0 or not finite.
-__device__ __forceinline__ double fast_rcp(double p) {
-  if (!(p > 1e-30 && p < 1e30)) return 1.0 / p;
-  double y;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(p));    // MUFU.RCP64H: ~2^-22, then two Newton steps
-  double e = fma(-p, y, 1.0);
-  y = fma(y, e, y);
-  e = fma(-p, y, 1.0);
-  y = fma(y, e, y);
-  return y;
-}
-
 __device__ void bb_small_border(const BBArgs& a, Smem& sm, int n7) {
   const int tid = threadIdx.x;
   const int nB = a.npadB;

@@ -65,47 +65,75 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// 1 / sqrt(p) to full double precision from the FP64 MUFU estimate (rsqrt.approx.ftz.f64 = MUFU.RSQ64H on the high word:
-// relative error ~2^-22, no conversion to fp32 and back on the pivot chain) and two Newton steps (2e-7 -> 6e-14 -> 5e-27
-// before rounding); pivots outside a comfortable range take the library routine
-__device__ __forceinline__ double fast_rsqrt(double p) {
-  if (!(p > 1e-30 && p < 1e30)) return rsqrt(p);
+// 1 / sqrt(p) and 1 / p to full double precision from the FP64 MUFU estimates (rsqrt / rcp.approx.ftz.f64 = MUFU.RSQ64H /
+// RCP64H on the high word, relative error e ~ 2^-22) and ONE third-order correction each: with e = 1 - p y0^2 the root is
+// y0 (1 + e / 2 + 3 e^2 / 8 + O(e^3)), with e = 1 - p r0 the reciprocal is r0 (1 + e + e^2 + O(e^3)) -- e^3 ~ 1e-20 is below
+// the rounding.  Dependent FP64 operations behind the MUFU: four for the root, three for the reciprocal (two Newton steps
+// are six and four; an FP64 operation that waits for its operand costs ~28 cycles here, and these sit on the pivot chains).
+// Pivots outside a comfortable range take the library routines.
+__device__ __forceinline__ double mufu_rsqrt(double p) {        // p inside (1e-30, 1e30)
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(p));
-  const double h = 0.5 * p;
-  y = y * fma(-h * y, y, 1.5);
-  y = y * fma(-h * y, y, 1.5);
-  return y;
+  const double e = fma(-(p * y), y, 1.0);
+  return fma(y * e, fma(e, 0.375, 0.5), y);
 }
+__device__ __forceinline__ double mufu_rcp(double p) {          // p inside (1e-30, 1e30)
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(p));
+  const double e = fma(-p, r, 1.0);
+  return fma(r * e, 1.0 + e, r);
+}
+__device__ __forceinline__ double fast_rsqrt(double p) { return (p > 1e-30 && p < 1e30) ? mufu_rsqrt(p) : rsqrt(p); }
+__device__ __forceinline__ double fast_rcp(double p) { return (p > 1e-30 && p < 1e30) ? mufu_rcp(p) : 1.0 / p; }
 
 // Cholesky of an N x N block (N <= 8, row stride ld) by one warp: lane r holds row r, pivots and columns travel by
-// shuffles, the column updates of a pivot run in parallel over the lanes.  Leaves L in the lower triangle (the strict upper
-// triangle is zeroed) and the reciprocal pivots in inv[]; returns false on a pivot that is <= 0 or not finite.
-template <int N>
-__device__ __forceinline__ bool potrf_warp(double* blk, int ld, double* inv, int lane) {
+// shuffles, the column updates of a pivot run in parallel over the lanes.  The chain from one pivot to the next is
+// broadcast -> 1 / pivot -> one FMA: the trailing entries take a_rp a_tp / d_p from the UNSCALED column (the products and
+// the shuffles do not wait for the reciprocal), and the scaling of the column by 1 / sqrt(d_p), which only the output
+// needs, happens beside it.  Leaves L in the lower triangle (the strict upper triangle is zeroed) and the reciprocal
+// pivots 1 / L_pp in inv[]; returns false on a pivot that is <= 0 or not finite.  kMufu: the MUFU-seeded root and
+// reciprocal, valid for pivots inside (1e-30, 1e30); a block with a pivot outside is redone with the library routines
+// (one warp-uniform branch per block, out of line, instead of a fallback inside every step of the chain).
+template <int N, bool kMufu>
+__device__ __forceinline__ int potrf_warp_impl(double* blk, int ld, double* inv, int lane) {
   double v[N];
 #pragma unroll
   for (int k = 0; k < N; ++k) v[k] = (lane < N) ? blk[lane * ld + k] : 0.0;
-  bool good = true;
+  bool good = true, in_range = true;
 #pragma unroll
   for (int p = 0; p < N; ++p) {
     const double piv = __shfl_sync(0xffffffffu, v[p], p);
     const bool gd = (piv > 0.0) && (piv < 1.0e300);           // false for NaN, <= 0, inf
     good = good && gd;
-    const double iv = gd ? fast_rsqrt(piv) : 1.0;
-    v[p] *= iv;
+    in_range = in_range && (piv > 1e-30) && (piv < 1e30);
+    const double ps = gd ? piv : 1.0;
+    const double rp = kMufu ? mufu_rcp(ps) : 1.0 / ps;
+    const double ap = v[p];                                    // a_rp of this lane's row, unscaled
 #pragma unroll
     for (int t = p + 1; t < N; ++t) {
-      const double lt = __shfl_sync(0xffffffffu, v[p], t);
-      v[t] = fma(-v[p], lt, v[t]);
+      const double at = __shfl_sync(0xffffffffu, ap, t);
+      v[t] = fma(-(ap * at), rp, v[t]);
     }
+    const double iv = kMufu ? mufu_rsqrt(ps) : rsqrt(ps);
+    v[p] = ap * iv;
     if (lane == 0) inv[p] = iv;
   }
+  if (kMufu && good && !in_range) return 2;                    // nothing has been written to blk yet
   if (lane < N) {
 #pragma unroll
     for (int k = 0; k < N; ++k) blk[lane * ld + k] = (k <= lane) ? v[k] : 0.0;
   }
-  return good;
+  return good ? 0 : 1;
+}
+template <int N>
+__device__ __noinline__ int potrf_warp_lib(double* blk, int ld, double* inv, int lane) {
+  return potrf_warp_impl<N, false>(blk, ld, inv, lane);
+}
+template <int N>
+__device__ __forceinline__ bool potrf_warp(double* blk, int ld, double* inv, int lane) {
+  int r = potrf_warp_impl<N, true>(blk, ld, inv, lane);
+  if (r == 2) r = potrf_warp_lib<N>(blk, ld, inv, lane);
+  return r == 0;
 }
 
 // ---- rank-8 update on the FP64 tensor pipe ----------------------------------------------------------
