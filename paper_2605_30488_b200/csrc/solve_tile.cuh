@@ -11,7 +11,10 @@ namespace sim3ba {
 namespace {
 
 constexpr int NB = kNB;          // 64
-constexpr int LDD = NB + 1;      // diagonal tile / TRSM tile in shared memory (odd stride: column walks are conflict-free)
+constexpr int LDD = NB + 4;      // diagonal tile / TRSM tile in shared memory.  LDD % 16 == 4: the DMMA fragment loads of the rank-8
+                                 // updates (address = (row block + lane / 4) * LDD + lane % 4) are conflict-free; the one-thread-per-row
+                                 // walks of the row solves take a 4-way conflict instead.  Measured (8 warps, one rank-8 task each):
+                                 // 390 cycles a task with the odd stride NB + 1, 200 with NB + 4
 constexpr int LDT = NB + 4;      // DMMA operand tiles (LDT % 16 == 4: fragment loads are conflict-free)
 constexpr int kSolveThreads = 256;
 
