@@ -19,6 +19,8 @@
 //   back     L^T tau = y block by block, last to first, over the row lists.
 // Grid-wide barriers are a monotonically increasing global counter (all CTAs are co-resident: the
 // kernel is launched with cudaLaunchCooperativeKernel, with no more CTAs than the widest phase needs).
+#include <stdlib.h>
+
 #include "solve_tile.cuh"
 
 namespace sim3ba {
@@ -116,7 +118,8 @@ cudaError_t launch_solve(Ctx* c) {
   const bool dense = c->dense_loaded || c->solver_mode == 1;
   SolvePlan& plan = dense ? c->plan_dense : c->plan_sparse;
   long long want = std::max<long long>({(long long)plan.max_upd, (long long)plan.max_col, (long long)plan.max_row, 1LL});
-  const int G = (int)std::min<long long>(want, (long long)num_sms * std::min(max_blocks_per_sm, 2));
+  int G = (int)std::min<long long>(want, (long long)num_sms * std::min(max_blocks_per_sm, 2));
+  if (const char* cap = getenv("SIM3BA_SOLVE_MAX_CTAS")) G = std::max(1, std::min(G, atoi(cap)));   // tests: several tiles / tasks per CTA
   SolveArgs a;
   AsmArgs& s = a.as;
   s.L = c->L; s.npad = c->npad; s.n = c->n; s.N = c->N; s.blocks35 = c->blocks35;

@@ -20,6 +20,8 @@
 // A pivot <= 0 or not finite anywhere fails the attempt; the retry re-assembles with eps * 100.
 #include <stdio.h>
 
+#include <stdlib.h>
+
 #include "solve_tile.cuh"
 
 namespace sim3ba {
@@ -633,7 +635,8 @@ cudaError_t launch_solve_bb(Ctx* c) {
   // one per segment / border keyframe / tile task
   long long want = std::max<long long>({(long long)P.n_seg, (long long)P.n_bord, (long long)D.max_upd, (long long)D.max_col,
                                         (long long)P.n_int, 1LL});
-  const int G = (int)std::min<long long>(want, (long long)num_sms * std::min(max_blocks_per_sm, 1));
+  int G = (int)std::min<long long>(want, (long long)num_sms * std::min(max_blocks_per_sm, 1));
+  if (const char* cap = getenv("SIM3BA_SOLVE_MAX_CTAS")) G = std::max(1, std::min(G, atoi(cap)));   // tests: several segments / tiles / tasks per CTA
   BBArgs a{};
   a.stamps = c->profiling ? c->solve_stamps : nullptr;
   a.blocks35 = c->blocks35; a.g = c->g; a.kf_ptr = c->kf_ptr; a.kf_edge = c->kf_edge; a.pair_ptr = c->pair_ptr; a.pair_edge = c->pair_edge;

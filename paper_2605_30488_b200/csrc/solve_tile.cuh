@@ -154,12 +154,17 @@ __device__ __forceinline__ void rank8_dmma(double* X, int ldx, const double* D, 
   cp[1] = v1;
 }
 
-// ---- Cholesky of the 64x64 tile in sm.D (lower triangle; the upper triangle is scratch) ---------
+// ---- Cholesky of the 64x64 tile in sm.D (lower triangle; the upper triangle is scratch), fused with the triangular
+// solve X L_kk^T = A of the tile in sm.A (rows 0 .. nrows - 1, nrows = 0 or NB; stride LDD) and of the right-hand-side
+// row NB of sm.A (if with_rhs) ---------
 // Returns false (uniformly) on a pivot that is <= 0 or not finite.  Only the first npan 8-column micro-panels are
-// factorised: the rows behind them are identity padding (pivot 1, nothing to eliminate).  Per micro-panel: the 8x8
-// diagonal block by one warp (lane = row, fp32-seeded Newton rsqrt), the rows below it by one thread each against that
-// block, the trailing matrix by rank-8 DMMA updates (lower block pairs spread over the warps).
-__device__ bool potrf64(Smem& sm, int tid, int npan) {
+// factorised: the rows behind them are identity padding (pivot 1, nothing to eliminate; X stays 0 in those columns).
+// Per micro-panel: the 8x8 diagonal block by one warp (lane = row), then every row under it -- of L_kk, of the tile and
+// the right-hand side -- against that block, one thread per row, then the trailing columns of all of them by rank-8
+// DMMA updates spread over the warps (the right-hand side by plain FMAs).  The rows of the tile ride along in the
+// phases the factorisation has anyway: a separate triangular solve after it would pay the sixteen block barriers and
+// the short task lists of the eight micro-panels a second time.
+__device__ bool panel64(Smem& sm, int nrows, bool with_rhs, int tid, int npan) {
   const int lane = tid & 31, warp = tid >> 5;
   if (tid == 0) sm.flag = 0;
   if (tid >= 8 * npan && tid < NB) sm.dinv[tid] = 1.0;
@@ -168,27 +173,45 @@ __device__ bool potrf64(Smem& sm, int tid, int npan) {
     const int c0 = 8 * pb;
     if (warp == 0 && !potrf_warp<8>(sm.D + c0 * LDD + c0, LDD, sm.dinv + c0, lane) && lane == 0) sm.flag = 1;
     __syncthreads();
-    const int below = NB - c0 - 8;                       // rows under the diagonal block
-    if (tid < below) {                                   // x L11^T = a, one row per thread
-      double* row = sm.D + (c0 + 8 + tid) * LDD + c0;
-      double x[8];
+    const int below = NB - c0 - 8;                       // rows of L_kk under the diagonal block
+    {                                                    // x L11^T = a, one row per thread: threads 0 .. below - 1 the rows of
+      double* row = nullptr;                             // L_kk, 64 .. 64 + nrows - 1 the tile, 128 the right-hand side
+      if (tid < below) row = sm.D + (c0 + 8 + tid) * LDD + c0;
+      else if (tid >= NB && tid < NB + nrows) row = sm.A + (tid - NB) * LDD + c0;
+      else if (tid == 2 * NB && with_rhs) row = sm.A + NB * LDD + c0;
+      if (row != nullptr) {
+        double x[8];
 #pragma unroll
-      for (int t = 0; t < 8; ++t) x[t] = row[t];
+        for (int t = 0; t < 8; ++t) x[t] = row[t];
 #pragma unroll
-      for (int s = 0; s < 8; ++s) {
+        for (int s = 0; s < 8; ++s) {
 #pragma unroll
-        for (int m = 0; m < s; ++m) x[s] = fma(-x[m], sm.D[(c0 + s) * LDD + c0 + m], x[s]);
-        x[s] *= sm.dinv[c0 + s];
+          for (int m = 0; m < s; ++m) x[s] = fma(-x[m], sm.D[(c0 + s) * LDD + c0 + m], x[s]);
+          x[s] *= sm.dinv[c0 + s];
+        }
+#pragma unroll
+        for (int t = 0; t < 8; ++t) row[t] = x[t];
       }
-#pragma unroll
-      for (int t = 0; t < 8; ++t) row[t] = x[t];
     }
     __syncthreads();
-    const int nb8 = below >> 3;                          // 8x8 blocks per side of the trailing matrix
-    for (int t = warp; t < nb8 * (nb8 + 1) / 2; t += kSolveThreads / 32) {
-      int bi = 0, rem = t;
-      while (rem > bi) { rem -= bi + 1; ++bi; }          // t -> (bi, bj = rem), bj <= bi
-      rank8_dmma(sm.D, LDD, sm.D, c0, c0 + 8 + 8 * bi, c0 + 8 + 8 * rem, lane);
+    const int nb8 = below >> 3;                          // 8-column blocks still to update (= blocks per side of the trailing matrix)
+    const int nd = nb8 * (nb8 + 1) / 2, na = (nrows >> 3) * nb8;
+    for (int t = warp; t < nd + na; t += kSolveThreads / 32) {
+      if (t < nd) {
+        int bi = 0, rem = t;
+        while (rem > bi) { rem -= bi + 1; ++bi; }        // t -> (bi, bj = rem), bj <= bi
+        rank8_dmma(sm.D, LDD, sm.D, c0, c0 + 8 + 8 * bi, c0 + 8 + 8 * rem, lane);
+      } else {
+        const int u = t - nd, r = u / nb8;
+        rank8_dmma(sm.A, LDD, sm.D, c0, 8 * r, c0 + 8 + 8 * (u - r * nb8), lane);
+      }
+    }
+    if (with_rhs && tid >= 192 && tid < 192 + 8 * nb8) {  // the right-hand-side row (warps 6, 7: last in the DMMA round-robin)
+      const int c = c0 + 8 + (tid - 192);
+      double acc = sm.A[NB * LDD + c];
+#pragma unroll
+      for (int s = 0; s < 8; ++s) acc = fma(-sm.A[NB * LDD + c0 + s], sm.D[c * LDD + c0 + s], acc);
+      sm.A[NB * LDD + c] = acc;
     }
     __syncthreads();
   }
@@ -234,6 +257,9 @@ __device__ void trsm64(Smem& sm, int nrows, bool with_rhs, int tid, int npan) {
 }
 
 // ---- phase A of block column k --------------------------------------------------------------------
+// Every CTA that owns a tile of the column (and CTA 0) factorises the diagonal tile for itself, its first tile riding
+// along (panel64); CTA 0 stores L_kk and y_k.  A CTA with more than one tile (more tile rows than CTAs) takes the others
+// by trsm64.
 __device__ void panel_phase(const SolveArgs& a, Smem& sm, int k, int G) {
   const int tid = threadIdx.x;
   const size_t ld = (size_t)a.npad;
@@ -244,9 +270,36 @@ __device__ void panel_phase(const SolveArgs& a, Smem& sm, int k, int G) {
     const int r = idx >> 6, cc = idx & 63;
     sm.D[r * LDD + cc] = __ldcg(Lkk + r * ld + cc);
   }
+  auto load_tile = [&](int t) -> double* {               // tile t of the column -> sm.A
+    const int i = a.col_rows[cbeg + t];
+    double* Aik = a.L + (size_t)i * NB * ld + (size_t)k * NB;
+    for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
+      const int r = idx >> 6, cc = idx & 63;
+      sm.A[r * LDD + cc] = __ldcg(Aik + r * ld + cc);
+    }
+    return Aik;
+  };
+  auto store_tile = [&](int t, double* Aik) {            // X back in place; b_i -= L_ik y_k: four threads per row, 16 columns each
+    const int i = a.col_rows[cbeg + t];
+    for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
+      const int r = idx >> 6, cc = idx & 63;
+      Aik[r * ld + cc] = sm.A[r * LDD + cc];
+    }
+    const int r = tid >> 2, g = tid & 3;
+    double dot = 0.0;
+#pragma unroll
+    for (int cc = 0; cc < 16; ++cc) dot = fma(sm.A[r * LDD + 16 * g + cc], sm.y[16 * g + cc], dot);
+    dot += __shfl_xor_sync(0xffffffffu, dot, 1);
+    dot += __shfl_xor_sync(0xffffffffu, dot, 2);
+    if (g == 0) a.rhs[i * NB + r] = __ldcg(a.rhs + i * NB + r) - dot;
+  };
+  int t = blockIdx.x;
+  const bool has_first = t < c;
+  double* Aik = has_first ? load_tile(t) : nullptr;
+  if (tid < NB) sm.A[NB * LDD + tid] = __ldcg(a.rhs + k * NB + tid);
   __syncthreads();
   const int npan = min(8, max(0, (a.n - k * NB + 7) / 8));   // micro-panels holding rows of the system (the rest is padding)
-  if (!potrf64(sm, tid, npan)) {
+  if (!panel64(sm, has_first ? NB : 0, true, tid, npan)) {
     if (blockIdx.x == 0 && tid == 0) a.status[0] = 1;
     return;
   }
@@ -257,49 +310,21 @@ __device__ void panel_phase(const SolveArgs& a, Smem& sm, int k, int G) {
     }
     if (tid < NB) a.Dinv[k * NB + tid] = sm.dinv[tid];
   }
-  bool have_y = false;
-  int t = blockIdx.x;
-  do {
-    const bool has_tile = t < c;
-    double* Aik = nullptr;
-    int i = 0;
-    if (has_tile) {
-      i = a.col_rows[cbeg + t];
-      Aik = a.L + (size_t)i * NB * ld + (size_t)k * NB;
-      for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
-        const int r = idx >> 6, cc = idx & 63;
-        sm.A[r * LDD + cc] = __ldcg(Aik + r * ld + cc);
-      }
-    }
-    if (!have_y && tid < NB) sm.A[NB * LDD + tid] = __ldcg(a.rhs + k * NB + tid);
+  if (tid < NB) {
+    const double yv = sm.A[NB * LDD + tid];
+    sm.y[tid] = yv;
+    if (blockIdx.x == 0) a.ysol[k * NB + tid] = yv;
+  }
+  __syncthreads();
+  if (has_first) store_tile(t, Aik);
+  for (t += G; t < c; t += G) {
     __syncthreads();
-    trsm64(sm, has_tile ? NB : 0, !have_y, tid, npan);
-    if (!have_y) {
-      if (tid < NB) {
-        const double yv = sm.A[NB * LDD + tid];
-        sm.y[tid] = yv;
-        if (blockIdx.x == 0) a.ysol[k * NB + tid] = yv;
-      }
-      have_y = true;
-      __syncthreads();
-    }
-    if (has_tile) {
-      for (int idx = tid; idx < NB * NB; idx += kSolveThreads) {
-        const int r = idx >> 6, cc = idx & 63;
-        Aik[r * ld + cc] = sm.A[r * LDD + cc];
-      }
-      // b_i -= L_ik y_k: four threads per row, 16 columns each
-      const int r = tid >> 2, g = tid & 3;
-      double dot = 0.0;
-#pragma unroll
-      for (int cc = 0; cc < 16; ++cc) dot = fma(sm.A[r * LDD + 16 * g + cc], sm.y[16 * g + cc], dot);
-      dot += __shfl_xor_sync(0xffffffffu, dot, 1);
-      dot += __shfl_xor_sync(0xffffffffu, dot, 2);
-      if (g == 0) a.rhs[i * NB + r] = __ldcg(a.rhs + i * NB + r) - dot;
-    }
+    Aik = load_tile(t);
     __syncthreads();
-    t += G;
-  } while (t < c);
+    trsm64(sm, NB, false, tid, npan);
+    store_tile(t, Aik);
+  }
+  __syncthreads();
 }
 
 // ---- phase B of block column k: C_ij -= L_ik L_jk^T on the FP64 tensor pipe --------------------

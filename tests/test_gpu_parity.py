@@ -263,11 +263,16 @@ def test_solver_modes_agree(k, monkeypatch):
     sol = orc.solve(sysm.H, sysm.g, g.fixed_kf, prm)
     tau_floor = 1e-6 * np.sqrt(sol.tau.size)
     taus = {}
-    for tag, mode, lmax in (("bb", 2, None), ("bb-short", 2, "5"), ("tile", 0, None), ("dense", 1, None)):
+    for tag, mode, lmax, max_ctas in (("bb", 2, None, None), ("bb-short", 2, "5", None), ("tile", 0, None, None), ("dense", 1, None, None),
+                                      ("bb-short-2ctas", 2, "5", "2"), ("tile-1cta", 0, None, "1"), ("dense-2ctas", 1, None, "2")):
         if lmax is None:
             monkeypatch.delenv("SIM3BA_BB_LMAX", raising=False)
         else:
             monkeypatch.setenv("SIM3BA_BB_LMAX", lmax)
+        if max_ctas is None:                              # a capped grid: several segments, tiles and update tasks per CTA
+            monkeypatch.delenv("SIM3BA_SOLVE_MAX_CTAS", raising=False)
+        else:
+            monkeypatch.setenv("SIM3BA_SOLVE_MAX_CTAS", max_ctas)
         ba = make_solver(g, prm)
         info = ba.bb_info()
         assert info["valid"] == 1 and info["n_interior"] + info["n_border"] == g.n_kf - len(g.fixed_kf)
@@ -284,8 +289,10 @@ def test_solver_modes_agree(k, monkeypatch):
         for kf in g.fixed_kf:
             assert np.all(taus[tag][7 * kf:7 * kf + 7] == 0.0)
         ba.close()
-    for tag in ("bb-short", "tile", "dense"):
+    for tag in taus:
         assert rel(taus[tag], taus["bb"], tau_floor) <= 1e-6, tag
+    for tag, same in (("bb-short-2ctas", "bb-short"), ("tile-1cta", "tile"), ("dense-2ctas", "dense")):
+        assert np.array_equal(taus[tag], taus[same]), tag          # the grid size does not change the order of any sum
 
 
 def test_band_border_zero_information_keyframe_and_all_attempts_fail():
