@@ -169,13 +169,42 @@ __device__ bool panel64(Smem& sm, int nrows, bool with_rhs, int tid, int npan) {
   if (tid == 0) sm.flag = 0;
   if (tid >= 8 * npan && tid < NB) sm.dinv[tid] = 1.0;
   __syncthreads();
+  const int nra = nrows >> 3;
+  // rank-8 updates with the factor columns cf .. cf + 7 onto the column blocks jb .. jb + nj - 1: task t < nd = a lower
+  // block pair (bi >= bj) of L_kk's trailing matrix, relative to block jb; the others the blocks (row block r, column
+  // block jb + jj) of the tile
+  auto task = [&](int cf, int jb, int nj, int t) {
+    const int nd = nj * (nj + 1) / 2;
+    if (t < nd) {
+      int bi = 0, rem = t;
+      while (rem > bi) { rem -= bi + 1; ++bi; }          // t -> (bi, bj = rem), bj <= bi
+      rank8_dmma(sm.D, LDD, sm.D, cf, 8 * (jb + bi), 8 * (jb + rem), lane);
+    } else {
+      const int u = t - nd, r = u / nj;
+      rank8_dmma(sm.A, LDD, sm.D, cf, 8 * r, 8 * (jb + u - r * nj), lane);
+    }
+  };
+  auto rhs_update = [&](int cf, int c) {                 // right-hand-side entry c against the factor columns cf .. cf + 7
+    double acc = sm.A[NB * LDD + c];
+#pragma unroll
+    for (int s = 0; s < 8; ++s) acc = fma(-sm.A[NB * LDD + cf + s], sm.D[c * LDD + cf + s], acc);
+    sm.A[NB * LDD + c] = acc;
+  };
   for (int pb = 0; pb < npan; ++pb) {
     const int c0 = 8 * pb;
-    if (warp == 0 && !potrf_warp<8>(sm.D + c0 * LDD + c0, LDD, sm.dinv + c0, lane) && lane == 0) sm.flag = 1;
+    // (1) warp 0: the diagonal block.  Warps 1 .. 7 meanwhile: the updates of micro-panel pb - 1 that were not urgent --
+    //     onto the column blocks behind pb (pb itself got them before the barrier) -- in the shadow of the pivot chain
+    if (warp == 0) {
+      if (!potrf_warp<8>(sm.D + c0 * LDD + c0, LDD, sm.dinv + c0, lane) && lane == 0) sm.flag = 1;
+    } else if (pb > 0) {
+      const int nj = 7 - pb, nt = nj * (nj + 1) / 2 + nra * nj;
+      for (int t = warp - 1; t < nt; t += kSolveThreads / 32 - 1) task(c0 - 8, pb + 1, nj, t);
+      if (with_rhs && tid >= 192 && tid < 192 + 8 * nj) rhs_update(c0 - 8, c0 + 8 + (tid - 192));
+    }
     __syncthreads();
     const int below = NB - c0 - 8;                       // rows of L_kk under the diagonal block
-    {                                                    // x L11^T = a, one row per thread: threads 0 .. below - 1 the rows of
-      double* row = nullptr;                             // L_kk, 64 .. 64 + nrows - 1 the tile, 128 the right-hand side
+    {                                                    // (2) x L11^T = a, one row per thread: threads 0 .. below - 1 the rows of
+      double* row = nullptr;                             //     L_kk, 64 .. 64 + nrows - 1 the tile, 128 the right-hand side
       if (tid < below) row = sm.D + (c0 + 8 + tid) * LDD + c0;
       else if (tid >= NB && tid < NB + nrows) row = sm.A + (tid - NB) * LDD + c0;
       else if (tid == 2 * NB && with_rhs) row = sm.A + NB * LDD + c0;
@@ -194,26 +223,17 @@ __device__ bool panel64(Smem& sm, int nrows, bool with_rhs, int tid, int npan) {
       }
     }
     __syncthreads();
-    const int nb8 = below >> 3;                          // 8-column blocks still to update (= blocks per side of the trailing matrix)
-    const int nd = nb8 * (nb8 + 1) / 2, na = (nrows >> 3) * nb8;
-    for (int t = warp; t < nd + na; t += kSolveThreads / 32) {
-      if (t < nd) {
-        int bi = 0, rem = t;
-        while (rem > bi) { rem -= bi + 1; ++bi; }        // t -> (bi, bj = rem), bj <= bi
-        rank8_dmma(sm.D, LDD, sm.D, c0, c0 + 8 + 8 * bi, c0 + 8 + 8 * rem, lane);
-      } else {
-        const int u = t - nd, r = u / nb8;
-        rank8_dmma(sm.A, LDD, sm.D, c0, 8 * r, c0 + 8 + 8 * (u - r * nb8), lane);
+    // (3) the urgent updates: column block pb + 1, the next to be factorised (blocks (i, pb + 1) of L_kk, i > pb, and of
+    //     the tile; eight entries of the right-hand side)
+    if (pb < 7) {
+      const int ni = 7 - pb, nt = ni + nra;
+      for (int t = warp; t < nt; t += kSolveThreads / 32) {
+        if (t < ni) rank8_dmma(sm.D, LDD, sm.D, c0, c0 + 8 + 8 * t, c0 + 8, lane);
+        else rank8_dmma(sm.A, LDD, sm.D, c0, 8 * (t - ni), c0 + 8, lane);
       }
+      if (with_rhs && tid >= 248) rhs_update(c0, c0 + 8 + (tid - 248));
+      __syncthreads();
     }
-    if (with_rhs && tid >= 192 && tid < 192 + 8 * nb8) {  // the right-hand-side row (warps 6, 7: last in the DMMA round-robin)
-      const int c = c0 + 8 + (tid - 192);
-      double acc = sm.A[NB * LDD + c];
-#pragma unroll
-      for (int s = 0; s < 8; ++s) acc = fma(-sm.A[NB * LDD + c0 + s], sm.D[c * LDD + c0 + s], acc);
-      sm.A[NB * LDD + c] = acc;
-    }
-    __syncthreads();
   }
   return sm.flag == 0;
 }
@@ -400,15 +420,17 @@ __device__ void back_phase(const SolveArgs& a, Smem& sm, int kb, int G) {
   }
   if (tid < NB) { sm.y[tid] = __ldcg(a.ysol + kb * NB + tid); sm.dinv[tid] = __ldcg(a.Dinv + kb * NB + tid); }
   __syncthreads();
-  // D^T x = y, warp 0: lane owns x[lane], x[lane+32]; c from NB-1 down to 0
+  // D^T x = y, warp 0: lane owns x[lane], x[lane+32]; c from NB-1 down to 0.  The entries are kept divided by their
+  // own pivot (b_r / d_r, with the column entries L(c, r) / d_r: products that do not wait for anything), so that the chain
+  // from one column to the next is a broadcast and one FMA
   if (tid < 32) {
-    double b0 = sm.y[tid], b1 = sm.y[tid + 32];
+    const double d0 = sm.dinv[tid], d1 = sm.dinv[tid + 32];
+    double b0 = sm.y[tid] * d0, b1 = sm.y[tid + 32] * d1;
+#pragma unroll 4
     for (int c = NB - 1; c >= 0; --c) {
-      const double own = (c < 32) ? b0 : b1;
-      const double xc = __shfl_sync(0xffffffffu, own, c & 31) * sm.dinv[c];
-      if (tid == (c & 31)) { if (c < 32) b0 = xc; else b1 = xc; }
-      if (tid < c) b0 -= sm.D[c * LDD + tid] * xc;
-      if (tid + 32 < c) b1 -= sm.D[c * LDD + tid + 32] * xc;
+      const double xc = __shfl_sync(0xffffffffu, (c < 32) ? b0 : b1, c & 31);
+      if (tid < c) b0 = fma(-(sm.D[c * LDD + tid] * d0), xc, b0);
+      if (tid + 32 < c) b1 = fma(-(sm.D[c * LDD + tid + 32] * d1), xc, b1);
     }
     sm.y[tid] = b0;
     sm.y[tid + 32] = b1;
