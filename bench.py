@@ -419,12 +419,23 @@ def run_ours(args):
             costs = w.ba.depth_refine(labels, d.n_seg, d.pairs, d.delta, d.anchor_kf, eta, n_dit)
             ev1.record()
             torch.cuda.synchronize()
-            it_ms = ev0.elapsed_time(ev1) / n_dit
+            pass_ms = ev0.elapsed_time(ev1)
+            it_ms = pass_ms / n_dit
+            # the same pass with twice the iterations: the difference is the cost of an iteration proper, the rest the
+            # once-per-pass part (k_depth_prep, the label tables)
+            eta.zero_()
+            torch.cuda.synchronize()
+            ev0.record()
+            w.ba.depth_refine(labels, d.n_seg, d.pairs, d.delta, d.anchor_kf, eta, 2 * n_dit)
+            ev1.record()
+            torch.cuda.synchronize()
+            marginal_ms = (ev0.elapsed_time(ev1) - pass_ms) / n_dit
             dbytes = 20.0 * g.n_edges * g.hw + 20.0 * g.n_kf * g.hw      # per iteration: record + label per candidate, X_i + label per pixel
             depth["per_labelling"].append({
                 "labels": "4x8 grid (BASELINE config 5: 32 segments per keyframe)" if irregular == 0 else
                           "jittered superpixels (the paper's M_k ~ 200, PAPER.md:126)",
                 "segments_per_kf": d.n_seg, "ms_per_iteration": it_ms,
+                "ms_per_iteration_marginal": marginal_ms, "ms_once_per_pass": pass_ms - n_dit * marginal_ms,
                 "roofline": {"bound": "hbm", "kernel": "k_depth_edge", "algorithmic_bytes_per_iteration": dbytes,
                              "achieved": dbytes / (it_ms * 1e-3) / 1e9, "peak": load_peaks()[0], "unit": "GB/s",
                              "frac": dbytes / (it_ms * 1e-3) / 1e9 / load_peaks()[0],

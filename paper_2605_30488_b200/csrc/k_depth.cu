@@ -512,25 +512,49 @@ __global__ void k_depth_update(const double* __restrict__ partial, const double*
   eta_out[s] = es + step;
 }
 
-constexpr int kDpCostThreads = 1024;
+// The objective of an iteration (Eq. (9) data term from the per-CTA records, boundary and prior terms of Eq. (10)), in two
+// stages with a fixed order: CTA j of kDpCostCtas sums slice j of the records, of the pairs and of the segments (thread
+// partials, then a shared-memory tree) into stage[j]; the CTA that arrives last (a counter that it also resets) adds the
+// kDpCostCtas slice sums in index order.  One 1024-thread CTA over everything took 100 us on config 5.
+constexpr int kDpCostThreads = 256, kDpCostCtas = 64;
 __global__ void __launch_bounds__(kDpCostThreads)
 k_depth_cost(const double* __restrict__ partial, int n_rec, int rec, const double* __restrict__ eta, int n_total,
-             const int32_t* __restrict__ pairs, const double* __restrict__ delta, int n_pairs, DepthDev prm, double* __restrict__ out) {
+             const int32_t* __restrict__ pairs, const double* __restrict__ delta, int n_pairs, DepthDev prm, double* __restrict__ stage,
+             unsigned int* __restrict__ counter, double* __restrict__ out) {
   __shared__ double s[kDpCostThreads];
+  __shared__ bool last;
+  const int j = blockIdx.x, tid = threadIdx.x;
+  auto slice = [&](int n, int& lo, int& hi) { const int per = (n + kDpCostCtas - 1) / kDpCostCtas; lo = min(n, j * per); hi = min(n, lo + per); };
   double v = 0.0;
-  for (int q = threadIdx.x; q < n_rec; q += kDpCostThreads) v += partial[(size_t)q * rec + rec - 1];
-  for (int q = threadIdx.x; q < n_pairs; q += kDpCostThreads) {
+  int lo, hi;
+  slice(n_rec, lo, hi);
+  for (int q = lo + tid; q < hi; q += kDpCostThreads) v += __ldcg(partial + (size_t)q * rec + rec - 1);
+  slice(n_pairs, lo, hi);
+  for (int q = lo + tid; q < hi; q += kDpCostThreads) {
     const double d = eta[pairs[2 * q]] - eta[pairs[2 * q + 1]] + delta[q];
     v += 0.5 * prm.lambda_smooth * d * d;
   }
-  for (int q = threadIdx.x; q < n_total; q += kDpCostThreads) v += 0.5 * prm.lambda_prior * eta[q] * eta[q];
-  s[threadIdx.x] = v;
+  slice(n_total, lo, hi);
+  for (int q = lo + tid; q < hi; q += kDpCostThreads) v += 0.5 * prm.lambda_prior * eta[q] * eta[q];
+  s[tid] = v;
   __syncthreads();
   for (int o = kDpCostThreads / 2; o > 0; o >>= 1) {
-    if (threadIdx.x < o) s[threadIdx.x] += s[threadIdx.x + o];
+    if (tid < o) s[tid] += s[tid + o];
     __syncthreads();
   }
-  if (threadIdx.x == 0) *out = s[0];
+  if (tid == 0) {
+    stage[j] = s[0];
+    __threadfence();
+    last = atomicAdd(counter, 1u) == (unsigned)(kDpCostCtas - 1);
+  }
+  __syncthreads();
+  if (last && tid == 0) {
+    __threadfence();
+    double t = 0.0;
+    for (int q = 0; q < kDpCostCtas; ++q) t += __ldcg(stage + q);
+    *out = t;
+    *counter = 0u;                                            // ready for the next iteration (stream order)
+  }
 }
 
 // pm <- packed (exp(eta_label) X, w): the pointmap the next pose passes see (alternation of PAPER.md:143)
@@ -606,7 +630,7 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
   ok(up(&d_pairs, pairs, c->stream)); ok(up(&d_delta, delta, c->stream)); ok(up(&d_anchor, anchor, c->stream));
   ok(dmalloc(reinterpret_cast<void**>(&d_partial), std::max<size_t>((size_t)c->E * tiles * rec, 1) * sizeof(double)));
   ok(dmalloc(reinterpret_cast<void**>(&d_eta2), std::max<size_t>(n_total, 1) * sizeof(double)));
-  ok(dmalloc(reinterpret_cast<void**>(&d_cost), std::max(n_iters, 1) * sizeof(double)));
+  ok(dmalloc(reinterpret_cast<void**>(&d_cost), (std::max(n_iters, 1) + kDpCostCtas + 1) * sizeof(double)));   // [n_iters] costs, [kDpCostCtas] stage, counter
   const size_t EHW = (size_t)c->E * c->HW;
   ok(dmalloc(reinterpret_cast<void**>(&d_rec), std::max<size_t>(EHW, 1) * sizeof(float4)));
   ok(dmalloc(reinterpret_cast<void**>(&d_labn), std::max<size_t>(EHW, 1) * sizeof(int32_t)));
@@ -616,12 +640,15 @@ cudaError_t run_depth_refine(Ctx* c, const int32_t* d_labels, int n_seg, const i
     ++c->launches;
     ok(cudaGetLastError());
   }
+  double* d_stage = d_cost + std::max(n_iters, 1);            // slice sums of k_depth_cost, then its arrival counter (zeroed here, reset by the kernel)
+  if (e == cudaSuccess) ok(cudaMemsetAsync(d_stage + kDpCostCtas, 0, sizeof(double), c->stream));
   double *cur = d_eta, *nxt = d_eta2;
   for (int it = 0; it < n_iters && e == cudaSuccess; ++it) {
     if (c->E > 0)
       k_depth_edge<<<c->E * tiles, kDpThreads, smem, c->stream>>>(pm_init, d_rec, d_labn, c->edges, c->grp_edge, d_labels, cur, c->poses, c->H, c->W,
                                                                  n_seg, tiles, tile_rows, dev, d_partial);
-    k_depth_cost<<<1, kDpCostThreads, 0, c->stream>>>(d_partial, c->E * tiles, rec, cur, n_total, d_pairs, d_delta, n_pairs, dev, d_cost + it);
+    k_depth_cost<<<kDpCostCtas, kDpCostThreads, 0, c->stream>>>(d_partial, c->E * tiles, rec, cur, n_total, d_pairs, d_delta, n_pairs, dev, d_stage,
+                                                               reinterpret_cast<unsigned int*>(d_stage + kDpCostCtas), d_cost + it);
     k_depth_update<<<(n_total + 127) / 128, 128, 0, c->stream>>>(d_partial, cur, nxt, c->edges, c->kf_ptr, c->kf_edge, d_sp_ptr, d_sp_other,
                                                                  d_sp_delta, d_anchor, n_seg, n_total, tiles, dev);
     c->launches += 3;
