@@ -262,10 +262,10 @@ int sim3ba_load_system(sim3ba_ctx* ctx, const double* d_H, const double* d_g);
  * mode 0: the tiled Cholesky walks only the non-zero 64x64 tiles of L (symbolic tile-level factorisation of the
  *   keyframe graph in temporal order, fill included, computed at create).
  * mode 1: every lower tile (the dense blocked factorisation; always used for sim3ba_load_system).
- * Two environment variables exist for tests and experiments only and change no result: SIM3BA_BB_LMAX (read at create:
- * cap on the segment length of mode 2, default 2 sqrt(free keyframes)) and SIM3BA_SOLVE_MAX_CTAS (read at every solve:
- * cap on the grid of the persistent solve kernel, so that a CTA takes several segments / tiles; tau is bitwise
- * independent of the grid). */
+ * Two environment variables exist for tests and experiments only: SIM3BA_BB_LMAX (read at create: cap on the segment
+ * length of mode 2, default 2 sqrt(free keyframes); another elimination order, tau equal up to rounding) and
+ * SIM3BA_SOLVE_MAX_CTAS (read at every solve: cap on the grid of the persistent solve kernel, so that a CTA takes several
+ * segments / tiles; tau is bitwise independent of the grid). */
 int sim3ba_set_solver_mode(sim3ba_ctx* ctx, int32_t mode);
 /* Band + border plan of the graph (host output): h_info[0] = 1 if mode 2 applies to this graph, [1] interior
  * keyframes, [2] segments, [3] border keyframes, [4] longest segment, [5] most border keyframes touched by a segment. */
