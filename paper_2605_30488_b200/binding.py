@@ -367,9 +367,10 @@ class Sim3BA:
 
     def bb_info(self) -> Dict[str, int]:
         """Band + border plan of the graph (solver mode 2)."""
-        info = (C.c_int32 * 6)()
+        info = (C.c_int32 * 8)()
         self._check(self.lib.sim3ba_get_bb_info(self._h, info))
-        return dict(zip(("valid", "n_interior", "n_segments", "n_border", "max_segment", "max_segment_border"), list(info)))
+        return dict(zip(("valid", "n_interior", "n_segments", "n_border", "max_segment", "max_segment_border", "n_groups_level2",
+                         "n_border_dense"), list(info)))
 
     def launch_count(self) -> int:
         n = C.c_int64()

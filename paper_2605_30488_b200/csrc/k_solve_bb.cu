@@ -130,6 +130,51 @@ __device__ void bb_assemble(const BBArgs& a, double eps, int G) {
   }
 }
 
+// ---- phase 2b: the columns of the second level, read out of S (the level-1 border system after the Schur rows) ----------
+// a2's "keyframes" are level-1 border indices.  Column c of a2 = separator keyframe b: D = S(b, b) (the lower triangle of
+// S is the valid one), band block t = S(b', b) for the next members b' of the same group, border block q = S(q, b) -- or
+// S(b, q)^T where q precedes b in S -- and the right-hand side b_B(b); then the dense system of the keyframes that stay.
+__device__ void bb_assemble2(const BBArgs& a, const BBArgs& a2, int G) {
+  const int tid = threadIdx.x;
+  const size_t nB = (size_t)a.npadB;
+  const double* S = a.B.L;
+  for (int c = blockIdx.x; c < a2.n_int; c += G) {
+    const int nb = a2.col_nb[c];
+    const int nel = (1 + kBand + nb) * 49 + 7;
+    const int b = a2.col_kf[c];
+    int s = 0;
+    while (a2.seg_ptr[s + 1] <= c) ++s;
+    const int last = a2.seg_ptr[s + 1] - 1;                   // last column of the group
+    const int32_t* sb = a2.seg_bord + a2.seg_bptr[s];
+    double* col = a2.colbuf + a2.col_ofs[c];
+    for (int idx = tid; idx < nel; idx += kSolveThreads) {
+      const int blk = idx / 49, e = idx - blk * 49, r = e / 7, cc = e - r * 7;
+      double v = 0.0;
+      if (blk == 0) {
+        v = __ldcg(S + (size_t)(7 * b + max(r, cc)) * nB + 7 * b + min(r, cc));
+      } else if (blk <= kBand) {
+        if (c + blk <= last) v = __ldcg(S + (size_t)(7 * a2.col_kf[c + blk] + r) * nB + 7 * b + cc);
+      } else if (blk < 1 + kBand + nb) {
+        const int q = a2.bord_kf[sb[blk - 1 - kBand]];        // level-1 index of the level-2 border keyframe
+        v = (q > b) ? __ldcg(S + (size_t)(7 * q + r) * nB + 7 * b + cc) : __ldcg(S + (size_t)(7 * b + cc) * nB + 7 * q + r);
+      } else {
+        v = __ldcg(a.B.rhs + 7 * b + e);
+      }
+      col[idx] = v;
+    }
+  }
+  const int nB2 = a2.npadB, n72 = 7 * a2.n_bord;
+  for (long long idx = (long long)blockIdx.x * kSolveThreads + tid; idx < (long long)nB2 * nB2; idx += (long long)G * kSolveThreads) {
+    const int R = (int)(idx / nB2), C = (int)(idx - (long long)R * nB2);
+    if (C / kNB > R / kNB) continue;
+    double v = 0.0;
+    if (R >= n72 || C >= n72) v = (R == C) ? 1.0 : 0.0;
+    else if (C <= R) v = __ldcg(S + (size_t)(7 * a2.bord_kf[R / 7] + R % 7) * nB + 7 * a2.bord_kf[C / 7] + C % 7);
+    a2.B.L[(size_t)R * nB2 + C] = v;
+    if (C == 0) a2.B.rhs[R] = (R < n72) ? __ldcg(a.B.rhs + 7 * a2.bord_kf[R / 7] + R % 7) : 0.0;
+  }
+}
+
 // ---- phase 1: block Cholesky of one segment -----------------------------------------------------------
 struct SegSmem {
   double inv[2][8];     // 1 / diag(L_cc) of the column being eliminated (parity of the column) and of the next one
@@ -513,14 +558,52 @@ __device__ void bb_back(const BBArgs& a, double* ring, double* z, double* tb, in
   __syncthreads();
 }
 
+// ---- phase 3: the dense border system of t (tiled Cholesky with the forward solve riding along, then the backward
+// solve; a system of one tile directly by CTA 0).  Returns true (uniformly) if a pivot failed; otherwise tau_B is final and
+// a grid barrier has been passed since it was written.
+__device__ bool bb_border_solve(const BBArgs& t, Smem& sm, int G, unsigned int& gen) {
+  const int nbB = t.npadB / kNB;
+  if (nbB == 0) return false;
+  bool failed = false;
+  if (nbB == 1) {                                             // one tile: direct solve by CTA 0
+    if (blockIdx.x == 0) bb_small_border(t, sm, 7 * t.n_bord);
+    grid_barrier(t.bar, G, gen);
+    return ld_flag(t.status) != 0;
+  }
+  for (int k = 0; k < nbB; ++k) {                             // tiled Cholesky of S, forward solve riding along
+    panel_phase(t.B, sm, k, G);
+    if (t.B.col_ptr[k + 1] > t.B.col_ptr[k]) {
+      grid_barrier(t.bar, G, gen);
+      if (ld_flag(t.status) != 0) { failed = true; break; }
+      update_phase(t.B, sm, k, G);
+      grid_barrier(t.bar, G, gen);
+    }
+  }
+  if (!failed) {
+    grid_barrier(t.bar, G, gen);
+    failed = ld_flag(t.status) != 0;
+  }
+  if (failed) return true;
+  for (int kb = nbB - 1; kb >= 0; --kb) {
+    back_phase(t.B, sm, kb, G);
+    if (t.B.row_ptr[kb + 1] > t.B.row_ptr[kb]) grid_barrier(t.bar, G, gen);
+  }
+  grid_barrier(t.bar, G, gen);                                // tau_B is final
+  return false;
+}
+
+// a: the graph's band + border plan.  a2: its second level (a2.n_seg = 0 if there is none): an independent set of separator
+// groups eliminated from the border system S before the dense solve, with the same four phases on columns read out of S.
 __global__ void __launch_bounds__(kSolveThreads, 1)
-k_solve_bb(BBArgs a) {
+k_solve_bb(BBArgs a, BBArgs a2) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);              // phase 3 view
   double* win = reinterpret_cast<double*>(smem_raw);          // phase 1 / 4 view
   const int G = gridDim.x, tid = threadIdx.x;
   double* brhs = win + (size_t)kWin * a.slot_doubles;         // [7 kMaxSegBorder]
   SegSmem& ss = *reinterpret_cast<SegSmem*>(brhs + 7 * kMaxSegBorder);
+  double* ring = win;                                         // phase 4 view
+  double* z = win + (size_t)kBackRing * (1 + kBand) * 49;
   unsigned int gen = 0;
   bool solved = false;
   double eps = a.eps0;
@@ -541,43 +624,34 @@ k_solve_bb(BBArgs a) {
       for (int b = blockIdx.x; b < a.n_bord; b += G) bb_schur_row(a, win, b);
       grid_barrier(a.bar, G, gen);
       BB_STAMP(4);
-      if (nbB == 1) {                                         // one tile: direct solve by CTA 0
-        if (blockIdx.x == 0) bb_small_border(a, sm, 7 * a.n_bord);
+      if (a2.n_seg > 0) {                                     // second level on S
+        bb_assemble2(a, a2, G);
+        grid_barrier(a.bar, G, gen);
+        for (int s = blockIdx.x; s < a2.n_seg; s += G) bb_segment(a2, win, brhs, ss, s);
         grid_barrier(a.bar, G, gen);
         failed = ld_flag(a.status) != 0;
+        if (!failed && a2.n_bord > 0) {
+          for (int b = blockIdx.x; b < a2.n_bord; b += G) bb_schur_row(a2, win, b);
+          grid_barrier(a.bar, G, gen);
+          failed = bb_border_solve(a2, sm, G, gen);
+        }
+        if (!failed) {                                        // back through the second level: tau_B of the first
+          for (int s = blockIdx.x; s < a2.n_seg; s += G) bb_back(a2, ring, z, z + 7 * a2.max_len, s);
+          for (int q = blockIdx.x * kSolveThreads + tid; q < 7 * a2.n_bord; q += G * kSolveThreads)
+            a.B.tau[7 * a2.bord_kf[q / 7] + q % 7] = __ldcg(a2.B.tau + q);
+          grid_barrier(a.bar, G, gen);
+        }
       } else {
-      for (int k = 0; k < nbB; ++k) {                         // tiled Cholesky of S, forward solve riding along
-        panel_phase(a.B, sm, k, G);
-        if (a.B.col_ptr[k + 1] > a.B.col_ptr[k]) {
-          grid_barrier(a.bar, G, gen);
-          if (ld_flag(a.status) != 0) { failed = true; break; }
-          update_phase(a.B, sm, k, G);
-          grid_barrier(a.bar, G, gen);
-        }
-      }
-      if (!failed) {
-        grid_barrier(a.bar, G, gen);
-        failed = ld_flag(a.status) != 0;
-      }
-      if (!failed) {
-        for (int kb = nbB - 1; kb >= 0; --kb) {
-          back_phase(a.B, sm, kb, G);
-          if (a.B.row_ptr[kb + 1] > a.B.row_ptr[kb]) grid_barrier(a.bar, G, gen);
-        }
-      }
+        failed = bb_border_solve(a, sm, G, gen);
       }
     }
     if (failed) {
       grid_barrier(a.bar, G, gen);   // everybody has seen the flag before it is cleared again
       continue;
     }
-    if (nbB != 1) grid_barrier(a.bar, G, gen);     // tau_B is final (the one-tile path has just passed a barrier)
     BB_STAMP(5);
     {
-      double* ring = win;
-      double* z = win + (size_t)kBackRing * (1 + kBand) * 49;
-      double* tb = z + 7 * a.max_len;
-      for (int s = blockIdx.x; s < a.n_seg; s += G) bb_back(a, ring, z, tb, s);
+      for (int s = blockIdx.x; s < a.n_seg; s += G) bb_back(a, ring, z, z + 7 * a.max_len, s);
       for (int q = blockIdx.x * kSolveThreads + tid; q < 7 * a.n_bord; q += G * kSolveThreads)
         a.tau[7 * a.bord_kf[q / 7] + q % 7] = __ldcg(a.B.tau + q);
     }
@@ -599,7 +673,7 @@ k_solve_bb(BBArgs a) {
 }  // namespace
 
 static size_t bb_smem_bytes(const BBPlan& P, int* slot_out) {
-  const int slot = ((1 + kBand + P.max_nb) * 49 + 7 + 1) & ~1;
+  const int slot = ((1 + kBand + std::max(P.max_nb, P.l2.valid ? P.l2.max_nb : 0)) * 49 + 7 + 1) & ~1;   // one window slot size for both levels
   const size_t smem_seg = ((size_t)kWin * slot + 7 * kMaxSegBorder) * sizeof(double) + sizeof(SegSmem);
   const size_t smem_back = ((size_t)kBackRing * (1 + kBand) * 49 + 7 * (size_t)P.max_len + 7 * kMaxSegBorder) * sizeof(double);
   const size_t smem_schur = (size_t)2 * kSchurCols * kSchurPart * sizeof(double);
@@ -635,6 +709,8 @@ cudaError_t launch_solve_bb(Ctx* c) {
   // one per segment / border keyframe / tile task
   long long want = std::max<long long>({(long long)P.n_seg, (long long)P.n_bord, (long long)D.max_upd, (long long)D.max_col,
                                         (long long)P.n_int, 1LL});
+  const BBLevel2& Q = P.l2;
+  if (Q.valid) want = std::max<long long>({want, (long long)Q.n_int, (long long)Q.dense.max_upd, (long long)Q.dense.max_col});
   int G = (int)std::min<long long>(want, (long long)num_sms * std::min(max_blocks_per_sm, 1));
   if (const char* cap = getenv("SIM3BA_SOLVE_MAX_CTAS")) G = std::max(1, std::min(G, atoi(cap)));   // tests: several segments / tiles / tasks per CTA
   BBArgs a{};
@@ -653,13 +729,29 @@ cudaError_t launch_solve_bb(Ctx* c) {
   B.eps0 = c->prm.eps0; B.max_attempts = c->prm.max_attempts; B.status = c->fail_flag; B.eps_used = c->d_eps_used; B.bar = c->bar;
   a.tau = c->tau; a.fixed = c->fixed_mask; a.N = c->N;
   a.eps0 = c->prm.eps0; a.max_attempts = c->prm.max_attempts; a.status = c->fail_flag; a.eps_used = c->d_eps_used; a.bar = c->bar;
+  BBArgs a2{};                                              // second level (n_seg = 0: none)
+  if (Q.valid) {
+    a2.n_int = Q.n_int; a2.n_seg = Q.n_seg; a2.n_bord = Q.n_bord; a2.npadB = Q.npadB; a2.slot_doubles = slot; a2.max_len = Q.max_len;
+    a2.seg_ptr = Q.seg_ptr; a2.seg_bptr = Q.seg_bptr; a2.seg_bord = Q.seg_bord; a2.col_kf = Q.col_kf; a2.col_nb = Q.col_nb;
+    a2.bord_kf = Q.bord_kf; a2.bord_sptr = Q.bord_sptr; a2.bord_seg = Q.bord_seg; a2.bord_slot = Q.bord_slot;
+    a2.col_ofs = reinterpret_cast<const long long*>(Q.col_ofs); a2.colbuf = Q.colbuf; a2.seg_rhs = Q.seg_rhs;
+    SolveArgs& B2 = a2.B;
+    const SolvePlan& D2 = Q.dense;
+    B2.L = Q.LB; B2.npad = Q.npadB; B2.n = 7 * Q.n_bord; B2.nb = Q.npadB / kNB;
+    B2.col_ptr = D2.col_ptr; B2.col_rows = D2.col_rows; B2.row_ptr = D2.row_ptr; B2.row_cols = D2.row_cols; B2.tiles = D2.tiles; B2.n_tiles = D2.n_tiles;
+    B2.rhs = Q.rhsB; B2.ysol = Q.ysolB; B2.Dinv = Q.DinvB; B2.tau = Q.tauB;
+    B2.eps0 = c->prm.eps0; B2.max_attempts = c->prm.max_attempts; B2.status = c->fail_flag; B2.eps_used = c->d_eps_used; B2.bar = c->bar;
+    a2.tau = P.tauB;                                          // the columns of the second level are border keyframes of the first
+    a2.N = P.n_bord;
+    a2.eps0 = c->prm.eps0; a2.max_attempts = c->prm.max_attempts; a2.status = c->fail_flag; a2.eps_used = c->d_eps_used; a2.bar = c->bar;
+  }
   cudaError_t e = cudaMemsetAsync(c->bar, 0, sizeof(unsigned int), c->stream);
   if (e != cudaSuccess) return e;
   if (c->profiling) {
     cudaMemsetAsync(c->solve_stamps, 0, 16 * sizeof(unsigned long long), c->stream);
     cudaEventRecord(c->ev[4], c->stream);
   }
-  void* args[] = {&a};
+  void* args[] = {&a, &a2};
   e = cudaLaunchCooperativeKernel((const void*)k_solve_bb, dim3(G), dim3(kSolveThreads), args, smem, c->stream);
   c->launches += 1;
   c->last_solve_grid = G;

@@ -68,8 +68,26 @@ struct SolvePlan {
 // update follows by back-substitution.  Same tau as the tile plans up to rounding.
 constexpr int kBand = 3;          // block band of a chain (edges (k, k+1..k+3))
 constexpr int kMaxSegBorder = 28; // border keyframes one segment may touch (else the plan is not used)
+// Second level of the band + border plan: the Schur complement S on the border keyframes is itself sparse -- a separator
+// group (the <= kBand keyframes of a cut) is coupled only to the groups and long-link keyframes that share a segment with
+// it.  An independent set of separator groups (no two of them coupled in S) is eliminated from S exactly like the
+// segments were from H -- each group a "segment" of <= kBand columns whose blocks are read out of S -- and the dense tiled
+// Cholesky runs on what is left.  Same array roles as in BBPlan; "keyframe" of a column / of a border entry here is a
+// level-1 BORDER INDEX.
+struct BBLevel2 {
+  bool valid = false;
+  int n_int = 0, n_seg = 0, n_bord = 0, max_nb = 0, max_len = 0, npadB = 0;
+  double flops_saved = 0.0;
+  int32_t *seg_ptr = nullptr, *seg_bptr = nullptr, *seg_bord = nullptr, *col_kf = nullptr, *col_nb = nullptr, *bord_kf = nullptr;
+  int32_t *bord_sptr = nullptr, *bord_seg = nullptr, *bord_slot = nullptr;
+  int64_t* col_ofs = nullptr;
+  double *colbuf = nullptr, *seg_rhs = nullptr, *LB = nullptr, *rhsB = nullptr, *ysolB = nullptr, *DinvB = nullptr, *tauB = nullptr;
+  SolvePlan dense;
+};
+
 struct BBPlan {
   bool ready = false, valid = false;
+  BBLevel2 l2;
   int n_int = 0, n_seg = 0, n_bord = 0, max_nb = 0, max_len = 0;
   int npadB = 0;                  // padded size of the border system (multiple of kNB), 0 if no border
   size_t col_doubles = 0;         // doubles of all interior block columns

@@ -264,7 +264,15 @@ def test_solver_modes_agree(k, monkeypatch):
     tau_floor = 1e-6 * np.sqrt(sol.tau.size)
     taus = {}
     for tag, mode, lmax, max_ctas in (("bb", 2, None, None), ("bb-short", 2, "5", None), ("tile", 0, None, None), ("dense", 1, None, None),
-                                      ("bb-short-2ctas", 2, "5", "2"), ("tile-1cta", 0, None, "1"), ("dense-2ctas", 1, None, "2")):
+                                      ("bb-short-2ctas", 2, "5", "2"), ("tile-1cta", 0, None, "1"), ("dense-2ctas", 1, None, "2"),
+                                      ("bb-1level", 2, None, None), ("bb-short-1level", 2, "5", None),
+                                      ("bb-2level", 2, None, None), ("bb-short-2level", 2, "5", None), ("bb-short-2level-2ctas", 2, "5", "2")):
+        if tag.endswith("1level"):                        # without the second level of the plan (separator groups out of S)
+            monkeypatch.setenv("SIM3BA_BB_LEVELS", "1")
+        elif "2level" in tag:                             # ... and with it wherever a group can be eliminated (by default: where it pays)
+            monkeypatch.setenv("SIM3BA_BB_LEVELS", "2")
+        else:
+            monkeypatch.delenv("SIM3BA_BB_LEVELS", raising=False)
         if lmax is None:
             monkeypatch.delenv("SIM3BA_BB_LMAX", raising=False)
         else:
@@ -278,6 +286,10 @@ def test_solver_modes_agree(k, monkeypatch):
         assert info["valid"] == 1 and info["n_interior"] + info["n_border"] == g.n_kf - len(g.fixed_kf)
         if lmax is not None:
             assert info["max_segment"] <= 5
+        if tag.endswith("1level"):
+            assert info["n_groups_level2"] == 0 and info["n_border_dense"] == info["n_border"]
+        elif "2level" in tag and k >= 4 + (lmax is None):  # reduced C4 / C5 with short segments, reduced C5 as it is: groups to eliminate
+            assert info["n_groups_level2"] > 0 and info["n_border_dense"] < info["n_border"]
         ba.set_solver_mode(mode)
         set_poses(ba, p0)
         ba.build_system()
@@ -291,7 +303,7 @@ def test_solver_modes_agree(k, monkeypatch):
         ba.close()
     for tag in taus:
         assert rel(taus[tag], taus["bb"], tau_floor) <= 1e-6, tag
-    for tag, same in (("bb-short-2ctas", "bb-short"), ("tile-1cta", "tile"), ("dense-2ctas", "dense")):
+    for tag, same in (("bb-short-2ctas", "bb-short"), ("tile-1cta", "tile"), ("dense-2ctas", "dense"), ("bb-short-2level-2ctas", "bb-short-2level")):
         assert np.array_equal(taus[tag], taus[same]), tag          # the grid size does not change the order of any sum
 
 
