@@ -258,22 +258,22 @@ int sim3ba_load_system(sim3ba_ctx* ctx, const double* d_H, const double* d_g);
  *   border keyframes (one endpoint of every longer link: loop closures, inter-agent edges; separator triples
  *   that cap a segment's length); segments are eliminated at 7x7 granularity in parallel, the Schur complement
  *   on the border is a small system S that is itself sparse: where that removes at least two 64-row tile columns,
- *   an independent set of separator groups is eliminated from S in the same way (second level) before the tiled
- *   Cholesky takes the dense rest.  Where the graph does not have that shape (a segment touching more than 28 border
+ *   an independent set of separator groups is eliminated from S in the same way, and again from what that leaves
+ *   (up to three further levels), before the tiled Cholesky takes the dense rest.  Where the graph does not have that shape (a segment touching more than 28 border
  *   keyframes, more than 292 border keyframes) mode 2 runs mode 0.
  * mode 0: the tiled Cholesky walks only the non-zero 64x64 tiles of L (symbolic tile-level factorisation of the
  *   keyframe graph in temporal order, fill included, computed at create).
  * mode 1: every lower tile (the dense blocked factorisation; always used for sim3ba_load_system).
  * Three environment variables exist for tests and experiments only: SIM3BA_BB_LMAX (read at create: cap on the segment
- * length of mode 2, default 1.4 sqrt(free keyframes)) and SIM3BA_BB_LEVELS (read at create: 1 = no second level, 2 = second
- * level wherever a separator group can be eliminated) -- other elimination orders, tau equal up to rounding -- and
+ * length of mode 2, default 0.9 sqrt(free keyframes)) and SIM3BA_BB_LEVELS (read at create: 1 = no further levels, 2 = a
+ * further level wherever a separator group can be eliminated) -- other elimination orders, tau equal up to rounding -- and
  * SIM3BA_SOLVE_MAX_CTAS (read at every solve: cap on the grid of the persistent solve kernel, so that a CTA takes several
  * segments / tiles; tau is bitwise independent of the grid). */
 int sim3ba_set_solver_mode(sim3ba_ctx* ctx, int32_t mode);
 /* Band + border plan of the graph (host output): h_info[0] = 1 if mode 2 applies to this graph, [1] interior
  * keyframes, [2] segments, [3] border keyframes, [4] longest segment, [5] most border keyframes touched by a segment,
- * [6] separator groups eliminated at the second level (0: no second level), [7] keyframes of the dense system that is
- * finally solved (= [3] without a second level). */
+ * [6] separator groups eliminated at the further levels (0: none), [7] keyframes of the dense system that is finally
+ * solved (= [3] without further levels). */
 int sim3ba_get_bb_info(sim3ba_ctx* ctx, int32_t h_info[8]);
 /* Host outputs (each may be NULL): non-zero tiles of the tile-sparse plan (of the dense plan in mode 1), lower tiles of
  * the dense plan, flop count of the ACTIVE plan (factor + both triangular solves, FMA = 2: at 7x7 granularity with a dense

@@ -69,6 +69,11 @@ struct BBArgs {
   int32_t* status; double* eps_used; unsigned int* bar;
 };
 
+struct BBLevels {
+  int n;                           // further levels behind the first (0: the border system of the first is solved densely)
+  BBArgs lv[BBPlan::kMaxLevels];
+};
+
 __device__ __forceinline__ int col_stride(int nb) { return ((1 + kBand + nb) * 49 + 7 + 1) & ~1; }
 __device__ __forceinline__ int tri77(int r, int c) { return r <= c ? r * 7 - r * (r - 1) / 2 + (c - r) : c * 7 - c * (c - 1) / 2 + (r - c); }
 
@@ -592,10 +597,11 @@ __device__ bool bb_border_solve(const BBArgs& t, Smem& sm, int G, unsigned int& 
   return false;
 }
 
-// a: the graph's band + border plan.  a2: its second level (a2.n_seg = 0 if there is none): an independent set of separator
-// groups eliminated from the border system S before the dense solve, with the same four phases on columns read out of S.
+// a: the graph's band + border plan.  L: its further levels: each eliminates an independent set of separator groups from
+// the border system the level before left, with the same phases on columns read out of that system; the dense solve
+// takes what the last level leaves.
 __global__ void __launch_bounds__(kSolveThreads, 1)
-k_solve_bb(BBArgs a, BBArgs a2) {
+k_solve_bb(const __grid_constant__ BBArgs a, const __grid_constant__ BBLevels L) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);              // phase 3 view
   double* win = reinterpret_cast<double*>(smem_raw);          // phase 1 / 4 view
@@ -624,25 +630,30 @@ k_solve_bb(BBArgs a, BBArgs a2) {
       for (int b = blockIdx.x; b < a.n_bord; b += G) bb_schur_row(a, win, b);
       grid_barrier(a.bar, G, gen);
       BB_STAMP(4);
-      if (a2.n_seg > 0) {                                     // second level on S
-        bb_assemble2(a, a2, G);
+      const BBArgs* prev = &a;
+      for (int k = 0; k < L.n && !failed; ++k) {              // further levels: groups out of the border system of the level before
+        const BBArgs& cur = L.lv[k];
+        bb_assemble2(*prev, cur, G);
         grid_barrier(a.bar, G, gen);
-        for (int s = blockIdx.x; s < a2.n_seg; s += G) bb_segment(a2, win, brhs, ss, s);
+        for (int s = blockIdx.x; s < cur.n_seg; s += G) bb_segment(cur, win, brhs, ss, s);
         grid_barrier(a.bar, G, gen);
         failed = ld_flag(a.status) != 0;
-        if (!failed && a2.n_bord > 0) {
-          for (int b = blockIdx.x; b < a2.n_bord; b += G) bb_schur_row(a2, win, b);
-          grid_barrier(a.bar, G, gen);
-          failed = bb_border_solve(a2, sm, G, gen);
-        }
-        if (!failed) {                                        // back through the second level: tau_B of the first
-          for (int s = blockIdx.x; s < a2.n_seg; s += G) bb_back(a2, ring, z, z + 7 * a2.max_len, s);
-          for (int q = blockIdx.x * kSolveThreads + tid; q < 7 * a2.n_bord; q += G * kSolveThreads)
-            a.B.tau[7 * a2.bord_kf[q / 7] + q % 7] = __ldcg(a2.B.tau + q);
+        if (!failed && cur.n_bord > 0) {
+          for (int b = blockIdx.x; b < cur.n_bord; b += G) bb_schur_row(cur, win, b);
           grid_barrier(a.bar, G, gen);
         }
-      } else {
-        failed = bb_border_solve(a, sm, G, gen);
+        prev = &cur;
+      }
+      if (!failed) failed = bb_border_solve(*prev, sm, G, gen);
+      if (!failed) {
+        for (int k = L.n - 1; k >= 0; --k) {                   // back through the levels: tau_B of the level before
+          const BBArgs& cur = L.lv[k];
+          const BBArgs& upper = (k > 0) ? L.lv[k - 1] : a;
+          for (int s = blockIdx.x; s < cur.n_seg; s += G) bb_back(cur, ring, z, z + 7 * cur.max_len, s);
+          for (int q = blockIdx.x * kSolveThreads + tid; q < 7 * cur.n_bord; q += G * kSolveThreads)
+            upper.B.tau[7 * cur.bord_kf[q / 7] + q % 7] = __ldcg(cur.B.tau + q);
+          grid_barrier(a.bar, G, gen);
+        }
       }
     }
     if (failed) {
@@ -673,7 +684,9 @@ k_solve_bb(BBArgs a, BBArgs a2) {
 }  // namespace
 
 static size_t bb_smem_bytes(const BBPlan& P, int* slot_out) {
-  const int slot = ((1 + kBand + std::max(P.max_nb, P.l2.valid ? P.l2.max_nb : 0)) * 49 + 7 + 1) & ~1;   // one window slot size for both levels
+  int max_nb = P.max_nb;
+  for (int k = 0; k < P.n_lv; ++k) max_nb = std::max(max_nb, P.lv[k].max_nb);
+  const int slot = ((1 + kBand + max_nb) * 49 + 7 + 1) & ~1;   // one window slot size for all levels
   const size_t smem_seg = ((size_t)kWin * slot + 7 * kMaxSegBorder) * sizeof(double) + sizeof(SegSmem);
   const size_t smem_back = ((size_t)kBackRing * (1 + kBand) * 49 + 7 * (size_t)P.max_len + 7 * kMaxSegBorder) * sizeof(double);
   const size_t smem_schur = (size_t)2 * kSchurCols * kSchurPart * sizeof(double);
@@ -709,8 +722,8 @@ cudaError_t launch_solve_bb(Ctx* c) {
   // one per segment / border keyframe / tile task
   long long want = std::max<long long>({(long long)P.n_seg, (long long)P.n_bord, (long long)D.max_upd, (long long)D.max_col,
                                         (long long)P.n_int, 1LL});
-  const BBLevel2& Q = P.l2;
-  if (Q.valid) want = std::max<long long>({want, (long long)Q.n_int, (long long)Q.dense.max_upd, (long long)Q.dense.max_col});
+  for (int k = 0; k < P.n_lv; ++k) want = std::max<long long>(want, (long long)P.lv[k].n_int);
+  if (P.n_lv > 0) want = std::max<long long>({want, (long long)P.lv[P.n_lv - 1].dense.max_upd, (long long)P.lv[P.n_lv - 1].dense.max_col});
   int G = (int)std::min<long long>(want, (long long)num_sms * std::min(max_blocks_per_sm, 1));
   if (const char* cap = getenv("SIM3BA_SOLVE_MAX_CTAS")) G = std::max(1, std::min(G, atoi(cap)));   // tests: several segments / tiles / tasks per CTA
   BBArgs a{};
@@ -729,20 +742,23 @@ cudaError_t launch_solve_bb(Ctx* c) {
   B.eps0 = c->prm.eps0; B.max_attempts = c->prm.max_attempts; B.status = c->fail_flag; B.eps_used = c->d_eps_used; B.bar = c->bar;
   a.tau = c->tau; a.fixed = c->fixed_mask; a.N = c->N;
   a.eps0 = c->prm.eps0; a.max_attempts = c->prm.max_attempts; a.status = c->fail_flag; a.eps_used = c->d_eps_used; a.bar = c->bar;
-  BBArgs a2{};                                              // second level (n_seg = 0: none)
-  if (Q.valid) {
+  BBLevels L{};
+  L.n = P.n_lv;
+  for (int k = 0; k < P.n_lv; ++k) {
+    const BBLevel2& Q = P.lv[k];
+    BBArgs& a2 = L.lv[k];
     a2.n_int = Q.n_int; a2.n_seg = Q.n_seg; a2.n_bord = Q.n_bord; a2.npadB = Q.npadB; a2.slot_doubles = slot; a2.max_len = Q.max_len;
     a2.seg_ptr = Q.seg_ptr; a2.seg_bptr = Q.seg_bptr; a2.seg_bord = Q.seg_bord; a2.col_kf = Q.col_kf; a2.col_nb = Q.col_nb;
     a2.bord_kf = Q.bord_kf; a2.bord_sptr = Q.bord_sptr; a2.bord_seg = Q.bord_seg; a2.bord_slot = Q.bord_slot;
     a2.col_ofs = reinterpret_cast<const long long*>(Q.col_ofs); a2.colbuf = Q.colbuf; a2.seg_rhs = Q.seg_rhs;
     SolveArgs& B2 = a2.B;
-    const SolvePlan& D2 = Q.dense;
+    const SolvePlan& D2 = Q.dense;                            // filled for the last level only: the others are never solved densely
     B2.L = Q.LB; B2.npad = Q.npadB; B2.n = 7 * Q.n_bord; B2.nb = Q.npadB / kNB;
     B2.col_ptr = D2.col_ptr; B2.col_rows = D2.col_rows; B2.row_ptr = D2.row_ptr; B2.row_cols = D2.row_cols; B2.tiles = D2.tiles; B2.n_tiles = D2.n_tiles;
     B2.rhs = Q.rhsB; B2.ysol = Q.ysolB; B2.Dinv = Q.DinvB; B2.tau = Q.tauB;
     B2.eps0 = c->prm.eps0; B2.max_attempts = c->prm.max_attempts; B2.status = c->fail_flag; B2.eps_used = c->d_eps_used; B2.bar = c->bar;
-    a2.tau = P.tauB;                                          // the columns of the second level are border keyframes of the first
-    a2.N = P.n_bord;
+    a2.tau = (k > 0) ? P.lv[k - 1].tauB : P.tauB;             // the columns of a level are border keyframes of the level before
+    a2.N = (k > 0) ? P.lv[k - 1].n_bord : P.n_bord;
     a2.eps0 = c->prm.eps0; a2.max_attempts = c->prm.max_attempts; a2.status = c->fail_flag; a2.eps_used = c->d_eps_used; a2.bar = c->bar;
   }
   cudaError_t e = cudaMemsetAsync(c->bar, 0, sizeof(unsigned int), c->stream);
@@ -751,7 +767,7 @@ cudaError_t launch_solve_bb(Ctx* c) {
     cudaMemsetAsync(c->solve_stamps, 0, 16 * sizeof(unsigned long long), c->stream);
     cudaEventRecord(c->ev[4], c->stream);
   }
-  void* args[] = {&a, &a2};
+  void* args[] = {&a, &L};
   e = cudaLaunchCooperativeKernel((const void*)k_solve_bb, dim3(G), dim3(kSolveThreads), args, smem, c->stream);
   c->launches += 1;
   c->last_solve_grid = G;

@@ -842,7 +842,9 @@ int sim3ba_get_bb_info(sim3ba_ctx* h, int32_t info[8]) {
   if (!h || !info) return SIM3BA_ERR_INVALID_ARG;
   const BBPlan& P = h->c.plan_bb;
   info[0] = P.valid ? 1 : 0; info[1] = P.n_int; info[2] = P.n_seg; info[3] = P.n_bord; info[4] = P.max_len; info[5] = P.max_nb;
-  info[6] = P.l2.valid ? P.l2.n_seg : 0; info[7] = P.l2.valid ? P.l2.n_bord : P.n_bord;
+  info[6] = 0;
+  for (int k = 0; k < P.n_lv; ++k) info[6] += P.lv[k].n_seg;
+  info[7] = P.n_lv > 0 ? P.lv[P.n_lv - 1].n_bord : P.n_bord;
   return SIM3BA_OK;
 }
 

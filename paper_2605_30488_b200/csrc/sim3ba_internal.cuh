@@ -68,12 +68,13 @@ struct SolvePlan {
 // update follows by back-substitution.  Same tau as the tile plans up to rounding.
 constexpr int kBand = 3;          // block band of a chain (edges (k, k+1..k+3))
 constexpr int kMaxSegBorder = 28; // border keyframes one segment may touch (else the plan is not used)
-// Second level of the band + border plan: the Schur complement S on the border keyframes is itself sparse -- a separator
+// Further levels of the band + border plan: the Schur complement S on the border keyframes is itself sparse -- a separator
 // group (the <= kBand keyframes of a cut) is coupled only to the groups and long-link keyframes that share a segment with
 // it.  An independent set of separator groups (no two of them coupled in S) is eliminated from S exactly like the
-// segments were from H -- each group a "segment" of <= kBand columns whose blocks are read out of S -- and the dense tiled
-// Cholesky runs on what is left.  Same array roles as in BBPlan; "keyframe" of a column / of a border entry here is a
-// level-1 BORDER INDEX.
+// segments were from H -- each group a "segment" of <= kBand columns whose blocks are read out of S -- which leaves a
+// smaller S' on which the groups that stayed are coupled to their new neighbours: the next level does the same to S', and
+// the dense tiled Cholesky runs on what the last level leaves.  Same array roles as in BBPlan; "keyframe" of a column /
+// of a border entry of a level is a BORDER INDEX OF THE LEVEL BEFORE.
 struct BBLevel2 {
   bool valid = false;
   int n_int = 0, n_seg = 0, n_bord = 0, max_nb = 0, max_len = 0, npadB = 0;
@@ -87,7 +88,9 @@ struct BBLevel2 {
 
 struct BBPlan {
   bool ready = false, valid = false;
-  BBLevel2 l2;
+  static constexpr int kMaxLevels = 3;   // further levels behind the first (each eliminates an independent set of the separator groups left)
+  BBLevel2 lv[kMaxLevels];
+  int n_lv = 0;
   int n_int = 0, n_seg = 0, n_bord = 0, max_nb = 0, max_len = 0;
   int npadB = 0;                  // padded size of the border system (multiple of kNB), 0 if no border
   size_t col_doubles = 0;         // doubles of all interior block columns
@@ -198,7 +201,7 @@ cudaError_t launch_solve(Ctx* c);                        // kernels 3+4: tile as
 bool build_plan(Ctx* c, bool dense, SolvePlan& plan, std::string& err);   // host symbolic factorisation + upload
 void free_plan(SolvePlan& plan);
 bool build_dense_plan(int nb, SolvePlan& plan, cudaStream_t stream, std::string& err);   // every lower tile of an nb x nb tile grid
-bool build_bb_plan(Ctx* c, std::string& err);          // host band + border analysis + upload; plan_bb.valid says whether it applies
+bool build_bb_plan(Ctx* c, std::string& err, int lmax_hint = 0);          // host band + border analysis + upload; plan_bb.valid says whether it applies
 void free_bb_plan(BBPlan& plan);
 cudaError_t launch_solve_bb(Ctx* c);                     // kernels 3+4, band + border variant (solver mode 2)
 cudaError_t launch_retract(Ctx* c);                      // kernel 5

@@ -307,6 +307,31 @@ def test_solver_modes_agree(k, monkeypatch):
         assert np.array_equal(taus[tag], taus[same]), tag          # the grid size does not change the order of any sum
 
 
+def test_band_border_plan_on_a_very_long_chain():
+    """12000 keyframes in one chain (tiny images): at the default segment length the cuts would put more than 292 keyframes on
+    the border; the plan then takes longer segments instead of giving up on the band + border solve, further levels take the
+    separator groups out again, and Gauss-Newton steps on it run in one attempt with a falling cost."""
+    spec = CONFIGS[5].scaled(name="chain12000", kf_per_agent=12000, height=6, width=8, n_scene=4_000, loop_every=0, p_out=0.05)
+    g = make_graph(spec)
+    prm = oracle_params("config", lm_lambda=1e-3)
+    ba = make_solver(g, prm)
+    info = ba.bb_info()
+    assert info["valid"] == 1 and 7 * info["n_border"] <= 2048
+    assert info["max_segment"] > int(0.9 * np.sqrt(g.n_kf - 1) + 0.5)            # the segments were lengthened
+    assert info["n_groups_level2"] > 0 and info["n_border_dense"] < info["n_border"]
+    set_poses(ba, g.poses_init)
+    costs = []
+    for _ in range(3):
+        ba.build_system()
+        ba.solve()
+        tau, attempts, _, cost = ba.update()
+        assert attempts == 1 and bool(np.isfinite(tau.cpu().numpy()).all())
+        costs.append(cost)
+        ba.retract()
+    assert costs[2] < costs[1] < costs[0], costs
+    ba.close()
+
+
 def test_band_border_zero_information_keyframe_and_all_attempts_fail():
     """A keyframe none of whose edges has a valid match has a zero diagonal block: with eps0 > 0 its update is 0 and the
     rest matches the oracle; with eps0 = 0 every attempt meets a zero pivot -> tau = 0, attempts = max."""
