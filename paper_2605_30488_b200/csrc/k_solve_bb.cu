@@ -136,21 +136,20 @@ __device__ void bb_assemble(const BBArgs& a, double eps, int G) {
 }
 
 // ---- phase 2b: the columns of the second level, read out of S (the level-1 border system after the Schur rows) ----------
-// a2's "keyframes" are level-1 border indices.  Column c of a2 = separator keyframe b: D = S(b, b) (the lower triangle of
+// a2's "keyframes" are border indices of the level before (a).  Column c of a2 = separator keyframe b: D = S(b, b) (the lower triangle of
 // S is the valid one), band block t = S(b', b) for the next members b' of the same group, border block q = S(q, b) -- or
 // S(b, q)^T where q precedes b in S -- and the right-hand side b_B(b); then the dense system of the keyframes that stay.
-__device__ void bb_assemble2(const BBArgs& a, const BBArgs& a2, int G) {
+// the columns of group s of a2, by the calling CTA (which then eliminates them: no grid barrier in between)
+__device__ void bb_assemble2_cols(const BBArgs& a, const BBArgs& a2, int s) {
   const int tid = threadIdx.x;
   const size_t nB = (size_t)a.npadB;
   const double* S = a.B.L;
-  for (int c = blockIdx.x; c < a2.n_int; c += G) {
+  const int last = a2.seg_ptr[s + 1] - 1;                     // last column of the group
+  const int32_t* sb = a2.seg_bord + a2.seg_bptr[s];
+  for (int c = a2.seg_ptr[s]; c <= last; ++c) {
     const int nb = a2.col_nb[c];
     const int nel = (1 + kBand + nb) * 49 + 7;
     const int b = a2.col_kf[c];
-    int s = 0;
-    while (a2.seg_ptr[s + 1] <= c) ++s;
-    const int last = a2.seg_ptr[s + 1] - 1;                   // last column of the group
-    const int32_t* sb = a2.seg_bord + a2.seg_bptr[s];
     double* col = a2.colbuf + a2.col_ofs[c];
     for (int idx = tid; idx < nel; idx += kSolveThreads) {
       const int blk = idx / 49, e = idx - blk * 49, r = e / 7, cc = e - r * 7;
@@ -160,7 +159,7 @@ __device__ void bb_assemble2(const BBArgs& a, const BBArgs& a2, int G) {
       } else if (blk <= kBand) {
         if (c + blk <= last) v = __ldcg(S + (size_t)(7 * a2.col_kf[c + blk] + r) * nB + 7 * b + cc);
       } else if (blk < 1 + kBand + nb) {
-        const int q = a2.bord_kf[sb[blk - 1 - kBand]];        // level-1 index of the level-2 border keyframe
+        const int q = a2.bord_kf[sb[blk - 1 - kBand]];        // index, in the level before, of this level's border keyframe
         v = (q > b) ? __ldcg(S + (size_t)(7 * q + r) * nB + 7 * b + cc) : __ldcg(S + (size_t)(7 * b + cc) * nB + 7 * q + r);
       } else {
         v = __ldcg(a.B.rhs + 7 * b + e);
@@ -168,6 +167,14 @@ __device__ void bb_assemble2(const BBArgs& a, const BBArgs& a2, int G) {
       col[idx] = v;
     }
   }
+  __syncthreads();                                            // the CTA's own cp.async reads follow
+}
+
+// the border system of a2 before its Schur rows: the blocks of S between the keyframes that stay (all CTAs)
+__device__ void bb_assemble2_rest(const BBArgs& a, const BBArgs& a2, int G) {
+  const int tid = threadIdx.x;
+  const size_t nB = (size_t)a.npadB;
+  const double* S = a.B.L;
   const int nB2 = a2.npadB, n72 = 7 * a2.n_bord;
   for (long long idx = (long long)blockIdx.x * kSolveThreads + tid; idx < (long long)nB2 * nB2; idx += (long long)G * kSolveThreads) {
     const int R = (int)(idx / nB2), C = (int)(idx - (long long)R * nB2);
@@ -633,9 +640,11 @@ k_solve_bb(const __grid_constant__ BBArgs a, const __grid_constant__ BBLevels L)
       const BBArgs* prev = &a;
       for (int k = 0; k < L.n && !failed; ++k) {              // further levels: groups out of the border system of the level before
         const BBArgs& cur = L.lv[k];
-        bb_assemble2(*prev, cur, G);
-        grid_barrier(a.bar, G, gen);
-        for (int s = blockIdx.x; s < cur.n_seg; s += G) bb_segment(cur, win, brhs, ss, s);
+        bb_assemble2_rest(*prev, cur, G);
+        for (int s = blockIdx.x; s < cur.n_seg; s += G) {
+          bb_assemble2_cols(*prev, cur, s);
+          bb_segment(cur, win, brhs, ss, s);
+        }
         grid_barrier(a.bar, G, gen);
         failed = ld_flag(a.status) != 0;
         if (!failed && cur.n_bord > 0) {
